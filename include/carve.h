@@ -1,0 +1,151 @@
+/*
+ * carve.h -- C ABI of the B200 (sm_100a) CARVE layer operator.
+ *
+ * The operator is the chunk-parallel key-axis-gated delta rule of arxiv/paper_2606_27229
+ * (/root/reference/PAPER.md, cited below as "P l.<line>"), forward and backward, for every
+ * (batch, head) chain independently:
+ *
+ *   for each chunk c of L tokens, with S = state entering the chunk (S_{c-1}):
+ *     q^ = q/sqrt(|q|^2+eps), k^ likewise                      (Fig. 2, P l.437; Alg. 3 step 3, P l.399)
+ *     g_t = -exp(A) . softplus(f_t + tau)                      (Eq. 9,  P l.151)
+ *     G   = [U_b;U_w] S ; t_t = tanh(G q^_t)                    (Eq. 7,  P l.134)  folded state readout
+ *     b_t = sigmoid(bx_t + V_b t_t^(b)),  w_t = sigmoid(wx_t + V_w t_t^(w))      (Eq. 8,  P l.140)
+ *     gamma_t = prod_{s<=t} exp(g_s).(1-b_s)                   (Eq. 14, P l.310)
+ *     A_ts = sum_j k^_t k^_s gamma_{t-1}/gamma_s (s<t)          (Eq. 15, P l.342, Eq. 5 indices)
+ *     (I + diag(beta) A) U = diag(beta) (w.v - K~ S^T),  K~_t = k^_t.gamma_{t-1}     (Alg. 2 steps 5-7, P l.333-352)
+ *     o_t = scale [ S (gamma_t.q^_t) + sum_{s<=t} u_s sum_j q^_t k^_s gamma_t/gamma_s ]   (Alg. 2 step 8, P l.354)
+ *     S  <- S diag(gamma_{L-1}) + sum_t u_t (k^_t.gamma_{L-1}/gamma_t)^T            (Alg. 2 step 9, P l.361)
+ *
+ *   which equals, token by token (Eq. 5, P l.108, with the gates frozen at the chunk boundary):
+ *     u_t = beta_t (w_t.v_t - S_{t-1} k^_t);  S_t = S_{t-1} diag(exp(g_t).(1-b_t)) + u_t k^_t^T;  o_t = scale S_t q^_t.
+ *
+ *   carve_bwd is the adjoint of that map (Alg. 4-5, P l.788-863).  DESIGN.md lists the readings of
+ *   the paper taken where it is ambiguous (write gate on v only, the scalar beta, the Eq. 5 order).
+ *
+ * Conventions
+ *   - Every tensor pointer of carve_fwd / carve_bwd is a DEVICE pointer owned by the caller; the
+ *     library allocates nothing and keeps no global state.  carve_fwd_bwd_host takes HOST pointers
+ *     for the tensors and one caller-owned DEVICE arena.
+ *   - Row-major, innermost dimension contiguous.  Token tensors are [B,T,H,d] (P l.125); the state is
+ *     [B,H,dv,dk] (P l.11).  Base pointers must be 16-byte aligned.
+ *   - `dtype` is the element type of the token tensors q,k,v,f,bx,wx,beta,O and of their gradients
+ *     (CARVE_F32: float, CARVE_BF16: __nv_bfloat16 bits).  A, tau, U_b, U_w, V_b, V_w, S0, S_final and
+ *     their gradients are always float.  All arithmetic on the state is fp32.
+ *   - Calls are asynchronous on `cuda_stream` (a cudaStream_t passed as void*, NULL = default
+ *     stream) and return after enqueueing.  Argument errors are detected on the host before any
+ *     launch and leave all outputs untouched.  Gradients are OVERWRITTEN, not accumulated.
+ *   - Results are run-to-run bitwise deterministic (no floating-point atomics).
+ *   - Supported: T % L == 0, L in {16,32,64,128}; dk, dv in {64,128,256} with dk*dv <= 32768;
+ *     r in {8,16,32}.  carve_bwd additionally needs dk*dv <= 16384.  Anything else returns
+ *     CARVE_ERR_SHAPE: there is no fallback path of any kind.
+ */
+#ifndef CARVE_H_
+#define CARVE_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    CARVE_OK = 0,
+    CARVE_ERR_NULL = 1,      /* a required pointer is NULL */
+    CARVE_ERR_SHAPE = 2,     /* unsupported B,H,T,L,dk,dv,r combination */
+    CARVE_ERR_DTYPE = 3,     /* dtype is neither CARVE_F32 nor CARVE_BF16 */
+    CARVE_ERR_ALIGN = 4,     /* a base pointer is not 16-byte aligned */
+    CARVE_ERR_WORKSPACE = 5, /* workspace missing or smaller than carve_workspace_bytes() */
+    CARVE_ERR_ARCH = 6,      /* current device is not compute capability 10.x */
+    CARVE_ERR_CUDA = 7       /* a CUDA runtime call failed (launch, attribute, copy) */
+} carve_status_t;
+
+typedef enum { CARVE_F32 = 0, CARVE_BF16 = 1 } carve_dtype_t;
+
+/* Kernel family.  AUTO picks TENSOR for bf16 shapes it supports and SIMT otherwise. */
+typedef enum { CARVE_PATH_AUTO = 0, CARVE_PATH_SIMT = 1, CARVE_PATH_TENSOR = 2 } carve_path_t;
+
+typedef struct {
+    int B, H, T;          /* batch, heads, tokens per sequence */
+    int L;                /* chunk length: the gates of a chunk read the state at its start (P l.136) */
+    int dk, dv, r;        /* key dim, value dim, gate bottleneck rank */
+    int dtype;            /* carve_dtype_t */
+    int qk_l2norm;        /* 1: L2-normalise q,k inside and differentiate through it; 0: use as given */
+    float scale;          /* multiplies O (the paper is silent; 1.0f) */
+    float eps;            /* inside the sqrt of the L2 norm (1e-6f) */
+    int path;             /* carve_path_t */
+} carve_params_t;
+
+/* Bytes of device workspace carve_fwd needs to save what carve_bwd reads (need_bwd != 0), or 0. */
+size_t carve_workspace_bytes(const carve_params_t *p, int need_bwd);
+
+/*
+ * Forward (Alg. 1-3, P l.160-196, l.315-365, l.395-409).
+ *   q,k   [B,T,H,dk] dtype      v   [B,T,H,dv] dtype
+ *   f,bx  [B,T,H,dk] dtype      decay logits, erase pre-activation (Eq. 6 ff., P l.128)
+ *   wx    [B,T,H,dv] dtype      write pre-activation
+ *   beta  [B,T,H]    dtype      write strength in [0,1], already activated
+ *   A,tau [H,dk] float          Eq. 9 parameters; either may be NULL (= 0)
+ *   Ub,Uw [r,dv] float          down-projections W_{U1,b}, W_{U1,w} (Eq. 7), shared by all heads
+ *   Vb [dk,r], Vw [dv,r] float  up-projections W_{U2,b}, W_{U2,w} (Eq. 8)
+ *   S0    [B,H,dv,dk] float     initial state, NULL = zeros
+ *   O     [B,T,H,dv] dtype      out
+ *   S_final [B,H,dv,dk] float   out
+ *   workspace                   NULL: inference, nothing saved.  Otherwise >= carve_workspace_bytes(p,1)
+ *                               bytes; it is filled for the matching carve_bwd call.
+ */
+carve_status_t carve_fwd(const carve_params_t *p, const void *q, const void *k, const void *v,
+                         const void *f, const void *bx, const void *wx, const void *beta,
+                         const float *A, const float *tau, const float *Ub, const float *Uw,
+                         const float *Vb, const float *Vw, const float *S0, void *O, float *S_final,
+                         void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/*
+ * Backward (Alg. 4-5, P l.788-863): adjoint of carve_fwd for the cotangents dO and dS_final.
+ * Same inputs as the carve_fwd call that filled `workspace`, plus
+ *   dO [B,T,H,dv] dtype;  dS_final [B,H,dv,dk] float, NULL = zeros.
+ * Outputs (overwritten): dq,dk,df,dbx [B,T,H,dk] dtype; dv,dwx [B,T,H,dv] dtype; dbeta [B,T,H] dtype;
+ *   dA,dtau [H,dk] float (either may be NULL to skip); dUb,dUw [r,dv]; dVb [dk,r]; dVw [dv,r];
+ *   dS0 [B,H,dv,dk] float.
+ */
+carve_status_t carve_bwd(const carve_params_t *p, const void *q, const void *k, const void *v,
+                         const void *f, const void *bx, const void *wx, const void *beta,
+                         const float *A, const float *tau, const float *Ub, const float *Uw,
+                         const float *Vb, const float *Vw, const float *S0, const void *dO,
+                         const float *dS_final, void *dq, void *dk, void *dv, void *df, void *dbx,
+                         void *dwx, void *dbeta, float *dA, float *dtau, float *dUb, float *dUw,
+                         float *dVb, float *dVw, float *dS0, void *workspace, size_t workspace_bytes,
+                         void *cuda_stream);
+
+/* Bytes of device arena carve_fwd_bwd_host needs (device copies of every tensor + workspace). */
+size_t carve_host_arena_bytes(const carve_params_t *p, int with_bwd);
+
+/*
+ * One forward (+ backward when with_bwd != 0) with HOST tensors: copies the inputs to the device
+ * arena, runs carve_fwd (and carve_bwd with the host cotangents dO, dS_final), copies O, S_final
+ * and the gradients back, all enqueued on `cuda_stream`.  Host buffers should be pinned for the
+ * copies to be asynchronous.  Pointer meanings and NULL rules are those of carve_fwd / carve_bwd;
+ * when with_bwd == 0 the cotangent and gradient pointers are ignored.
+ */
+carve_status_t carve_fwd_bwd_host(const carve_params_t *p, int with_bwd, const void *q, const void *k,
+                                  const void *v, const void *f, const void *bx, const void *wx,
+                                  const void *beta, const float *A, const float *tau, const float *Ub,
+                                  const float *Uw, const float *Vb, const float *Vw, const float *S0,
+                                  void *O, float *S_final, const void *dO, const float *dS_final,
+                                  void *dq, void *dk, void *dv, void *df, void *dbx, void *dwx,
+                                  void *dbeta, float *dA, float *dtau, float *dUb, float *dUw,
+                                  float *dVb, float *dVw, float *dS0, void *device_arena,
+                                  size_t arena_bytes, void *cuda_stream);
+
+/* Number of kernel launches carve_fwd / carve_bwd enqueue for these parameters (for accounting). */
+int carve_num_launches(const carve_params_t *p, int bwd);
+
+/* Which kernel family (CARVE_PATH_SIMT / CARVE_PATH_TENSOR) the parameters resolve to, or -1. */
+int carve_resolved_path(const carve_params_t *p, int bwd);
+
+const char *carve_status_string(carve_status_t s);
+const char *carve_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CARVE_H_ */

@@ -1,0 +1,165 @@
+"""Thin Python binding of include/carve.h (ctypes).  Argument marshalling only: every step of
+the operator runs inside csrc/libcarve.so.  There is no fallback of any kind -- if the shared
+library is missing or a call returns a non-zero status this module raises.
+
+Arguments are objects with a `.data_ptr()` method (torch tensors: CUDA tensors for carve_fwd /
+carve_bwd, pinned CPU tensors for carve_fwd_bwd_host), raw integer addresses, or None where the
+header allows NULL.  The caller owns all memory; nothing is allocated here.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "csrc", "libcarve.so")
+
+CARVE_F32, CARVE_BF16 = 0, 1
+CARVE_PATH_AUTO, CARVE_PATH_SIMT, CARVE_PATH_TENSOR = 0, 1, 2
+
+# Every symbol include/carve.h declares (tests check the library exports them all).
+SYMBOLS = ("carve_workspace_bytes", "carve_fwd", "carve_bwd", "carve_host_arena_bytes", "carve_fwd_bwd_host",
+           "carve_num_launches", "carve_resolved_path", "carve_status_string", "carve_version")
+
+
+class CarveError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"carve status {status}: {msg}")
+        self.status = status
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [("B", ctypes.c_int), ("H", ctypes.c_int), ("T", ctypes.c_int), ("L", ctypes.c_int),
+                ("dk", ctypes.c_int), ("dv", ctypes.c_int), ("r", ctypes.c_int), ("dtype", ctypes.c_int),
+                ("qk_l2norm", ctypes.c_int), ("scale", ctypes.c_float), ("eps", ctypes.c_float),
+                ("path", ctypes.c_int)]
+
+
+@dataclass
+class Params:
+    B: int
+    H: int
+    T: int
+    L: int
+    dk: int
+    dv: int
+    r: int
+    dtype: int = CARVE_BF16
+    qk_l2norm: int = 1
+    scale: float = 1.0
+    eps: float = 1e-6
+    path: int = CARVE_PATH_AUTO
+
+    def c(self) -> _Params:
+        return _Params(self.B, self.H, self.T, self.L, self.dk, self.dv, self.r, self.dtype, self.qk_l2norm,
+                       self.scale, self.eps, self.path)
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen csrc/libcarve.so (built by `python -m paper_2606_27229_b200.build`); raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_2606_27229_b200.build` "
+                "(there is no CPU or PyTorch fallback)")
+        lib = ctypes.CDLL(LIB_PATH)
+        vp, sz, ci = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int
+        pp = ctypes.POINTER(_Params)
+        lib.carve_workspace_bytes.restype = sz
+        lib.carve_workspace_bytes.argtypes = [pp, ci]
+        lib.carve_host_arena_bytes.restype = sz
+        lib.carve_host_arena_bytes.argtypes = [pp, ci]
+        lib.carve_num_launches.restype = ci
+        lib.carve_num_launches.argtypes = [pp, ci]
+        lib.carve_resolved_path.restype = ci
+        lib.carve_resolved_path.argtypes = [pp, ci]
+        lib.carve_status_string.restype = ctypes.c_char_p
+        lib.carve_status_string.argtypes = [ci]
+        lib.carve_version.restype = ctypes.c_char_p
+        lib.carve_fwd.restype = ci
+        lib.carve_fwd.argtypes = [pp] + [vp] * 16 + [vp, sz, vp]
+        lib.carve_bwd.restype = ci
+        lib.carve_bwd.argtypes = [pp] + [vp] * 30 + [vp, sz, vp]
+        lib.carve_fwd_bwd_host.restype = ci
+        lib.carve_fwd_bwd_host.argtypes = [pp, ci] + [vp] * 32 + [vp, sz, vp]
+        _lib = lib
+    return _lib
+
+
+def _ptr(x):
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return ctypes.c_void_p(x)
+    return ctypes.c_void_p(x.data_ptr())
+
+
+def _nbytes(x) -> int:
+    return 0 if x is None else x.numel() * x.element_size()
+
+
+def _check(status: int):
+    if status != 0:
+        raise CarveError(status, load_library().carve_status_string(status).decode())
+
+
+def carve_version() -> str:
+    return load_library().carve_version().decode()
+
+
+def carve_workspace_bytes(p: Params, need_bwd: bool = True) -> int:
+    cp = p.c()
+    return int(load_library().carve_workspace_bytes(ctypes.byref(cp), int(need_bwd)))
+
+
+def carve_host_arena_bytes(p: Params, with_bwd: bool = True) -> int:
+    cp = p.c()
+    return int(load_library().carve_host_arena_bytes(ctypes.byref(cp), int(with_bwd)))
+
+
+def carve_num_launches(p: Params, bwd: bool) -> int:
+    cp = p.c()
+    return int(load_library().carve_num_launches(ctypes.byref(cp), int(bwd)))
+
+
+def carve_resolved_path(p: Params, bwd: bool) -> int:
+    cp = p.c()
+    return int(load_library().carve_resolved_path(ctypes.byref(cp), int(bwd)))
+
+
+_FWD_IN = ("q", "k", "v", "f", "bx", "wx", "beta", "A", "tau", "Ub", "Uw", "Vb", "Vw", "S0")
+_GRADS = ("dq", "dk", "dv", "df", "dbx", "dwx", "dbeta", "dA", "dtau", "dUb", "dUw", "dVb", "dVw", "dS0")
+
+
+def carve_fwd(p: Params, x: dict, O, S_final, workspace=None, stream: int = 0) -> None:
+    """carve_fwd of carve.h.  `x` maps the names q,k,v,f,bx,wx,beta,A,tau,Ub,Uw,Vb,Vw,S0 to device
+    tensors (A, tau, S0 may be None); O, S_final are written; workspace (a device byte tensor of
+    carve_workspace_bytes(p) bytes) is filled for carve_bwd, or None for inference."""
+    cp = p.c()
+    _check(load_library().carve_fwd(ctypes.byref(cp), *[_ptr(x.get(n)) for n in _FWD_IN], _ptr(O), _ptr(S_final),
+                                    _ptr(workspace), _nbytes(workspace), ctypes.c_void_p(stream)))
+
+
+def carve_bwd(p: Params, x: dict, dO, dS_final, grads: dict, workspace, stream: int = 0) -> None:
+    """carve_bwd of carve.h.  `grads` maps dq,dk,dv,df,dbx,dwx,dbeta,dA,dtau,dUb,dUw,dVb,dVw,dS0 to
+    preallocated device tensors (dA, dtau may be None); they are overwritten."""
+    cp = p.c()
+    _check(load_library().carve_bwd(ctypes.byref(cp), *[_ptr(x.get(n)) for n in _FWD_IN], _ptr(dO), _ptr(dS_final),
+                                    *[_ptr(grads.get(n)) for n in _GRADS], _ptr(workspace), _nbytes(workspace),
+                                    ctypes.c_void_p(stream)))
+
+
+def carve_fwd_bwd_host(p: Params, with_bwd: bool, x: dict, O, S_final, dO, dS_final, grads: dict, arena,
+                       stream: int = 0) -> None:
+    """carve_fwd_bwd_host of carve.h: all tensors are HOST (pinned) tensors, `arena` is a device byte
+    tensor of carve_host_arena_bytes(p, with_bwd) bytes."""
+    cp = p.c()
+    g = grads or {}
+    _check(load_library().carve_fwd_bwd_host(
+        ctypes.byref(cp), int(with_bwd), *[_ptr(x.get(n)) for n in _FWD_IN], _ptr(O), _ptr(S_final), _ptr(dO),
+        _ptr(dS_final), *[_ptr(g.get(n)) for n in _GRADS], _ptr(arena), _nbytes(arena), ctypes.c_void_p(stream)))

@@ -1,0 +1,70 @@
+// Internal declarations shared by the translation units of libcarve.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "carve.h"
+
+namespace carve {
+
+// Everything a kernel needs, passed by value.
+struct Args {
+    int B, H, T, L, dk, dv, r;
+    int l2norm;
+    float scale, eps;
+    // forward inputs
+    const void *q, *k, *v, *f, *bx, *wx, *beta;
+    const float *A, *tau, *Ub, *Uw, *Vb, *Vw, *S0;
+    // forward outputs
+    void* O;
+    float* S_final;
+    // backward inputs / outputs
+    const void* dO;
+    const float* dS_final;
+    void *dq, *dk_, *dv_, *df, *dbx, *dwx, *dbeta;
+    float* dS0;
+    // workspace views (nullptr in inference forward)
+    float* ws_states;  // [chains][T/LS][dv][dk]   state entering every solve sub-chunk
+    float* ws_E;       // [B,T,H,dv]               pre-beta error e_t (u_t = beta_t e_t)
+    float* ws_tt;      // [B,T,H,2r]               tanh bottleneck
+    float* ws_G;       // [chains][T/L][2r][dk]    folded readout of every gate chunk
+    float* ws_part;    // [chains][part_stride]    per-chain partial weight gradients
+    int part_stride;
+};
+
+// Workspace layout (in floats) for the SIMT path; `total` in bytes.
+struct WsLayout {
+    size_t states, E, tt, G, part, total_bytes;
+    int part_stride;
+};
+
+constexpr int kSimtSub = 16;  // solve sub-chunk of the SIMT path (tokens)
+
+inline int part_stride_of(int dk, int dv, int r) { return 2 * r * dv + dk * r + dv * r + 2 * dk; }
+
+inline WsLayout simt_ws_layout(const carve_params_t& p)
+{
+    WsLayout w{};
+    const size_t chains = (size_t)p.B * p.H, tok = chains * p.T;
+    size_t off = 0;
+    auto take = [&](size_t n) { size_t o = off; off += (n + 3) & ~(size_t)3; return o; };
+    w.states = take(chains * (p.T / kSimtSub) * p.dv * p.dk);
+    w.E = take(tok * p.dv);
+    w.tt = take(tok * 2 * p.r);
+    w.G = take(chains * (p.T / p.L) * 2 * p.r * p.dk);
+    w.part_stride = part_stride_of(p.dk, p.dv, p.r);
+    w.part = take(chains * (size_t)w.part_stride);
+    w.total_bytes = off * sizeof(float);
+    return w;
+}
+
+// SIMT path (carve_simt.cu).  Return cudaSuccess or the failing CUDA error.
+size_t simt_fwd_smem_bytes(int dk, int dv, int r);
+size_t simt_bwd_smem_bytes(int dk, int dv, int r);
+cudaError_t simt_fwd_launch(const Args& a, int dtype, cudaStream_t st);
+cudaError_t simt_bwd_launch(const Args& a, int dtype, float* dA, float* dtau, float* dUb, float* dUw,
+                            float* dVb, float* dVw, cudaStream_t st);
+
+}  // namespace carve

@@ -1,0 +1,150 @@
+"""GPU parity: the CUDA path (through the C ABI) vs the fp64 oracle, element by element, on the
+same seeded inputs.  Tolerances are north_star's: max|x-ref|/max|ref| <= 1e-4 for fp32 inputs;
+<= 2e-2 on O (and S_final) and <= 3e-2 on every gradient for bf16 inputs with fp32 state.
+"""
+import numpy as np
+import pytest
+
+from paper_2606_27229_b200 import carve, synth
+from tests.gpu_util import GRADS, oracle_shape, params_of, relerr, run_bwd, run_fwd
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f32": dict(O=1e-4, S=1e-4, g=1e-4), "bf16": dict(O=2e-2, S=2e-2, g=3e-2)}
+
+
+def _check_fwd_bwd(oracle, cfg, x, with_bwd=True, path=carve.CARVE_PATH_AUTO, ct=None):
+    p = params_of(cfg, path=path)
+    s = oracle_shape(oracle, cfg)
+    O_ref, S_ref = oracle.fwd(s, x)
+    O, Sf, handles = run_fwd(p, x, need_bwd=with_bwd)
+    tol = TOL[cfg.dtype]
+    errs = {"O": relerr(O, O_ref), "S_final": relerr(Sf, S_ref)}
+    assert np.isfinite(O).all() and np.isfinite(Sf).all()
+    assert errs["O"] <= tol["O"], errs
+    assert errs["S_final"] <= tol["S"], errs
+    if with_bwd:
+        ct = ct or synth.make_cotangents(cfg)
+        g_ref = oracle.bwd(s, x, ct["dO"], ct["dS_final"])
+        g, _ = run_bwd(p, handles, ct)
+        for n in GRADS:
+            if x.get(n[1:]) is None and n in ("dA", "dtau"):
+                pass  # gradients w.r.t. absent A/tau are still defined (they default to 0)
+            assert np.isfinite(g[n]).all(), n
+            errs[n] = relerr(g[n], g_ref[n])
+            assert errs[n] <= tol["g"], (n, errs)
+    return errs
+
+
+# ---- config 0 of BASELINE.json, exactly, plus its U=0 run --------------------------------------
+@pytest.mark.parametrize("zero_content", [False, True])
+@pytest.mark.parametrize("l2norm", [1, 0])
+def test_config0_fp32(oracle, zero_content, l2norm):
+    cfg = synth.CFG0.with_(qk_l2norm=l2norm)
+    x = synth.make_inputs(cfg, zero_content=zero_content)
+    _check_fwd_bwd(oracle, cfg, x)
+
+
+# ---- small cases spanning several sub-chunks, every chunk length, ragged structure -------------
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("L", [16, 32, 64, 128])
+def test_chunk_lengths(oracle, dtype, L):
+    cfg = synth.Config("t", B=2, H=2, T=256, L=L, dk=64, dv=64, r=8, dtype=dtype, wstd=0.1, s0_std=0.05, seed=L)
+    x = synth.make_inputs(cfg, with_decay_params=True)
+    _check_fwd_bwd(oracle, cfg, x)
+
+
+@pytest.mark.parametrize("dk,dv,r", [(128, 128, 16), (64, 128, 8), (128, 64, 32), (64, 256, 16), (256, 64, 8)])
+def test_head_dims_bf16(oracle, dk, dv, r):
+    cfg = synth.Config("t", B=1, H=3, T=128, L=32, dk=dk, dv=dv, r=r, dtype="bf16", wstd=0.1, s0_std=0.02, seed=7)
+    x = synth.make_inputs(cfg)
+    _check_fwd_bwd(oracle, cfg, x)
+
+
+def test_dv256_forward_only(oracle):
+    """dk=128, dv=256 (config 3's head shape) is forward-only: bwd must refuse it, not fall back."""
+    cfg = synth.Config("t", B=1, H=2, T=128, L=64, dk=128, dv=256, r=16, dtype="bf16", s0_std=0.01, seed=5)
+    x = synth.make_inputs(cfg)
+    _check_fwd_bwd(oracle, cfg, x, with_bwd=False)
+    assert carve.carve_workspace_bytes(params_of(cfg), True) == 0
+
+
+def test_single_chunk_and_scale(oracle):
+    cfg = synth.Config("t", B=1, H=1, T=16, L=16, dk=64, dv=64, r=8, dtype="f32", wstd=0.3, s0_std=0.5,
+                       scale=0.125, seed=2)
+    x = synth.make_inputs(cfg, with_decay_params=True)
+    _check_fwd_bwd(oracle, cfg, x)
+
+
+def test_stress_conditioning(oracle):
+    """Config 4's stress structure at small size: beta = 1 on 10 % of tokens, no decay on 10 % of key dims."""
+    cfg = synth.CFG4.with_(B=2, H=2, T=256)
+    x = synth.make_inputs(cfg)
+    _check_fwd_bwd(oracle, cfg, x)
+
+
+def test_extreme_decay_no_overflow(oracle):
+    """Strong decay/erase (log gamma_L ~ -600 per chunk): every ratio is formed as exp(<=0)."""
+    cfg = synth.Config("t", B=1, H=1, T=128, L=64, dk=64, dv=64, r=8, dtype="f32", wstd=0.1, s0_std=0.1, seed=4)
+    x = synth.make_inputs(cfg)
+    x["f"] = x["f"] + 5.0
+    x["bx"] = x["bx"] + 5.0
+    _check_fwd_bwd(oracle, cfg, x)
+
+
+# ---- invariants that need no oracle -------------------------------------------------------------
+def test_split_call_bitwise(oracle):
+    """One call over T == two calls over T/2 with S_final -> S0 (Table 2 l.452), bit for bit."""
+    cfg = synth.Config("t", B=2, H=2, T=256, L=64, dk=64, dv=64, r=8, dtype="bf16", wstd=0.1, seed=9)
+    x = synth.make_inputs(cfg)
+    p = params_of(cfg)
+    O, Sf, _ = run_fwd(p, x)
+    half = cfg.with_(T=128)
+    xa = {n: (a[:, :128] if n in synth.TOKEN_TENSORS else a) for n, a in x.items()}
+    xb = {n: (a[:, 128:] if n in synth.TOKEN_TENSORS else a) for n, a in x.items()}
+    Oa, Sa, _ = run_fwd(params_of(half), xa)
+    xb["S0"] = Sa.astype(np.float32)
+    Ob, Sb, _ = run_fwd(params_of(half), xb)
+    assert np.array_equal(np.concatenate([Oa, Ob], axis=1), O)
+    assert np.array_equal(Sb, Sf)
+
+
+def test_determinism_and_zero_content_grads(oracle):
+    cfg = synth.Config("t", B=2, H=4, T=128, L=32, dk=64, dv=64, r=8, dtype="bf16", seed=12)
+    x = synth.make_inputs(cfg, zero_content=True)
+    ct = synth.make_cotangents(cfg)
+    p = params_of(cfg)
+    outs = []
+    for _ in range(2):
+        O, Sf, h = run_fwd(p, x, need_bwd=True)
+        g, _ = run_bwd(p, h, ct)
+        outs.append((O, Sf, g))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    for n in GRADS:
+        assert np.array_equal(outs[0][2][n], outs[1][2][n]), n
+    for n in ("dUb", "dUw", "dVb", "dVw"):
+        assert np.all(outs[0][2][n] == 0.0), n
+
+
+def test_host_entry_point_matches_device_entry_point(oracle):
+    import torch
+    cfg = synth.Config("t", B=1, H=2, T=128, L=64, dk=64, dv=64, r=8, dtype="bf16", wstd=0.1, seed=21)
+    x = synth.make_inputs(cfg)
+    ct = synth.make_cotangents(cfg)
+    p = params_of(cfg)
+    O, Sf, h = run_fwd(p, x, need_bwd=True)
+    g, _ = run_bwd(p, h, ct)
+    from tests.gpu_util import alloc_grads, to_device
+    xh = {n: (None if t is None else t.pin_memory()) for n, t in to_device(x, torch.bfloat16, "cpu").items()}
+    dOh = to_device({"dO": ct["dO"]}, torch.bfloat16, "cpu")["dO"].pin_memory()
+    dSfh = torch.from_numpy(ct["dS_final"]).pin_memory()
+    Oh = torch.empty(cfg.B, cfg.T, cfg.H, cfg.dv, dtype=torch.bfloat16).pin_memory()
+    Sfh = torch.empty(cfg.B, cfg.H, cfg.dv, cfg.dk, dtype=torch.float32).pin_memory()
+    gh = {n: (None if t is None else t.pin_memory()) for n, t in alloc_grads(p, torch.bfloat16, "cpu").items()}
+    arena = torch.empty(carve.carve_host_arena_bytes(p, True), dtype=torch.uint8, device="cuda")
+    carve.carve_fwd_bwd_host(p, True, xh, Oh, Sfh, dOh, dSfh, gh, arena, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(Oh.float().numpy().astype(np.float64), O)
+    assert np.array_equal(Sfh.numpy().astype(np.float64), Sf)
+    for n in GRADS:
+        assert np.array_equal(gh[n].float().numpy().astype(np.float64), g[n]), n
