@@ -1,0 +1,365 @@
+#!/usr/bin/env python
+"""bench.py -- CARVE layer-operator fwd+bwd throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config cfg1]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: carve_fwd (saving
+for backward) + carve_bwd through the C ABI (paper_2606_27229_b200/csrc/libcarve.so).  The default
+workload is BASELINE.json configs[1] (B=8,H=16,T=4096,L=64,dk=dv=128,r=16, bf16 tokens, fp32 state),
+the shape the metric is quoted on.  Prints ONE JSON line (rank 0):
+  value     tokens/s, inputs resident in HBM, CUDA events on the launching stream, max over ranks
+  e2e       same metric through carve_fwd_bwd_host: pinned HOST buffers, H2D/D2H copies inside the timing
+  roofline  dominant kernel: algorithmic bytes per launch / its event-timed duration vs measured HBM peak
+  cpu_baseline  the fp64 oracle, as it stands, on the host cores, on a bounded sample of the same workload
+With N > 1 (torchrun) every rank runs the same per-GPU workload on its own batch shard (weak scaling:
+chains are independent); the only exchange is one NCCL all-reduce of the shared weight
+gradients (tens of KB) per step.  `--impl reference` times the oracle (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_27229_b200 import synth  # noqa: E402
+
+METRIC = "CARVE layer fwd+bwd tokens/sec"
+PAPER_CONTEXT = ("paper: full-model training throughput 95.52K vs 94.21K tok/s, 1xH100, bf16, Table 3 "
+                 "(captioned 125M/T=1024; not an operator timing, not comparable)")
+
+
+def get_cfg(name: str) -> synth.Config:
+    table = {"cfg0": synth.CFG0, "cfg1": synth.CFG1, "cfg3": synth.CFG3, "cfg4": synth.CFG4}
+    table.update({f"cfg2_L{L}": c for L, c in synth.CFG2.items()})
+    return table[name]
+
+
+# ---- algorithmic bytes / flops -------------------------------
+def algorithmic(cfg: synth.Config):
+    e = 2 if cfg.dtype == "bf16" else 4
+    dk, dv, r, L = cfg.dk, cfg.dv, cfg.r, cfg.L
+    tokh = cfg.B * cfg.T * cfg.H
+    chains = cfg.B * cfg.H
+    n_in = 2 * dk + dv + dk + dk + dv + 1
+    fwd_b = tokh * (e * n_in + e * dv) + chains * 4 * dv * dk * 2
+    bwd_b = tokh * (e * n_in + e * dv + e * n_in) + chains * 4 * dv * dk * 2
+    fwd_f = (4 * r * dv * dk + 4 * L * r * dk + 2 * L * r * (dk + dv) + L * (L - 1) * dk + L * (L + 1) * dk +
+             L * (L - 1) * dv + 3 * 2 * L * dk * dv + L * (L + 1) * dv)
+    fwd_f *= chains * (cfg.T // L)
+    return dict(fwd_bytes=fwd_b, bwd_bytes=0 if cfg.fwd_only else bwd_b, fwd_flops=fwd_f,
+                bwd_flops=0 if cfg.fwd_only else 2 * fwd_f)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), bf16_tflops=float(d["bf16_tflops"]),
+                    bf16_tflops_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), source="measured")
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks/throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc, self.thr = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            return
+        self.thr = threading.Thread(target=lambda: self.rows.extend(self.proc.stdout), daemon=True)
+        self.thr.start()
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.thr.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.rows:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---- CPU oracle leg ------------------------------------------------------------------------------
+def oracle_sample(cfg: synth.Config, x: dict, ct: dict, nchains: int):
+    """The first `nchains` (batch, head) chains of the workload, full T, as a B'=n, H'=1 problem."""
+    chains = [(i // cfg.H, i % cfg.H) for i in range(min(nchains, cfg.B * cfg.H))]
+    xs = synth.slice_chains({k: v for k, v in x.items() if k not in ("A", "tau")}, chains)
+    xs["A"] = xs["tau"] = None
+    cts = synth.slice_chains(ct, chains)
+    return chains, xs, cts
+
+
+def time_oracle(cfg: synth.Config, x: dict, ct: dict, steps: int, warmup: int):
+    from oracle import carve_oracle as orc
+    cores = orc.num_threads()
+    n = min(cfg.B * cfg.H, 2 * cores)
+    chains, xs, cts = oracle_sample(cfg, x, ct, n)
+    s = orc.Shape(B=len(chains), H=1, T=cfg.T, L=cfg.L, dk=cfg.dk, dv=cfg.dv, r=cfg.r,
+                  qk_l2norm=cfg.qk_l2norm, scale=cfg.scale, eps=cfg.eps)
+    times = []
+    for i in range(warmup + steps):
+        t0 = time.perf_counter()
+        orc.fwd(s, xs)
+        if not cfg.fwd_only:
+            orc.bwd(s, xs, cts["dO"], cts["dS_final"])
+        if i >= warmup:
+            times.append(time.perf_counter() - t0)
+    tok_equiv = len(chains) * cfg.T / cfg.H   # a token carries all H heads; the sample holds n of B*H chains
+    sec = sum(times) / len(times)
+    return dict(value=tok_equiv / sec, unit="tokens/s", cores=cores, kind="oracle",
+                sample=f"{len(chains)} of {cfg.B * cfg.H} (batch,head) chains of {cfg.name}, full T={cfg.T}, "
+                       f"fp64 oracle fwd{'' if cfg.fwd_only else '+bwd'}, {sec:.2f} s per step"), sec
+
+
+def base_line(cfg: synth.Config, args, n_gpus: int) -> dict:
+    return {"metric": METRIC, "unit": "tokens/s", "n_gpus": n_gpus, "steps": args.steps, "warmup": args.warmup,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16 tokens, f32 state/accumulate" if cfg.dtype == "bf16" else "f32", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: B={cfg.B} (per GPU),H={cfg.H},T={cfg.T},L={cfg.L},dk={cfg.dk},"
+                                   f"dv={cfg.dv},r={cfg.r},{cfg.dtype},S0={'N(0,%g)' % cfg.s0_std if cfg.s0_std else 0}"
+                                   f"{', fwd only' if cfg.fwd_only else ', fwd+bwd'}",
+                       "seed": cfg.seed, "parallelism": f"dp{n_gpus} over batch (independent chains)",
+                       "l2": "inputs (>=0.8 GB per pass) exceed the 126 MB L2; no explicit flush"},
+            "context": PAPER_CONTEXT}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = get_cfg(args.config)
+    cores = os.cpu_count() or 1
+    n = min(cfg.B * cfg.H, 2 * cores)
+    small = cfg.with_(B=max(1, -(-n // cfg.H)))       # only generate the batches the sample touches
+    x, ct = synth.make_inputs(small), synth.make_cotangents(small)
+    cb, sec = time_oracle(small.with_(name=cfg.name), x, ct, args.steps, min(args.warmup, 1))
+    cb["sample"] = cb["sample"].replace(f"of {small.B * small.H}", f"of {cfg.B * cfg.H}")
+    line = base_line(cfg, args, args.gpus)
+    line.update({"impl": "reference", "value": cb["value"], "ms_per_step": sec * 1e3, "cpu_baseline": cb,
+                 "e2e": {"value": cb["value"], "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                 "gpu_launches": 0, "dtype": "f64"})
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2606_27229_b200 import carve
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the CARVE path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = get_cfg(args.config).with_(seed=rank)       # each rank owns a different batch shard
+    carve.load_library()
+    tok_dt = torch.bfloat16 if cfg.dtype == "bf16" else torch.float32
+    p = carve.Params(B=cfg.B, H=cfg.H, T=cfg.T, L=cfg.L, dk=cfg.dk, dv=cfg.dv, r=cfg.r,
+                     dtype=carve.CARVE_BF16 if cfg.dtype == "bf16" else carve.CARVE_F32,
+                     qk_l2norm=cfg.qk_l2norm, scale=cfg.scale, eps=cfg.eps)
+    with_bwd = not cfg.fwd_only
+
+    # ---- seeded synthetic inputs: host (pinned) and device copies
+    x, ct = synth.make_inputs(cfg), synth.make_cotangents(cfg)
+
+    def host_t(name, a):
+        if a is None:
+            return None
+        t = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32))
+        if name in synth.TOKEN_TENSORS or name == "dO":
+            t = t.to(tok_dt)
+        return t.contiguous().pin_memory()
+
+    xh = {n: host_t(n, a) for n, a in x.items()}
+    dOh, dSfh = host_t("dO", ct["dO"]), host_t("dS_final", ct["dS_final"])
+    xd = {n: (None if t is None else t.cuda()) for n, t in xh.items()}
+    dOd, dSfd = dOh.cuda(), dSfh.cuda()
+    dev = torch.device("cuda", local)
+    O = torch.empty(cfg.B, cfg.T, cfg.H, cfg.dv, dtype=tok_dt, device=dev)
+    Sf = torch.empty(cfg.B, cfg.H, cfg.dv, cfg.dk, dtype=torch.float32, device=dev)
+    wgrad = torch.zeros(2 * cfg.r * cfg.dv + cfg.dk * cfg.r + cfg.dv * cfg.r + 2 * cfg.H * cfg.dk,
+                        dtype=torch.float32, device=dev)     # packed weight grads: one all-reduce buffer
+
+    def mk_grads(device, pin=False):
+        B, H, T, dk, dv, r = cfg.B, cfg.H, cfg.T, cfg.dk, cfg.dv, cfg.r
+        mk = lambda dt, *s: (torch.empty(*s, dtype=dt).pin_memory() if pin else torch.empty(*s, dtype=dt, device=device))
+        g = {"dq": mk(tok_dt, B, T, H, dk), "dk": mk(tok_dt, B, T, H, dk), "dv": mk(tok_dt, B, T, H, dv),
+             "df": mk(tok_dt, B, T, H, dk), "dbx": mk(tok_dt, B, T, H, dk), "dwx": mk(tok_dt, B, T, H, dv),
+             "dbeta": mk(tok_dt, B, T, H), "dS0": mk(torch.float32, B, H, dv, dk)}
+        if pin:
+            g.update({"dUb": mk(torch.float32, r, dv), "dUw": mk(torch.float32, r, dv),
+                      "dVb": mk(torch.float32, dk, r), "dVw": mk(torch.float32, dv, r),
+                      "dA": mk(torch.float32, H, dk), "dtau": mk(torch.float32, H, dk)})
+        else:
+            o = 0
+            for n, shp in (("dUb", (r, dv)), ("dUw", (r, dv)), ("dVb", (dk, r)), ("dVw", (dv, r)),
+                           ("dA", (H, dk)), ("dtau", (H, dk))):
+                k = shp[0] * shp[1]
+                g[n] = wgrad[o:o + k].view(*shp)
+                o += k
+        return g
+
+    grads = mk_grads(dev) if with_bwd else None
+    ws = torch.empty(carve.carve_workspace_bytes(p, True), dtype=torch.uint8, device=dev) if with_bwd else None
+    stream = torch.cuda.current_stream()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step(evs=None):
+        if evs: evs[0].record(stream)
+        carve.carve_fwd(p, xd, O, Sf, ws, stream.cuda_stream)
+        if evs: evs[1].record(stream)
+        if with_bwd:
+            carve.carve_bwd(p, xd, dOd, dSfd, grads, ws, stream.cuda_stream)
+            if evs: evs[2].record(stream)
+            if world > 1:
+                dist.all_reduce(wgrad)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    kev = [[ev(), ev(), ev()] for _ in range(args.steps)]
+    t_begin, t_end = ev(), ev()
+    barrier()
+    t_begin.record(stream)
+    for i in range(args.steps):
+        step(kev[i])
+    t_end.record(stream)
+    barrier()
+    ms_total = t_begin.elapsed_time(t_end)
+    clocks = sampler.stop() if rank == 0 else None
+    fwd_ms = statistics.mean(k[0].elapsed_time(k[1]) for k in kev)
+    bwd_ms = statistics.mean(k[1].elapsed_time(k[2]) for k in kev) if with_bwd else 0.0
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    tokens_job = cfg.tokens * world
+    value = tokens_job / (ms_step * 1e-3)
+
+    # ---- e2e: the host-buffer C-ABI call, copies inside the timed region
+    Oh = torch.empty(cfg.B, cfg.T, cfg.H, cfg.dv, dtype=tok_dt).pin_memory()
+    Sfh = torch.empty(cfg.B, cfg.H, cfg.dv, cfg.dk, dtype=torch.float32).pin_memory()
+    gh = mk_grads("cpu", pin=True) if with_bwd else None
+    del ws
+    arena = torch.empty(carve.carve_host_arena_bytes(p, with_bwd), dtype=torch.uint8, device=dev)
+    nb = lambda t: 0 if t is None else t.numel() * t.element_size()
+    h2d = sum(nb(t) for t in xh.values()) + (nb(dOh) + nb(dSfh) if with_bwd else 0)
+    d2h = nb(Oh) + nb(Sfh) + (sum(nb(t) for t in gh.values()) if with_bwd else 0)
+    e2e_steps = max(1, min(args.steps, 5))
+
+    def e2e_step():
+        carve.carve_fwd_bwd_host(p, with_bwd, xh, Oh, Sfh, dOh if with_bwd else None, dSfh if with_bwd else None,
+                                 gh, arena, stream.cuda_stream)
+    e2e_step()
+    barrier()
+    e0, e1 = ev(), ev()
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    e2e_ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_value = tokens_job / (e2e_ms / e2e_steps * 1e-3)
+
+    if rank == 0:
+        alg = algorithmic(cfg)
+        peaks = load_peaks()
+        dom = "bwd" if (with_bwd and bwd_ms >= fwd_ms) else "fwd"
+        dom_ms = bwd_ms if dom == "bwd" else fwd_ms
+        dom_bytes = alg[f"{dom}_bytes"]
+        achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
+        t_hbm = (alg["fwd_bytes"] + alg["bwd_bytes"]) / (peaks["hbm_gbs"] * 1e9)
+        t_tc = (alg["fwd_flops"] + alg["bwd_flops"]) / (peaks["bf16_tflops"] * 1e12)
+        path = carve.carve_resolved_path(p, with_bwd)
+        line = base_line(cfg, args, world)
+        line.update({
+            "value": value, "ms_per_step": ms_step, "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": "tokens/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+            "gpu_launches": args.steps * (carve.carve_num_launches(p, False) +
+                                          (carve.carve_num_launches(p, True) if with_bwd else 0)),
+            "kernel_path": {1: "simt-fp32", 2: "tensor-tcgen05"}.get(path, str(path)),
+            "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
+            "roofline": {"bound": "hbm", "kernel": f"carve_{dom}", "achieved": achieved, "peak": peaks["hbm_gbs"],
+                         "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"], "traffic": None,
+                         "peak_source": f"{peaks['source']} (MEASURED_PEAKS.json hbm_gbs)" if peaks["source"] == "measured"
+                         else "fallback 6650 GB/s",
+                         "algorithmic_bytes_per_launch": dom_bytes},
+            "layer_roofline": {"t_hbm_ms": t_hbm * 1e3, "t_tensor_ms": t_tc * 1e3, "binding": "hbm" if t_hbm >= t_tc else "tensor",
+                               "roofline_tokens_per_s": cfg.tokens / max(t_hbm, t_tc),
+                               "frac": max(t_hbm, t_tc) * 1e3 / ms_step,
+                               "algorithmic_bytes": alg["fwd_bytes"] + alg["bwd_bytes"],
+                               "algorithmic_flops": alg["fwd_flops"] + alg["bwd_flops"]},
+        })
+        if world == 1 and not args.no_cpu_baseline:
+            cb, _ = time_oracle(cfg, x, ct, 1, 0)
+            line["cpu_baseline"] = cb
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg1")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

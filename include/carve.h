@@ -36,7 +36,7 @@
  *     launch and leave all outputs untouched.  Gradients are OVERWRITTEN, not accumulated.
  *   - Results are run-to-run bitwise deterministic (no floating-point atomics).
  *   - Supported: T % L == 0, L in {16,32,64,128}; dk, dv in {64,128,256} with dk*dv <= 32768;
- *     r in {8,16,32}.  carve_bwd additionally needs dk*dv <= 16384.  Anything else returns
+ *     r in {8,16,32}.  carve_bwd additionally needs dk*dv <= 16384 and dk <= 128.  Anything else returns
  *     CARVE_ERR_SHAPE: there is no fallback path of any kind.
  */
 #ifndef CARVE_H_
