@@ -36,10 +36,16 @@ carve_status_t check_params(const carve_params_t* p, bool bwd)
     return CARVE_OK;
 }
 
-int resolve_path(const carve_params_t* p, bool /*bwd*/)
+// Kernel family of a call.  `bwd` = the call is carve_bwd or a carve_fwd that saves for it: the two
+// must agree because the workspace layouts differ.  The tensor-core backward does not exist yet, so
+// training calls resolve to SIMT and an explicit CARVE_PATH_TENSOR request for them is refused
+// (no silent substitution).
+int resolve_path(const carve_params_t* p, bool bwd)
 {
-    if (p->path == CARVE_PATH_TENSOR) return -1;  // tensor-core family not built yet: no silent substitution
-    return CARVE_PATH_SIMT;
+    const bool tc_ok = tc_fwd_supported(*p) && !bwd;
+    if (p->path == CARVE_PATH_TENSOR) return tc_ok ? CARVE_PATH_TENSOR : -1;
+    if (p->path == CARVE_PATH_SIMT) return CARVE_PATH_SIMT;
+    return tc_ok ? CARVE_PATH_TENSOR : CARVE_PATH_SIMT;
 }
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -127,7 +133,8 @@ carve_status_t carve_fwd(const carve_params_t* p, const void* q, const void* k, 
                             (const void*)S_final, (const void*)workspace})
         if (!aligned16(ptr)) return CARVE_ERR_ALIGN;
     if (workspace && workspace_bytes < simt_ws_layout(*p).total_bytes) return CARVE_ERR_WORKSPACE;
-    if (resolve_path(p, false) < 0) return CARVE_ERR_SHAPE;
+    const int path = resolve_path(p, workspace != nullptr);
+    if (path < 0) return CARVE_ERR_SHAPE;
     if ((s = check_arch()) != CARVE_OK) return s;
 
     Args a{};
@@ -136,6 +143,8 @@ carve_status_t carve_fwd(const carve_params_t* p, const void* q, const void* k, 
     a.q = q; a.k = k; a.v = v; a.f = f; a.bx = bx; a.wx = wx; a.beta = beta;
     a.A = A; a.tau = tau; a.Ub = Ub; a.Uw = Uw; a.Vb = Vb; a.Vw = Vw; a.S0 = S0;
     a.O = O; a.S_final = S_final;
+    if (path == CARVE_PATH_TENSOR)
+        return tc_fwd_launch(a, nullptr, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess ? CARVE_OK : CARVE_ERR_CUDA;
     fill_ws(a, *p, workspace);
     return simt_fwd_launch(a, p->dtype, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess ? CARVE_OK
                                                                                               : CARVE_ERR_CUDA;

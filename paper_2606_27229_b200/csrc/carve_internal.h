@@ -67,4 +67,9 @@ cudaError_t simt_fwd_launch(const Args& a, int dtype, cudaStream_t st);
 cudaError_t simt_bwd_launch(const Args& a, int dtype, float* dA, float* dtau, float* dUb, float* dUw,
                             float* dVb, float* dVw, cudaStream_t st);
 
+// Tensor-core path (carve_tc_fwd.cu): bf16 tokens, dk == dv in {64,128}, r <= 16.
+bool tc_fwd_supported(const carve_params_t& p);
+size_t tc_state_tile_bytes(const carve_params_t& p);
+cudaError_t tc_fwd_launch(const Args& a, uint8_t* ws_S, cudaStream_t st);
+
 }  // namespace carve

@@ -1,0 +1,93 @@
+// carve_tc.cuh -- shared pieces of the tensor-core (tcgen05 + TMA) CARVE kernels: the shared-memory
+// and TMEM maps, the thread <-> tile-row mapping, and small math helpers.
+// walks through the phases; the comments here state what each buffer holds.
+//
+// One CTA of 256 threads owns one (batch, head) chain for the whole sequence.  Every MMA has M = 128:
+// accumulator row r lives in TMEM lane r, warp w reads lanes 32*(w%4).., and the two warpgroups
+// (w/4 = 0, 1) split the columns of a tile in halves.  Rows 0..63 of a stacked tile are the
+// "K-role" rows of the chunk's 64 tokens, rows 64..127 the "Q-role" rows of the same tokens, so
+// one instruction computes e.g. [Kbar; Qbar] S^T.
+#pragma once
+#include "carve_internal.h"
+#include "tc_common.cuh"
+
+namespace carve {
+namespace tcp {
+
+using namespace tc;
+
+constexpr int NT = 256;  // threads per CTA
+constexpr int LC = 64;   // tokens per solve chunk (gate chunks of L = 128 run as two solve chunks)
+constexpr int AB = 16;   // anchor block: decay ratios > 1 are only ever formed inside one 16-token block
+
+// TMEM column map (512 columns x 128 lanes of fp32).
+constexpr uint32_t TM_S = 0;      // [dv lanes][dk]   fp32 state S_{c-1}, updated in place at the chunk end
+constexpr uint32_t TM_ACC = 128;  // [128][dv]        rows 0..63  Kbar S^T (prediction), rows 64..127 Qbar S^T + P U (output)
+constexpr uint32_t TM_X1 = 256;   // [128][max d]     gate up-projections, later U = T (beta R)
+constexpr uint32_t TM_X2 = 384;   // G^T | Z, then the log-retention scan, then A|P blocks, then the state increment
+constexpr uint32_t TM_COLS = 512;
+
+struct Layout {  // byte offsets into the 1024-aligned dynamic shared memory
+    uint32_t Sb, Ucat, Vcat, KQraw, F, BX, WX, V, KQbar, Ktil, Us, Y0, Y1, Y2, TP, Mm, Tm, misc, total;
+    __host__ __device__ Layout(int dk, int dv, int r2)
+    {
+        uint32_t o = 0;
+        auto take = [&](uint32_t n) { uint32_t r = o; o += (n + 1023u) & ~1023u; return r; };
+        const int dm = dk > dv ? dk : dv;
+        Sb = take(tile_bytes(dv, dk));      // bf16 S_{c-1}: rows x, cols j
+        Ucat = take(tile_bytes(r2, dv));    // [Ub; Uw]: rows i, cols x
+        Vcat = take(tile_bytes(dm, 64));    // row n: [Vb[n][0..r) | Vw[n][0..r)]
+        KQraw = take(tile_bytes(128, dk));  // TMA: rows 0..63 k, rows 64..127 q
+        F = take(tile_bytes(64, dk));       // TMA: decay logits            | later Kbar,Qbar (with BX)
+        BX = take(tile_bytes(64, dk));      // TMA: erase pre-activation
+        WX = take(tile_bytes(64, dv));      // TMA: write pre-activation    | later Ktil
+        V = take(tile_bytes(64, dv));       // TMA: values -> V' = w.v      | later U
+        KQbar = F; Ktil = WX; Us = V;
+        Y0 = take((uint32_t)dk * 128);      // G (rows j, cols i) | la_hi | row operands re-anchored at token 32
+        Y1 = take(16384);                   // [0 tt_w; tt_b 0] | la_lo | C (column operand of A and P)
+        Y2 = take(16384);                   // block-triangular ones | beta R
+        TP = take(16384);                   // rows 0..63 T = (I + beta A)^-1, rows 64..127 P
+        if (tile_bytes(128, dk) >= 32768) { Mm = KQraw; Tm = KQraw + 16384; }
+        else { Mm = take(16384); Tm = take(16384); }  // fp32 scratch of the triangular inverse
+        misc = take(7168);
+        total = o + 1024;                   // slack for the manual 1024-byte alignment
+    }
+};
+
+// misc area (floats unless noted)
+struct Misc {
+    float eA[128], tau[128];    // exp(A_h), tau_h
+    float etot[4][128];         // exp(sum of log a over 16-token anchor block b)
+    float suf[4][128];          // product of etot[b'] over b' > b
+    float gamL[128];            // gamma_{L-1} of the chunk
+    float nrm[128][2];          // partial sums of squares: rows 0..63 k, 64..127 q; [half]
+    float beta[64];             // write strength of the chunk's tokens
+    uint64_t bar_mma, bar_kq, bar_fb, bar_wv;
+    uint32_t tmem_base;
+};
+
+static_assert(sizeof(Misc) <= 7168, "misc area too small");
+
+__device__ __forceinline__ float softplus_fast(float x) { return fmaxf(x, 0.f) + __logf(1.f + __expf(-fabsf(x))); }
+__device__ __forceinline__ float sigmoid_fast(float x) { return __fdividef(1.f, 1.f + __expf(-x)); }
+__device__ __forceinline__ float tanh_fast(float x)
+{
+    float y;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ uint4 lds128(const uint8_t* p) { return *reinterpret_cast<const uint4*>(p); }
+__device__ __forceinline__ void sts128(uint8_t* p, uint4 v) { *reinterpret_cast<uint4*>(p) = v; }
+__device__ __forceinline__ void unpack8(uint4 w, float (&f)[8])
+{
+    f[0] = bf16_lo(w.x); f[1] = bf16_hi(w.x); f[2] = bf16_lo(w.y); f[3] = bf16_hi(w.y);
+    f[4] = bf16_lo(w.z); f[5] = bf16_hi(w.z); f[6] = bf16_lo(w.w); f[7] = bf16_hi(w.w);
+}
+__device__ __forceinline__ uint4 pack8(const float* f)
+{
+    return make_uint4(pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
+}
+
+}  // namespace tcp
+}  // namespace carve

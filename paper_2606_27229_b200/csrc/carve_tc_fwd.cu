@@ -1,0 +1,805 @@
+// carve_tc_fwd.cu -- tensor-core forward of the CARVE layer operator for bf16 token tensors
+// (tcgen05.mma with TMEM accumulators, operands staged by TMA, fp32 state kept on chip).
+//
+// One persistent CTA per (batch, head) chain walks the sequence in solve chunks of LC = 64 tokens
+// (a gate chunk of L = 128 is two solve chunks that share one folded readout G_c; L = 16, 32 run
+// as short solve chunks).  Per solve chunk, in the order of PAPER.md Alg. 1-2 (l.160-196, l.315-365):
+//   P0  G^T = S^T [Ub;Uw]^T                       fold, Eq. 7 (l.134)                       [MMA]
+//   P2  Z = [k;q] G^T, tt = tanh(Z rnorm_q)       bottleneck, Eq. 7                          [MMA]
+//   P4  [w_proj; b_proj] = [0 tt_w; tt_b 0] [Vb|Vw]^T   up-projections, Eq. 8 (l.140)       [MMA]
+//   P5  la = g - softplus(bx + b_proj)  (= log a_t, Eq. 9 l.151, Eq. 14 l.310);  V' = sigmoid(wx + w_proj) v
+//   P6  block-local prefix sums of la over tokens (Eq. 14) as a product with a 0/+-1 triangular
+//       matrix, la split in bf16 hi + lo so the sums keep fp32 accuracy                      [MMA]
+//   P7  decayed operands, every exponent relative to the start of its 32-token block:
+//       Kbar_t = k^_t gamma_{t-1}, Qbar_t = q^_t gamma_t, C_s = k^_s gamma_a/gamma_s, Ktil_t = k^_t gamma_L/gamma_t
+//   P8  A|P blocks = [Kbar;Qbar] C^T (Eq. 15 l.342);  [Kbar;Qbar] S^T (Alg. 2 steps 5, 8)   [MMA]
+//   P9  T = (I + diag(beta) A)^-1 by blocked forward substitution (Alg. 2 step 7);  beta R = beta (V' - Kbar S^T)
+//   P10 U = T (beta R)                                                                     [MMA]
+//   P12 O += P U (step 8);  W = U^T Ktil (step 9)                                          [MMA]
+//   P13 O -> HBM;  S <- S diag(gamma_L) + W  (fp32, TMEM), bf16 copy for the next chunk's MMAs
+// Decay ratios: with log a ~ -1.6 per token gamma_L reaches e^-100 per chunk, so no 1/gamma is ever
+// formed over more than one 32-token block; across blocks only ratios <= 1 are multiplied in.
+#include <mutex>
+
+#include "carve_tc.cuh"
+
+namespace carve {
+namespace {
+
+using namespace tcp;
+
+struct TcArgs {
+    int B, H, T, L, r;
+    int l2norm;
+    float scale, eps;
+    const __nv_bfloat16* beta;
+    const float *A, *tau, *Ub, *Uw, *Vb, *Vw, *S0;
+    __nv_bfloat16* O;
+    float* S_final;
+    uint8_t* ws_S;  // bf16 row tiles of the state entering every solve chunk, or nullptr
+};
+
+// Runtime-shaped product from two row tiles (see tc_common.cuh umma_tiles); M fixed at compile time.
+template <int M, int AMAJ, int BMAJ>
+__device__ __forceinline__ void mma_rt(uint32_t d_tmem, int N, uint32_t a_saddr, int a_rows, int a_o0, uint32_t b_saddr,
+                                       int b_rows, int b_o0, int K, bool accumulate)
+{
+    const uint32_t idesc = umma_idesc(M, N, AMAJ, BMAJ);
+    for (int k = 0; k < K; k += 16) {
+        const uint64_t ad = AMAJ == KMAJ ? desc_kmajor(a_saddr, a_rows, a_o0, k) : desc_mnmajor(a_saddr, a_rows, a_o0, k);
+        const uint64_t bd = BMAJ == KMAJ ? desc_kmajor(b_saddr, b_rows, b_o0, k) : desc_mnmajor(b_saddr, b_rows, b_o0, k);
+        umma(d_tmem, ad, bd, idesc, (accumulate || k > 0) ? 1u : 0u);
+    }
+}
+
+// fp32 scratch matrices of the triangular inverse: [64][64], columns XOR-swizzled by the row.
+__device__ __forceinline__ int mm_idx(int r, int c) { return r * 64 + (c ^ ((r & 7) << 2)); }
+
+__device__ __forceinline__ void mma_tf32(float (&d)[4], const uint32_t (&a)[4], const uint32_t (&b)[2])
+{
+    asm volatile(
+        "mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+}
+
+// One warp: D[16*MT x 8] = sum over k < 8*KS of P[pr + .][pc + k] * Q[qr + k][qc + .]  (fp32 swizzled matrices).
+template <int MT, int KS>
+__device__ __forceinline__ void warp_prod(float (&d)[MT][4], const float* P, int pr, int pc, const float* Q, int qr, int qc,
+                                          int lane)
+{
+    const int g = lane >> 2, l4 = lane & 3;
+#pragma unroll
+    for (int m = 0; m < MT; ++m)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) d[m][e] = 0.f;
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks) {
+        uint32_t bfr[2];
+        bfr[0] = __float_as_uint(Q[mm_idx(qr + 8 * ks + l4, qc + g)]);
+        bfr[1] = __float_as_uint(Q[mm_idx(qr + 8 * ks + l4 + 4, qc + g)]);
+#pragma unroll
+        for (int m = 0; m < MT; ++m) {
+            uint32_t afr[4];
+            afr[0] = __float_as_uint(P[mm_idx(pr + 16 * m + g, pc + 8 * ks + l4)]);
+            afr[1] = __float_as_uint(P[mm_idx(pr + 16 * m + g + 8, pc + 8 * ks + l4)]);
+            afr[2] = __float_as_uint(P[mm_idx(pr + 16 * m + g, pc + 8 * ks + l4 + 4)]);
+            afr[3] = __float_as_uint(P[mm_idx(pr + 16 * m + g + 8, pc + 8 * ks + l4 + 4)]);
+            mma_tf32(d[m], afr, bfr);
+        }
+    }
+}
+template <int MT>
+__device__ __forceinline__ void warp_store(float* Q, int qr, int qc, const float (&d)[MT][4], float sign, int lane)
+{
+    const int g = lane >> 2, l4 = lane & 3;
+#pragma unroll
+    for (int m = 0; m < MT; ++m) {
+        Q[mm_idx(qr + 16 * m + g, qc + 2 * l4)] = sign * d[m][0];
+        Q[mm_idx(qr + 16 * m + g, qc + 2 * l4 + 1)] = sign * d[m][1];
+        Q[mm_idx(qr + 16 * m + g + 8, qc + 2 * l4)] = sign * d[m][2];
+        Q[mm_idx(qr + 16 * m + g + 8, qc + 2 * l4 + 1)] = sign * d[m][3];
+    }
+}
+
+// Tm <- (I + Mm)^-1 for the leading n x n block (n in {16,32,64}); Mm strictly lower (only that part is read).
+// Blocked forward substitution (Alg. 2 step 7): 16x16 diagonal blocks by substitution, then
+// T_ij = -T_ii (M_ij T_jj) one level at a time, the block products on tensor cores (tf32 mma.sync).
+__device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid)
+{
+    const int warp = tid >> 5, lane = tid & 31;
+    if (tid < n) {
+        const int blk = tid >> 4, c = tid & 15, o = 16 * blk;
+        float x[16];
+#pragma unroll
+        for (int tt = 0; tt < 16; ++tt) {
+            float acc = 0.f;
+#pragma unroll
+            for (int s = 0; s < tt; ++s) acc += Mm[mm_idx(o + tt, o + s)] * x[s];
+            x[tt] = (tt == c) ? 1.f : (tt < c ? 0.f : -acc);
+            Tm[mm_idx(o + tt, o + c)] = x[tt];
+        }
+    } else if (n >= 64) {
+        // blocks (0,1) and (2,3) of T are zero; the level-64 products read them
+        for (int i = tid - 64; i < 512; i += NT - 64) {
+            const int blk = i >> 8, rr = (i >> 4) & 15, cc = i & 15;
+            Tm[mm_idx(32 * blk + rr, 32 * blk + 16 + cc)] = 0.f;
+        }
+    }
+    __syncthreads();
+    if (n >= 32) {
+        // level 32: blocks (1,0) and (3,2); warp = (pair, 8-column tile)
+        const int npair = n / 32;
+        if (warp < 2 * npair) {
+            const int pair = warp >> 1, nt = warp & 1, i0 = 32 * pair + 16, j0 = 32 * pair;
+            float d[1][4];
+            warp_prod<1, 2>(d, Mm, i0, j0, Tm, j0, j0 + 8 * nt, lane);   // X = M_ij T_jj
+            warp_store<1>(Tm, i0, j0 + 8 * nt, d, 1.f, lane);
+            __syncwarp();
+            warp_prod<1, 2>(d, Tm, i0, i0, Tm, i0, j0 + 8 * nt, lane);   // T_ii X
+            __syncwarp();
+            warp_store<1>(Tm, i0, j0 + 8 * nt, d, -1.f, lane);
+        }
+        __syncthreads();
+    }
+    if (n >= 64) {
+        // level 64: rows 32..63 x cols 0..31; warp = 8-column tile
+        if (warp < 4) {
+            float d[2][4];
+            warp_prod<2, 4>(d, Mm, 32, 0, Tm, 0, 8 * warp, lane);
+            warp_store<2>(Tm, 32, 8 * warp, d, 1.f, lane);
+            __syncwarp();
+            warp_prod<2, 4>(d, Tm, 32, 32, Tm, 32, 8 * warp, lane);
+            __syncwarp();
+            warp_store<2>(Tm, 32, 8 * warp, d, -1.f, lane);
+        }
+        __syncthreads();
+    }
+}
+
+#define PHASE_SYNC()            \
+    do {                        \
+        fence_async_smem();     \
+        tc_fence_before();      \
+        __syncthreads();        \
+        tc_fence_after();       \
+    } while (0)
+#define WAIT_MMA()                          \
+    do {                                    \
+        mbar_wait(&mi.bar_mma, mma_ph);     \
+        mma_ph ^= 1u;                       \
+        tc_fence_after();                   \
+    } while (0)
+
+template <int DK, int DV>
+__global__ void __launch_bounds__(NT, 1)
+carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, const __grid_constant__ CUtensorMap mk,
+                    const __grid_constant__ CUtensorMap mv, const __grid_constant__ CUtensorMap mf,
+                    const __grid_constant__ CUtensorMap mbx, const __grid_constant__ CUtensorMap mwx)
+{
+    static_assert(DK == DV, "the shared-memory map assumes dk == dv");
+    constexpr int DM = DK > DV ? DK : DV;
+    constexpr int HK = DK / 2, HV = DV / 2;  // columns per warpgroup half
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* sm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    const int r = a.r, R2 = 2 * r;
+    const Layout Lo(DK, DV, R2);
+    Misc& mi = *reinterpret_cast<Misc*>(sm + Lo.misc);
+    float* sBeta = mi.beta;
+    const uint32_t sb = smem_u32(sm);
+    float* Mm = reinterpret_cast<float*>(sm + Lo.Mm);
+    float* Tm = reinterpret_cast<float*>(sm + Lo.Tm);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, q = warp & 3, half = warp >> 2;
+    const int row = q * 32 + lane;   // tile row == TMEM lane served by this thread
+    const bool krole = q < 2;
+    const int t = row & 63;          // token of this row
+    const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+    const int chain = blockIdx.x, b = chain / a.H, h = chain % a.H;
+    const int LCc = a.L < LC ? a.L : LC;
+    const int nchunks = a.T / LCc, gate_every = a.L / LCc;
+    const bool warp_active = (q & 1) * 32 < LCc;  // this warp holds at least one live token row
+    const bool live = t < LCc;
+
+    // ---- one-time setup --------------------------------------------------------------------------
+    if (tid == 0) {
+        mbar_init(&mi.bar_mma, 1); mbar_init(&mi.bar_kq, 1); mbar_init(&mi.bar_fb, 1); mbar_init(&mi.bar_wv, 1);
+        mbar_fence_init();
+        tma_prefetch_desc(&mq); tma_prefetch_desc(&mk); tma_prefetch_desc(&mv);
+        tma_prefetch_desc(&mf); tma_prefetch_desc(&mbx); tma_prefetch_desc(&mwx);
+    }
+    if (warp == 0) tmem_alloc(&mi.tmem_base, TM_COLS);
+    for (int i = tid; i < R2 * DV; i += NT) {
+        const int ii = i / DV, x = i % DV;
+        const float v = ii < r ? __ldg(a.Ub + (size_t)ii * DV + x) : __ldg(a.Uw + (size_t)(ii - r) * DV + x);
+        *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Ucat + tile_off(R2, ii, x)) = __float2bfloat16_rn(v);
+    }
+    for (int i = tid; i < DM * 64; i += NT) {
+        const int n = i / 64, c = i % 64;
+        float v = 0.f;
+        if (c < r) { if (n < DK) v = __ldg(a.Vb + (size_t)n * r + c); }
+        else if (c < R2) { if (n < DV) v = __ldg(a.Vw + (size_t)n * r + (c - r)); }
+        *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Vcat + tile_off(DM, n, c)) = __float2bfloat16_rn(v);
+    }
+    for (int j = tid; j < DK; j += NT) {
+        mi.eA[j] = a.A ? __expf(__ldg(a.A + h * DK + j)) : 1.f;
+        mi.tau[j] = a.tau ? __ldg(a.tau + h * DK + j) : 0.f;
+    }
+    PHASE_SYNC();
+    const uint32_t tmem = mi.tmem_base;
+    const size_t state_tile = tile_bytes(DV, DK);
+    uint8_t* ws_chain = a.ws_S ? a.ws_S + (size_t)chain * nchunks * state_tile : nullptr;
+
+    // initial state: fp32 -> TMEM, bf16 -> Sb (and the workspace slot of chunk 0)
+    if (row < DV) {
+        const float* s0 = a.S0 ? a.S0 + ((size_t)chain * DV + row) * DK : nullptr;
+#pragma unroll
+        for (int s = 0; s < HK; s += 32) {
+            const int c0 = half * HK + s;
+            uint32_t v[32];
+#pragma unroll
+            for (int e = 0; e < 32; e += 4) {
+                float4 f4 = s0 ? __ldg(reinterpret_cast<const float4*>(s0 + c0 + e)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                v[e] = __float_as_uint(f4.x); v[e + 1] = __float_as_uint(f4.y);
+                v[e + 2] = __float_as_uint(f4.z); v[e + 3] = __float_as_uint(f4.w);
+            }
+            tmem_st32(tmem + TM_S + lane_base + c0, v);
+#pragma unroll
+            for (int ch = 0; ch < 4; ++ch) {
+                float f8[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) f8[e] = __uint_as_float(v[8 * ch + e]);
+                const uint4 w = pack8(f8);
+                const uint32_t off = tile_chunk_off(DV, row, c0 / 8 + ch);
+                sts128(sm + Lo.Sb + off, w);
+                if (ws_chain) *reinterpret_cast<uint4*>(ws_chain + off) = w;
+            }
+        }
+        tmem_wait_st();
+    }
+
+    auto issue_kq = [&](int c) {
+        mbar_expect_tx(&mi.bar_kq, 2u * LCc * DK * 2u);
+        const int tr = b * a.T + c * LCc;
+        for (int cb = 0; cb < DK / 64; ++cb) {
+            tma_load_3d(sm + Lo.KQraw + cb * 128 * 128, &mk, &mi.bar_kq, cb * 64, h, tr);
+            tma_load_3d(sm + Lo.KQraw + cb * 128 * 128 + 64 * 128, &mq, &mi.bar_kq, cb * 64, h, tr);
+        }
+    };
+    auto issue_fb = [&](int c) {
+        mbar_expect_tx(&mi.bar_fb, 2u * LCc * DK * 2u);
+        const int tr = b * a.T + c * LCc;
+        for (int cb = 0; cb < DK / 64; ++cb) {
+            tma_load_3d(sm + Lo.F + cb * 64 * 128, &mf, &mi.bar_fb, cb * 64, h, tr);
+            tma_load_3d(sm + Lo.BX + cb * 64 * 128, &mbx, &mi.bar_fb, cb * 64, h, tr);
+        }
+    };
+    auto issue_wv = [&](int c) {
+        mbar_expect_tx(&mi.bar_wv, 2u * LCc * DV * 2u);
+        const int tr = b * a.T + c * LCc;
+        for (int cb = 0; cb < DV / 64; ++cb) {
+            tma_load_3d(sm + Lo.WX + cb * 64 * 128, &mwx, &mi.bar_wv, cb * 64, h, tr);
+            tma_load_3d(sm + Lo.V + cb * 64 * 128, &mv, &mi.bar_wv, cb * 64, h, tr);
+        }
+    };
+    if (tid == 0) { fence_async_smem(); issue_kq(0); issue_fb(0); issue_wv(0); }
+
+    uint32_t mma_ph = 0, tma_ph = 0;
+    for (int c = 0; c < nchunks; ++c) {
+        const bool fold_now = (c % gate_every) == 0;
+        const size_t tok0 = (size_t)b * a.T + (size_t)c * LCc;  // first token of the chunk
+        // ---- P0: fold G^T = S^T Ucat^T -> TM_X2[0, R2)
+        PHASE_SYNC();
+        if (fold_now && tid == 0) {
+            mma_rt<128, MNMAJ, KMAJ>(tmem + TM_X2, R2, sb + Lo.Sb, DV, 0, sb + Lo.Ucat, R2, 0, DV, false);
+            umma_commit(&mi.bar_mma);
+        }
+        // meanwhile: raw k, q have landed -> partial sums of squares; beta
+        mbar_wait(&mi.bar_kq, tma_ph);
+        if (live) {
+            float ss = 0.f;
+#pragma unroll
+            for (int ch = 0; ch < HK / 8; ++ch) {
+                float f8[8];
+                unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, row, half * (HK / 8) + ch)), f8);
+#pragma unroll
+                for (int e = 0; e < 8; ++e) ss += f8[e] * f8[e];
+            }
+            mi.nrm[row][half] = ss;
+            if (krole && half == 0) sBeta[t] = __bfloat162float(a.beta[(tok0 + t) * a.H + h]);
+        }
+        if (fold_now) {
+            WAIT_MMA();
+            // ---- P1: G^T (lanes j) -> bf16 into the spare columns [32, 32+R2) of the Vcat tile
+            if (half == 0 && q * 32 < DK) {
+                for (int c0 = 0; c0 < R2; c0 += 16) {
+                    uint32_t v[16];
+                    tmem_ld16(tmem + TM_X2 + lane_base + c0, v);
+                    tmem_wait_ld();
+                    float f[16];
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) f[e] = __uint_as_float(v[e]);
+                    sts128(sm + Lo.Vcat + tile_chunk_off(DM, row, (32 + c0) / 8), pack8(f));
+                    sts128(sm + Lo.Vcat + tile_chunk_off(DM, row, (32 + c0) / 8 + 1), pack8(f + 8));
+                }
+            }
+        }
+        // ---- P2: Z = [k;q] G^T -> TM_X2[32, 32+R2)
+        PHASE_SYNC();
+        if (tid == 0) {
+            mma_rt<128, KMAJ, MNMAJ>(tmem + TM_X2 + 32, R2, sb + Lo.KQraw, 128, 0, sb + Lo.Vcat, DM, 32, DK, false);
+            umma_commit(&mi.bar_mma);
+        }
+        WAIT_MMA();
+        // ---- P3: tt = tanh(Z rnorm_q) -> [0 tt_w; tt_b 0];  block-triangular +-1 matrix
+        if (!krole && half == 0 && warp_active) {
+            const float rnq = a.l2norm ? rsqrtf(mi.nrm[row][0] + mi.nrm[row][1] + a.eps) : 1.f;
+            const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
+            for (int c0 = 0; c0 < R2; c0 += 16) {
+                uint32_t v[16];
+                tmem_ld16(tmem + TM_X2 + 32 + lane_base + c0, v);
+                tmem_wait_ld();
+                if (live) {
+                    float f[16];
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) f[e] = tanh_fast(__uint_as_float(v[e]) * rnq);
+#pragma unroll
+                    for (int k8 = 0; k8 < 2; ++k8) {
+                        const int col = c0 + 8 * k8;       // tt columns [col, col+8)
+                        const uint4 w = pack8(f + 8 * k8);
+                        const bool is_b = col < r;         // erase-gate half of the bottleneck
+                        sts128(sm + Lo.Y1 + tile_chunk_off(128, 64 + t, col / 8), is_b ? w : z4);
+                        sts128(sm + Lo.Y1 + tile_chunk_off(128, t, col / 8), is_b ? z4 : w);
+                    }
+                }
+            }
+        }
+        if (half == 1) {
+            const uint32_t one = krole ? 0xBF80u : 0x3F80u;  // bf16 -1 / +1
+#pragma unroll
+            for (int ch = 0; ch < 8; ++ch) {
+                uint32_t w[4];
+#pragma unroll
+                for (int p = 0; p < 4; ++p) {
+                    const int s0 = 8 * ch + 2 * p, s1 = s0 + 1;
+                    const uint32_t lo = (s0 <= t && (s0 >> 4) == (t >> 4)) ? one : 0u;
+                    const uint32_t hi = (s1 <= t && (s1 >> 4) == (t >> 4)) ? one : 0u;
+                    w[p] = lo | (hi << 16);
+                }
+                sts128(sm + Lo.Y2 + tile_chunk_off(128, row, ch), make_uint4(w[0], w[1], w[2], w[3]));
+            }
+        }
+        // ---- P4: [w_proj; b_proj] = Ablk Vcat^T -> TM_X1
+        PHASE_SYNC();
+        if (tid == 0) {
+            mma_rt<128, KMAJ, KMAJ>(tmem + TM_X1, DM, sb + Lo.Y1, 128, 0, sb + Lo.Vcat, DM, 0, R2, false);
+            umma_commit(&mi.bar_mma);
+        }
+        mbar_wait(&mi.bar_fb, tma_ph);
+        mbar_wait(&mi.bar_wv, tma_ph);
+        WAIT_MMA();
+        // ---- P5: gates (8 columns per step; cc = 16-byte chunk index inside the row)
+        if (warp_active) {
+            if (!krole) {
+#pragma unroll 1
+                for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
+                    uint32_t pr[8];
+                    tmem_ld8(tmem + TM_X1 + lane_base + 8 * cc, pr);
+                    tmem_wait_ld();
+                    if (live) {
+                        float fb[8], ff[8], hi[8], lo[8];
+                        const uint32_t off = tile_chunk_off(64, t, cc);
+                        unpack8(lds128(sm + Lo.BX + off), fb);
+                        unpack8(lds128(sm + Lo.F + off), ff);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            const int j = 8 * cc + e;
+                            const float pre = fb[e] + __uint_as_float(pr[e]);
+                            const float g = -mi.eA[j] * softplus_fast(ff[e] + mi.tau[j]);
+                            const float la = g - softplus_fast(pre);
+                            const float h16 = __bfloat162float(__float2bfloat16_rn(la));
+                            hi[e] = h16;
+                            lo[e] = la - h16;
+                        }
+                        sts128(sm + Lo.Y0 + off, pack8(hi));
+                        sts128(sm + Lo.Y1 + off, pack8(lo));
+                    }
+                }
+            } else {
+#pragma unroll 1
+                for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
+                    uint32_t pr[8];
+                    tmem_ld8(tmem + TM_X1 + lane_base + 8 * cc, pr);
+                    tmem_wait_ld();
+                    if (live) {
+                        float fw[8], fv[8];
+                        const uint32_t off = tile_chunk_off(64, t, cc);
+                        unpack8(lds128(sm + Lo.WX + off), fw);
+                        unpack8(lds128(sm + Lo.V + off), fv);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) fv[e] *= sigmoid_fast(fw[e] + __uint_as_float(pr[e]));
+                        sts128(sm + Lo.V + off, pack8(fv));
+                    }
+                }
+            }
+        }
+        // ---- P6: block-local prefix sums -> TM_X2[0, DK): rows 0..63 a_b - lg_t, rows 64..127 lg_t - a_b
+        PHASE_SYNC();
+        if (tid == 0) {
+            mma_rt<128, KMAJ, MNMAJ>(tmem + TM_X2, DK, sb + Lo.Y2, 128, 0, sb + Lo.Y0, 64, 0, LCc, false);
+            mma_rt<128, KMAJ, MNMAJ>(tmem + TM_X2, DK, sb + Lo.Y2, 128, 0, sb + Lo.Y1, 64, 0, LCc, true);
+            umma_commit(&mi.bar_mma);
+        }
+        WAIT_MMA();
+        // ---- P7a: exp of the block totals (last token of each 16-token anchor block), then their suffix products
+        if (!krole && warp_active) {
+            const int blk = t >> 4;
+            const bool last = live && (t & 15) == 15;
+#pragma unroll 1
+            for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
+                uint32_t v[8];
+                tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, v);
+                tmem_wait_ld();
+                if (last) {
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) mi.etot[blk][8 * cc + e] = __expf(__uint_as_float(v[e]));
+                }
+            }
+        }
+        __syncthreads();
+        if (tid < DK) {
+            const int nb = LCc >> 4;
+            float p = 1.f;  // suf[b] = prod of etot[b'] over b' > b
+#pragma unroll
+            for (int b2 = 3; b2 >= 0; --b2) {
+                mi.suf[b2][tid] = p;
+                if (b2 < nb) p *= mi.etot[b2][tid];
+            }
+            mi.gamL[tid] = p;
+        }
+        __syncthreads();
+        // ---- P7b: decayed operands.  Row operands exist in up to four anchorings: version 0 relative to the chunk
+        //      start (Kbar, Qbar: also the operand of the state products), version jb relative to the start of
+        //      anchor block jb (only rows at or after that block).  Column operand C_s is relative to its own block.
+        if (warp_active) {
+            const int blk = t >> 4;
+            // smem address of chunk cc of the row of (version, role, token)
+            auto ver_row = [&](int jb, bool qrole, int tok, int cc) -> uint8_t* {
+                switch (jb) {
+                    case 0: return sm + Lo.KQbar + tile_chunk_off(128, (qrole ? 64 : 0) + tok, cc);
+                    case 1: return sm + Lo.Y2 + tile_chunk_off(96, (qrole ? 48 : 0) + tok - 16, cc);
+                    case 2: return sm + Lo.Y0 + tile_chunk_off(64, (qrole ? 32 : 0) + tok - 32, cc);
+                    default: return sm + Lo.Y2 + tile_bytes(96, DK) + tile_chunk_off(32, (qrole ? 16 : 0) + tok - 48, cc);
+                }
+            };
+            if (!krole) {
+                const float rnq = a.l2norm ? rsqrtf(mi.nrm[row][0] + mi.nrm[row][1] + a.eps) : 1.f;
+                const int tn = t + 1;  // the key row that shares this token's retention (Kbar_{t+1} = k^_{t+1} gamma_t)
+                const bool has_next = tn < LCc;
+                const int bn = tn >> 4, krow = has_next ? tn : 0;
+                const float rnk = a.l2norm ? rsqrtf(mi.nrm[krow][0] + mi.nrm[krow][1] + a.eps) : 1.f;
+#pragma unroll 1
+                for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
+                    uint32_t v[8];
+                    tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, v);
+                    tmem_wait_ld();
+                    if (live) {
+                        float Fp[8], qv[8], kv[8], o[8];
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) Fp[e] = __expf(__uint_as_float(v[e]));  // gamma_t / gamma_{a_blk}
+                        unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, 64 + t, cc)), qv);
+                        unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, krow, cc)), kv);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) { qv[e] *= rnq; kv[e] *= rnk; }
+                        if (has_next && bn > blk) sts128(ver_row(bn, false, tn, cc), pack8(kv));  // first row of its block
+#pragma unroll
+                        for (int jb = 3; jb >= 0; --jb) {
+                            if (jb <= blk) {
+#pragma unroll
+                                for (int e = 0; e < 8; ++e) o[e] = qv[e] * Fp[e];
+                                sts128(ver_row(jb, true, t, cc), pack8(o));
+                                if (has_next) {
+#pragma unroll
+                                    for (int e = 0; e < 8; ++e) o[e] = kv[e] * Fp[e];
+                                    sts128(ver_row(jb, false, tn, cc), pack8(o));
+                                }
+                                if (jb > 0) {
+                                    const float4 e0 = *reinterpret_cast<const float4*>(&mi.etot[jb - 1][8 * cc]);
+                                    const float4 e1 = *reinterpret_cast<const float4*>(&mi.etot[jb - 1][8 * cc + 4]);
+                                    Fp[0] *= e0.x; Fp[1] *= e0.y; Fp[2] *= e0.z; Fp[3] *= e0.w;
+                                    Fp[4] *= e1.x; Fp[5] *= e1.y; Fp[6] *= e1.z; Fp[7] *= e1.w;
+                                }
+                            }
+                        }
+                        if (!has_next) sts128(sm + Lo.KQbar + tile_chunk_off(128, 0, cc), pack8(kv));  // Kbar_0 = k^_0
+                    }
+                }
+            } else {
+                const float rnk = a.l2norm ? rsqrtf(mi.nrm[row][0] + mi.nrm[row][1] + a.eps) : 1.f;
+#pragma unroll 1
+                for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
+                    uint32_t v[8];
+                    tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, v);
+                    tmem_wait_ld();
+                    if (live) {
+                        float kv[8], o1[8], o2[8], et[8], sf[8];
+                        unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, t, cc)), kv);
+                        *reinterpret_cast<float4*>(et) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc]);
+                        *reinterpret_cast<float4*>(et + 4) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc + 4]);
+                        *reinterpret_cast<float4*>(sf) = *reinterpret_cast<const float4*>(&mi.suf[blk][8 * cc]);
+                        *reinterpret_cast<float4*>(sf + 4) = *reinterpret_cast<const float4*>(&mi.suf[blk][8 * cc + 4]);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            const float cx = __expf(__uint_as_float(v[e]));   // gamma_{a_blk} / gamma_t >= 1
+                            const float kh = kv[e] * rnk;
+                            o1[e] = kh * cx;
+                            o2[e] = kh * ((cx * et[e]) * sf[e]);              // k^ gamma_L / gamma_t, every factor <= 1
+                        }
+                        sts128(sm + Lo.Y1 + tile_chunk_off(64, t, cc), pack8(o1));      // C_t
+                        sts128(sm + Lo.Ktil + tile_chunk_off(64, t, cc), pack8(o2));    // Ktil_t
+                    }
+                }
+            }
+        }
+        // ---- P8: A|P blocks (one 16-column block per anchoring) and the state products
+        PHASE_SYNC();
+        if (tid == 0) {
+            const int nb = LCc >> 4;
+            mma_rt<128, KMAJ, KMAJ>(tmem + TM_X2, 16, sb + Lo.KQbar, 128, 0, sb + Lo.Y1, 64, 0, DK, false);
+            if (nb > 1) mma_rt<128, KMAJ, KMAJ>(tmem + TM_X2 + 16, 16, sb + Lo.Y2, 96, 0, sb + Lo.Y1, 64, 16, DK, false);
+            if (nb > 2) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 32, 16, sb + Lo.Y0, 64, 0, sb + Lo.Y1, 64, 32, DK, false);
+            if (nb > 3) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 48, 16, sb + Lo.Y2 + tile_bytes(96, DK), 32, 0, sb + Lo.Y1, 64, 48, DK, false);
+            mma_rt<128, KMAJ, KMAJ>(tmem + TM_ACC, DV, sb + Lo.KQbar, 128, 0, sb + Lo.Sb, DV, 0, DK, false);
+            umma_commit(&mi.bar_mma);
+        }
+        WAIT_MMA();
+        // ---- P9a: beta A -> Mm (fp32, only the strictly lower part is ever read), P -> TP rows 64.. (bf16, masked s <= t)
+        {
+            // one 16-column piece [16 jb, 16 jb + 16) of row `tok`
+            auto put_piece = [&](bool qrole, int tok, int jb, const uint32_t (&v)[16]) {
+                if (!qrole) {
+                    const float bt = sBeta[tok];
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) Mm[mm_idx(tok, 16 * jb + e)] = bt * __uint_as_float(v[e]);
+                } else {
+                    float f[16];
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) f[e] = (16 * jb + e <= tok) ? __uint_as_float(v[e]) : 0.f;
+                    sts128(sm + Lo.TP + tile_chunk_off(128, 64 + tok, 2 * jb), pack8(f));
+                    sts128(sm + Lo.TP + tile_chunk_off(128, 64 + tok, 2 * jb + 1), pack8(f + 8));
+                }
+            };
+            const int nb = LCc >> 4;
+            uint32_t v[16];
+            if (half == 0) {
+                // version 0: lane = stacked row
+                tmem_ld16(tmem + TM_X2 + lane_base, v);
+                tmem_wait_ld();
+                if (live) {
+                    put_piece(!krole, t, 0, v);
+                    if (!krole) {  // pieces above the row's own block are zero
+                        const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
+                        for (int jb = (t >> 4) + 1; jb < 4; ++jb) {
+                            sts128(sm + Lo.TP + tile_chunk_off(128, 64 + t, 2 * jb), z4);
+                            sts128(sm + Lo.TP + tile_chunk_off(128, 64 + t, 2 * jb + 1), z4);
+                        }
+                    }
+                }
+                if (nb > 2) {
+                    // version 2 (M = 64): compact row m = 16 q + lane sits in lane < 16 of warp q; m < 32: K token 32+m, else Q token m
+                    tmem_ld16(tmem + TM_X2 + 32 + lane_base, v);
+                    tmem_wait_ld();
+                    if (lane < 16) {
+                        const int tok = 32 + 16 * (q & 1) + lane;
+                        if (tok < LCc) put_piece(q >= 2, tok, 2, v);
+                    }
+                }
+            } else {
+                if (nb > 1) {
+                    // version 1 (M = 128 over a 96-row tile): lanes 0..47 K tokens 16.., lanes 48..95 Q tokens 16..
+                    tmem_ld16(tmem + TM_X2 + 16 + lane_base, v);
+                    tmem_wait_ld();
+                    if (row < 96) {
+                        const bool qr = row >= 48;
+                        const int tok = 16 + (qr ? row - 48 : row);
+                        if (tok < LCc) put_piece(qr, tok, 1, v);
+                    }
+                }
+                if (nb > 3) {
+                    // version 3 (M = 64 over a 32-row tile): m < 16: K token 48+m (warp 0), 16 <= m < 32: Q token 32+m (warp 1)
+                    tmem_ld16(tmem + TM_X2 + 48 + lane_base, v);
+                    tmem_wait_ld();
+                    if (lane < 16 && q < 2) put_piece(q == 1, 48 + lane, 3, v);
+                }
+            }
+        }
+        // ---- P9b: beta R = beta (V' - Kbar S^T) -> Y2 (rows t)
+        if (krole && warp_active) {
+            const float bt = live ? sBeta[t] : 0.f;
+#pragma unroll 1
+            for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
+                uint32_t v[8];
+                tmem_ld8(tmem + TM_ACC + lane_base + 8 * cc, v);
+                tmem_wait_ld();
+                if (live) {
+                    float fv[8];
+                    const uint32_t off = tile_chunk_off(64, t, cc);
+                    unpack8(lds128(sm + Lo.V + off), fv);
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) fv[e] = bt * (fv[e] - __uint_as_float(v[e]));
+                    sts128(sm + Lo.Y2 + off, pack8(fv));
+                }
+            }
+        }
+        __syncthreads();
+        // ---- P9c: T = (I + beta A)^-1 -> TP rows 0..63 (bf16, zero above the diagonal)
+        tri_inverse(Mm, Tm, LCc, tid);
+        {
+            const int tr_ = tid >> 2, qq = tid & 3;  // row, 16-column quarter
+            if (tr_ < LCc) {
+#pragma unroll
+                for (int k8 = 0; k8 < 2; ++k8) {
+                    float f[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const int s = 16 * qq + 8 * k8 + e;
+                        f[e] = s <= tr_ ? Tm[mm_idx(tr_, s)] : 0.f;
+                    }
+                    sts128(sm + Lo.TP + tile_chunk_off(128, tr_, 2 * qq + k8), pack8(f));
+                }
+            }
+        }
+        // ---- P10: U = T (beta R) -> TM_X1
+        PHASE_SYNC();
+        if (tid == 0) {
+            mma_rt<128, KMAJ, MNMAJ>(tmem + TM_X1, DV, sb + Lo.TP, 128, 0, sb + Lo.Y2, 64, 0, LCc, false);
+            umma_commit(&mi.bar_mma);
+            if (c + 1 < nchunks) issue_kq(c + 1);
+        }
+        WAIT_MMA();
+        // ---- P11: U -> bf16 rows (over V')
+        if (krole && warp_active) {
+#pragma unroll 1
+            for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
+                uint32_t v[8];
+                tmem_ld8(tmem + TM_X1 + lane_base + 8 * cc, v);
+                tmem_wait_ld();
+                if (live) {
+                    float f[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[e]);
+                    sts128(sm + Lo.Us + tile_chunk_off(64, t, cc), pack8(f));
+                }
+            }
+        }
+        // ---- P12: O += P U;  W = U^T Ktil -> TM_X2
+        PHASE_SYNC();
+        if (tid == 0) {
+            mma_rt<128, KMAJ, MNMAJ>(tmem + TM_ACC, DV, sb + Lo.TP, 128, 0, sb + Lo.Us, 64, 0, LCc, true);
+            mma_rt<128, MNMAJ, MNMAJ>(tmem + TM_X2, DK, sb + Lo.Us, 64, 0, sb + Lo.Ktil, 64, 0, LCc, false);
+            umma_commit(&mi.bar_mma);
+        }
+        WAIT_MMA();
+        if (tid == 0 && c + 1 < nchunks) { fence_async_smem(); issue_fb(c + 1); issue_wv(c + 1); }
+        // ---- P13: outputs and the state carry
+        if (!krole && warp_active) {
+            __nv_bfloat16* dst = a.O + ((tok0 + t) * a.H + h) * DV;
+#pragma unroll 1
+            for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
+                uint32_t v[8];
+                tmem_ld8(tmem + TM_ACC + lane_base + 8 * cc, v);
+                tmem_wait_ld();
+                if (live) {
+                    float f[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) f[e] = a.scale * __uint_as_float(v[e]);
+                    *reinterpret_cast<uint4*>(dst + 8 * cc) = pack8(f);
+                }
+            }
+        }
+        if (q * 32 < DV) {
+            const bool last_chunk = c + 1 == nchunks;
+            uint8_t* ws_next = (ws_chain && !last_chunk) ? ws_chain + (size_t)(c + 1) * state_tile : nullptr;
+#pragma unroll 1
+            for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
+                uint32_t sv[8], wv[8];
+                tmem_ld8(tmem + TM_S + lane_base + 8 * cc, sv);
+                tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, wv);
+                tmem_wait_ld();
+                float f[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    f[e] = __uint_as_float(sv[e]) * mi.gamL[8 * cc + e] + __uint_as_float(wv[e]);
+                    sv[e] = __float_as_uint(f[e]);
+                }
+                tmem_st8(tmem + TM_S + lane_base + 8 * cc, sv);
+                const uint4 w = pack8(f);
+                const uint32_t off = tile_chunk_off(DV, row, cc);
+                sts128(sm + Lo.Sb + off, w);
+                if (ws_next) *reinterpret_cast<uint4*>(ws_next + off) = w;
+                if (last_chunk) {
+                    float* dst = a.S_final + ((size_t)chain * DV + row) * DK + 8 * cc;
+                    *reinterpret_cast<float4*>(dst) = make_float4(f[0], f[1], f[2], f[3]);
+                    *reinterpret_cast<float4*>(dst + 4) = make_float4(f[4], f[5], f[6], f[7]);
+                }
+            }
+            tmem_wait_st();
+        }
+        tma_ph ^= 1u;
+    }
+    PHASE_SYNC();
+    if (warp == 0) tmem_dealloc(tmem, TM_COLS);
+}
+
+// ---- host side ---------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    });
+    return fn;
+}
+
+}  // namespace
+
+// [B,T,H,d] bf16 seen as (d, H, B*T); one box = 64 channels x 1 head x `rows` tokens, 128B-swizzled.
+bool tc_make_token_map(CUtensorMap* map, const void* base, int B, int T, int H, int d, int rows)
+{
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[3] = {(cuuint64_t)d, (cuuint64_t)H, (cuuint64_t)B * T};
+    cuuint64_t strides[2] = {(cuuint64_t)d * 2, (cuuint64_t)H * d * 2};
+    cuuint32_t box[3] = {64, 1, (cuuint32_t)rows};
+    cuuint32_t es[3] = {1, 1, 1};
+    return fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+bool tc_fwd_supported(const carve_params_t& p)
+{
+    return p.dtype == CARVE_BF16 && p.dk == p.dv && (p.dk == 64 || p.dk == 128) && p.r <= 16;
+}
+
+size_t tc_state_tile_bytes(const carve_params_t& p) { return tc::tile_bytes(p.dv, p.dk); }
+
+template <int D>
+static cudaError_t launch_tc_fwd(const Args& a, uint8_t* ws_S, cudaStream_t st)
+{
+    const int LCc = a.L < tcp::LC ? a.L : tcp::LC;
+    CUtensorMap mq, mk, mv, mf, mbx, mwx;
+    if (!tc_make_token_map(&mq, a.q, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mk, a.k, a.B, a.T, a.H, D, LCc) ||
+        !tc_make_token_map(&mv, a.v, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mf, a.f, a.B, a.T, a.H, D, LCc) ||
+        !tc_make_token_map(&mbx, a.bx, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mwx, a.wx, a.B, a.T, a.H, D, LCc))
+        return cudaErrorInvalidValue;
+    TcArgs t{};
+    t.B = a.B; t.H = a.H; t.T = a.T; t.L = a.L; t.r = a.r; t.l2norm = a.l2norm; t.scale = a.scale; t.eps = a.eps;
+    t.beta = static_cast<const __nv_bfloat16*>(a.beta);
+    t.A = a.A; t.tau = a.tau; t.Ub = a.Ub; t.Uw = a.Uw; t.Vb = a.Vb; t.Vw = a.Vw; t.S0 = a.S0;
+    t.O = static_cast<__nv_bfloat16*>(a.O); t.S_final = a.S_final; t.ws_S = ws_S;
+    const size_t smem = tcp::Layout(D, D, 2 * a.r).total;
+    auto kern = carve_fwd_tc_kernel<D, D>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<a.B * a.H, tcp::NT, smem, st>>>(t, mq, mk, mv, mf, mbx, mwx);
+    return cudaGetLastError();
+}
+
+cudaError_t tc_fwd_launch(const Args& a, uint8_t* ws_S, cudaStream_t st)
+{
+    if (a.dk == 128) return launch_tc_fwd<128>(a, ws_S, st);
+    if (a.dk == 64) return launch_tc_fwd<64>(a, ws_S, st);
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace carve
