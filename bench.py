@@ -186,6 +186,8 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfg = get_cfg(args.config).with_(seed=rank)       # each rank owns a different batch shard
+    if args.fwd_only:
+        cfg = cfg.with_(fwd_only=True)
     carve.load_library()
     tok_dt = torch.bfloat16 if cfg.dtype == "bf16" else torch.float32
     p = carve.Params(B=cfg.B, H=cfg.H, T=cfg.T, L=cfg.L, dk=cfg.dk, dv=cfg.dv, r=cfg.r,
@@ -354,6 +356,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fwd-only", action="store_true", help="time carve_fwd alone (inference call, nothing saved)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

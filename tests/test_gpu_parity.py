@@ -13,12 +13,12 @@ pytestmark = pytest.mark.gpu
 TOL = {"f32": dict(O=1e-4, S=1e-4, g=1e-4), "bf16": dict(O=2e-2, S=2e-2, g=3e-2)}
 
 
-def _check_fwd_bwd(oracle, cfg, x, with_bwd=True, path=carve.CARVE_PATH_AUTO, ct=None):
+def _check_fwd_bwd(oracle, cfg, x, with_bwd=True, path=carve.CARVE_PATH_AUTO, ct=None, tol=None):
     p = params_of(cfg, path=path)
     s = oracle_shape(oracle, cfg)
     O_ref, S_ref = oracle.fwd(s, x)
     O, Sf, handles = run_fwd(p, x, need_bwd=with_bwd)
-    tol = TOL[cfg.dtype]
+    tol = tol or TOL[cfg.dtype]
     errs = {"O": relerr(O, O_ref), "S_final": relerr(Sf, S_ref)}
     assert np.isfinite(O).all() and np.isfinite(Sf).all()
     assert errs["O"] <= tol["O"], errs
@@ -85,12 +85,14 @@ def test_stress_conditioning(oracle):
 
 
 def test_extreme_decay_no_overflow(oracle):
-    """Strong decay/erase (log gamma_L ~ -600 per chunk): every ratio is formed as exp(<=0)."""
+    """Strong decay/erase (log gamma_L ~ -600 per chunk): every ratio is formed as exp(<=0).
+    Gradient tolerance 5e-4: an fp32 prefix sum of magnitude ~150 puts ~8e-6 absolute error
+    into every exp(lg_a - lg_b), and df sums ~1e2 such terms of both signs."""
     cfg = synth.Config("t", B=1, H=1, T=128, L=64, dk=64, dv=64, r=8, dtype="f32", wstd=0.1, s0_std=0.1, seed=4)
     x = synth.make_inputs(cfg)
     x["f"] = x["f"] + 5.0
     x["bx"] = x["bx"] + 5.0
-    _check_fwd_bwd(oracle, cfg, x)
+    _check_fwd_bwd(oracle, cfg, x, tol=dict(O=1e-4, S=1e-4, g=5e-4))
 
 
 # ---- invariants that need no oracle -------------------------------------------------------------
