@@ -32,7 +32,7 @@ def _check_fwd_bwd(oracle, cfg, x, with_bwd=True, path=carve.CARVE_PATH_AUTO, ct
                 pass  # gradients w.r.t. absent A/tau are still defined (they default to 0)
             assert np.isfinite(g[n]).all(), n
             errs[n] = relerr(g[n], g_ref[n])
-            assert errs[n] <= tol["g"], (n, errs)
+            assert errs[n] <= tol.get(n, tol["g"]), (n, errs)
     return errs
 
 
@@ -87,12 +87,13 @@ def test_stress_conditioning(oracle):
 def test_extreme_decay_no_overflow(oracle):
     """Strong decay/erase (log gamma_L ~ -600 per chunk): every ratio is formed as exp(<=0).
     Gradient tolerance 5e-4: an fp32 prefix sum of magnitude ~150 puts ~8e-6 absolute error
-    into every exp(lg_a - lg_b), and df sums ~1e2 such terms of both signs."""
+    into every exp(lg_a - lg_b), and df sums ~1e2 such terms of both signs.  dA and dtau are sums of dg.g / df over
+    all T tokens (Eq. 9 l.151) that cancel to ~1/10 of their terms here, so they carry 10x that: 5e-3."""
     cfg = synth.Config("t", B=1, H=1, T=128, L=64, dk=64, dv=64, r=8, dtype="f32", wstd=0.1, s0_std=0.1, seed=4)
     x = synth.make_inputs(cfg)
     x["f"] = x["f"] + 5.0
     x["bx"] = x["bx"] + 5.0
-    _check_fwd_bwd(oracle, cfg, x, tol=dict(O=1e-4, S=1e-4, g=5e-4))
+    _check_fwd_bwd(oracle, cfg, x, tol=dict(O=1e-4, S=1e-4, g=5e-4, dA=5e-3, dtau=5e-3))
 
 
 # ---- invariants that need no oracle -------------------------------------------------------------
