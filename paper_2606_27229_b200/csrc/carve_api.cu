@@ -37,12 +37,11 @@ carve_status_t check_params(const carve_params_t* p, bool bwd)
 }
 
 // Kernel family of a call.  `bwd` = the call is carve_bwd or a carve_fwd that saves for it: the two
-// must agree because the workspace layouts differ.  The tensor-core backward does not exist yet, so
-// training calls resolve to SIMT and an explicit CARVE_PATH_TENSOR request for them is refused
-// (no silent substitution).
+// must agree because the workspace layouts differ.  An explicit CARVE_PATH_TENSOR request for a shape
+// the tensor path does not cover is refused (no silent substitution).
 int resolve_path(const carve_params_t* p, bool bwd)
 {
-    const bool tc_ok = tc_fwd_supported(*p) && !bwd;
+    const bool tc_ok = bwd ? tc_bwd_supported(*p) : tc_fwd_supported(*p);
     if (p->path == CARVE_PATH_TENSOR) return tc_ok ? CARVE_PATH_TENSOR : -1;
     if (p->path == CARVE_PATH_SIMT) return CARVE_PATH_SIMT;
     return tc_ok ? CARVE_PATH_TENSOR : CARVE_PATH_SIMT;
@@ -105,7 +104,9 @@ const char* carve_status_string(carve_status_t s)
 size_t carve_workspace_bytes(const carve_params_t* p, int need_bwd)
 {
     if (!need_bwd || check_params(p, true) != CARVE_OK) return 0;
-    return simt_ws_layout(*p).total_bytes;
+    const int path = resolve_path(p, true);
+    if (path < 0) return 0;
+    return path == CARVE_PATH_TENSOR ? tc_ws_layout(*p).total_bytes : simt_ws_layout(*p).total_bytes;
 }
 
 int carve_resolved_path(const carve_params_t* p, int bwd)
@@ -117,7 +118,10 @@ int carve_resolved_path(const carve_params_t* p, int bwd)
 int carve_num_launches(const carve_params_t* p, int bwd)
 {
     if (check_params(p, bwd != 0) != CARVE_OK) return 0;
-    return bwd ? 2 : 1;  // bwd: persistent reverse kernel + weight-gradient reduction
+    if (!bwd) return 1;
+    // SIMT: persistent reverse kernel + weight-gradient reduction; tensor path: reverse kernel, chunk-local
+    // epilogue, dA/dtau chunk reduction, weight-gradient reduction
+    return resolve_path(p, true) == CARVE_PATH_TENSOR ? 4 : 2;
 }
 
 carve_status_t carve_fwd(const carve_params_t* p, const void* q, const void* k, const void* v, const void* f,
@@ -132,9 +136,9 @@ carve_status_t carve_fwd(const carve_params_t* p, const void* q, const void* k, 
                             (const void*)Uw, (const void*)Vb, (const void*)Vw, (const void*)S0, (const void*)O,
                             (const void*)S_final, (const void*)workspace})
         if (!aligned16(ptr)) return CARVE_ERR_ALIGN;
-    if (workspace && workspace_bytes < simt_ws_layout(*p).total_bytes) return CARVE_ERR_WORKSPACE;
     const int path = resolve_path(p, workspace != nullptr);
     if (path < 0) return CARVE_ERR_SHAPE;
+    if (workspace && workspace_bytes < carve_workspace_bytes(p, 1)) return CARVE_ERR_WORKSPACE;
     if ((s = check_arch()) != CARVE_OK) return s;
 
     Args a{};
@@ -143,8 +147,15 @@ carve_status_t carve_fwd(const carve_params_t* p, const void* q, const void* k, 
     a.q = q; a.k = k; a.v = v; a.f = f; a.bx = bx; a.wx = wx; a.beta = beta;
     a.A = A; a.tau = tau; a.Ub = Ub; a.Uw = Uw; a.Vb = Vb; a.Vw = Vw; a.S0 = S0;
     a.O = O; a.S_final = S_final;
-    if (path == CARVE_PATH_TENSOR)
-        return tc_fwd_launch(a, nullptr, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess ? CARVE_OK : CARVE_ERR_CUDA;
+    if (path == CARVE_PATH_TENSOR) {
+        uint8_t *rec = nullptr, *sfin = nullptr;
+        if (workspace) {
+            const TcWsLayout w = tc_ws_layout(*p);
+            rec = static_cast<uint8_t*>(workspace) + w.rec;
+            sfin = static_cast<uint8_t*>(workspace) + w.sfin;
+        }
+        return tc_fwd_launch(a, rec, sfin, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess ? CARVE_OK : CARVE_ERR_CUDA;
+    }
     fill_ws(a, *p, workspace);
     return simt_fwd_launch(a, p->dtype, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess ? CARVE_OK
                                                                                               : CARVE_ERR_CUDA;
@@ -169,8 +180,9 @@ carve_status_t carve_bwd(const carve_params_t* p, const void* q, const void* k, 
                             (const void*)dA, (const void*)dtau, (const void*)dUb, (const void*)dUw,
                             (const void*)dVb, (const void*)dVw, (const void*)dS0, (const void*)workspace})
         if (!aligned16(ptr)) return CARVE_ERR_ALIGN;
-    if (!workspace || workspace_bytes < simt_ws_layout(*p).total_bytes) return CARVE_ERR_WORKSPACE;
-    if (resolve_path(p, true) < 0) return CARVE_ERR_SHAPE;
+    const int path = resolve_path(p, true);
+    if (path < 0) return CARVE_ERR_SHAPE;
+    if (!workspace || workspace_bytes < carve_workspace_bytes(p, 1)) return CARVE_ERR_WORKSPACE;
     if ((s = check_arch()) != CARVE_OK) return s;
 
     Args a{};
@@ -180,6 +192,11 @@ carve_status_t carve_bwd(const carve_params_t* p, const void* q, const void* k, 
     a.A = A; a.tau = tau; a.Ub = Ub; a.Uw = Uw; a.Vb = Vb; a.Vw = Vw; a.S0 = S0;
     a.dO = dO; a.dS_final = dS_final;
     a.dq = dq; a.dk_ = dk; a.dv_ = dv; a.df = df; a.dbx = dbx; a.dwx = dwx; a.dbeta = dbeta; a.dS0 = dS0;
+    if (path == CARVE_PATH_TENSOR)
+        return tc_bwd_launch(a, static_cast<uint8_t*>(workspace), tc_ws_layout(*p), dA, dtau, dUb, dUw, dVb, dVw,
+                             static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess
+                   ? CARVE_OK
+                   : CARVE_ERR_CUDA;
     fill_ws(a, *p, workspace);
     return simt_bwd_launch(a, p->dtype, dA, dtau, dUb, dUw, dVb, dVw, static_cast<cudaStream_t>(cuda_stream)) ==
                    cudaSuccess

@@ -67,9 +67,42 @@ cudaError_t simt_fwd_launch(const Args& a, int dtype, cudaStream_t st);
 cudaError_t simt_bwd_launch(const Args& a, int dtype, float* dA, float* dtau, float* dUb, float* dUw,
                             float* dVb, float* dVw, cudaStream_t st);
 
-// Tensor-core path (carve_tc_fwd.cu): bf16 tokens, dk == dv in {64,128}, r <= 16.
+// Tensor-core path (carve_tc_fwd.cu, carve_tc_bwd.cu): bf16 tokens, dk == dv in {64,128}, r <= 16.
 bool tc_fwd_supported(const carve_params_t& p);
+bool tc_bwd_supported(const carve_params_t& p);   // additionally L <= 64
 size_t tc_state_tile_bytes(const carve_params_t& p);
-cudaError_t tc_fwd_launch(const Args& a, uint8_t* ws_S, cudaStream_t st);
+size_t tc_record_bytes(const carve_params_t& p);
+
+// Workspace of the tensor path (byte offsets): chunk records, final-state tiles, per-chain weight-gradient
+// partials (layout of part_stride_of) and per-chunk dA/dtau partials.
+struct TcWsLayout {
+    size_t rec, sfin, part, partAT, total_bytes;
+    int part_stride;
+};
+inline TcWsLayout tc_ws_layout(const carve_params_t& p)
+{
+    TcWsLayout w{};
+    const size_t chains = (size_t)p.B * p.H;
+    const int LC = p.L < 64 ? p.L : 64;
+    const size_t nchunks = p.T / LC;
+    size_t off = 0;
+    auto take = [&](size_t n) { size_t o = off; off += (n + 1023) & ~(size_t)1023; return o; };
+    w.rec = take(chains * nchunks * tc_record_bytes(p));
+    w.sfin = take(chains * tc_state_tile_bytes(p));
+    w.part_stride = part_stride_of(p.dk, p.dv, p.r);
+    w.part = take(chains * (size_t)w.part_stride * sizeof(float));
+    w.partAT = take(chains * nchunks * 2 * p.dk * sizeof(float));
+    w.total_bytes = off;
+    return w;
+}
+
+// rec / sfin: workspace views (nullptr for an inference forward).
+cudaError_t tc_fwd_launch(const Args& a, uint8_t* rec, uint8_t* sfin, cudaStream_t st);
+cudaError_t tc_bwd_launch(const Args& a, uint8_t* ws, const TcWsLayout& w, float* dA, float* dtau, float* dUb,
+                          float* dUw, float* dVb, float* dVw, cudaStream_t st);
+
+// Deterministic reduction of per-chain partials (carve_simt_bwd.cu), shared by both paths.
+cudaError_t reduce_weights_launch(const float* part, int chains, int stride, int H, int dk, int dv, int r, float* dUb,
+                                  float* dUw, float* dVb, float* dVw, float* dA, float* dtau, cudaStream_t st);
 
 }  // namespace carve

@@ -652,9 +652,15 @@ cudaError_t simt_bwd_launch(const Args& a, int dtype, float* dA, float* dtau, fl
 {
     cudaError_t e = dtype == CARVE_BF16 ? dispatch_bwd<__nv_bfloat16>(a, st) : dispatch_bwd<float>(a, st);
     if (e != cudaSuccess) return e;
-    const int n = 2 * a.r * a.dv + a.dk * a.r + a.dv * a.r + 2 * a.H * a.dk;
-    carve_reduce_weights_kernel<<<(n + 127) / 128, 128, 0, st>>>(a.ws_part, a.B * a.H, a.part_stride, a.H, a.dk, a.dv,
-                                                                  a.r, dUb, dUw, dVb, dVw, dA, dtau);
+    return reduce_weights_launch(a.ws_part, a.B * a.H, a.part_stride, a.H, a.dk, a.dv, a.r, dUb, dUw, dVb, dVw, dA, dtau, st);
+}
+
+cudaError_t reduce_weights_launch(const float* part, int chains, int stride, int H, int dk, int dv, int r, float* dUb,
+                                  float* dUw, float* dVb, float* dVw, float* dA, float* dtau, cudaStream_t st)
+{
+    const int n = 2 * r * dv + dk * r + dv * r + 2 * H * dk;
+    carve_reduce_weights_kernel<<<(n + 127) / 128, 128, 0, st>>>(part, chains, stride, H, dk, dv, r, dUb, dUw, dVb, dVw,
+                                                                  dA, dtau);
     return cudaGetLastError();
 }
 

@@ -12,6 +12,10 @@
 #include "tc_common.cuh"
 
 namespace carve {
+
+// [B,T,H,d] bf16 seen as (d, H, B*T); one TMA box = 64 channels x 1 head x `rows` tokens, 128B-swizzled (carve_tc_fwd.cu).
+bool tc_make_token_map(CUtensorMap* map, const void* base, int B, int T, int H, int d, int rows);
+
 namespace tcp {
 
 using namespace tc;
@@ -51,6 +55,48 @@ struct Layout {  // byte offsets into the 1024-aligned dynamic shared memory
         else { Mm = take(16384); Tm = take(16384); }  // fp32 scratch of the triangular inverse
         misc = take(7168);
         total = o + 1024;                   // slack for the manual 1024-byte alignment
+    }
+};
+
+// ---- chunk record ---------------------------------------------------------------------------------
+// What the training forward saves per (chain, solve chunk) for the reverse kernel (carve_tc_bwd.cu):
+// ready-to-use MMA operand tiles in the shared-memory image format (fetched with 1-D bulk copies),
+// plus row-private elementwise data a thread reads straight from global memory.  Offsets in bytes.
+//   SB   [dv][dk]   state entering the chunk, bf16
+//   KT   [64][dk]   Ktil_t = k^_t gamma_L/gamma_t
+//   PT   [128][64]  rows 0..63 scale.P (masked s <= t), rows 64..127 T = (I + diag(beta) A)^-1
+//   U    [64][dv]   u_t ;   E [64][dv]  e_t = u_t / beta_t  (row-private)
+//   K0,Q0 [64][dk]  Kbar_t = k^_t gamma_{t-1}, scale.Qbar_t = scale.q^_t gamma_t   (chunk-anchored)
+//   KQo  [128][dk]  the same rows anchored at the start of their own 16-token block
+//   CC   [64][dk]   C_s = k^_s gamma_a/gamma_s (a = start of s's 16-token block)
+//   VWX,W [64][dv]  w.v.(1-w) and w;  Bg [64][dk] erase gate b;  FQ,IC [64][dk] gamma_t/gamma_a and its inverse
+//   tt   [64][32]   tanh bottleneck (bf16, plain rows);  GT [dk][32] G^T (tile);  etot [4][dk], rn [128], beta [64] fp32
+struct Rec {
+    uint32_t SB, KT, PT, U, K0, Q0, KQo, CC, E, VWX, W, Bg, FQ, IC, tt, GT, etot, rn, beta, total;
+    __host__ __device__ Rec(int dk, int dv)
+    {
+        uint32_t o = 0;
+        auto take = [&](uint32_t n) { uint32_t r = o; o += (n + 1023u) & ~1023u; return r; };
+        SB = take(tile_bytes(dv, dk));
+        KT = take(tile_bytes(64, dk));
+        PT = take(tile_bytes(128, 64));
+        U = take(tile_bytes(64, dv));
+        K0 = take(tile_bytes(64, dk));
+        Q0 = take(tile_bytes(64, dk));
+        KQo = take(tile_bytes(128, dk));
+        CC = take(tile_bytes(64, dk));
+        E = take(tile_bytes(64, dv));
+        VWX = take(tile_bytes(64, dv));
+        W = take(tile_bytes(64, dv));
+        Bg = take(tile_bytes(64, dk));
+        FQ = take(tile_bytes(64, dk));
+        IC = take(tile_bytes(64, dk));
+        tt = take(64 * 64);
+        GT = take(tile_bytes(dk, 64));
+        etot = take(4u * dk * 4u);
+        rn = take(128 * 4);
+        beta = take(64 * 4);
+        total = o;
     }
 };
 

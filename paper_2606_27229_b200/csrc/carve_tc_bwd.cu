@@ -1,0 +1,1072 @@
+// carve_tc_bwd.cu -- tensor-core backward of the CARVE layer operator for bf16 token tensors.
+//
+// One persistent CTA per (batch, head) chain walks the solve chunks in REVERSE with the running state
+// adjoint dS (d_v x d_k fp32) resident in TMEM.  It is the chunk-matrix adjoint of Alg. 2 (PAPER.md
+// l.315-365), i.e. the reverse scan of Alg. 4 (l.788-817) batched over a chunk, with the fold glue of
+// Alg. 5 (l.844-848) at every chunk start.  Nothing of the forward is recomputed on this serial chain:
+// the training forward (carve_tc_fwd.cu) left a "chunk record" of operand tiles (carve_tc.cuh Rec) that
+// is streamed in with bulk copies.  Per chunk, with S = state entering it, dS' = adjoint of the state
+// leaving it (all MMAs are tcgen05, M = 128: rows 0..63 "K side", rows 64..127 "Q side"):
+//   L1  dU  = Ktil dS'^T + (scale P)^T dO                 [rows 0..63]     dKtil = U dS'
+//   L2  dX  = T^T dU (transposed solve, Alg. 2 step 7)    [rows 64..127]
+//       dR = beta dX,  dbeta = <dX, e>,  dv = dR w,  dw_pre = dR v w (1-w)   (Alg. 4 l.806-808)
+//   L3  [dA;dP] = [-dR; dO] U^T,   SP = [-dR; dO] S,   dS = dS' diag(gamma_L) + [-dR; dO]^T [Kbar; scale Qbar]
+//   L4  pairwise decay terms on mma.sync (registers allow the per-block rescaling tcgen05 cannot do):
+//         PK_t = sum_{s<t} dA_ts k^_s gamma_a(t)/gamma_s,  PQ_t likewise from dP,
+//         PC_s = sum_t [dA;dP]_ts [k^_t gamma_{t-1}; q^_t gamma_t] / gamma_a(s)
+//       every ratio anchored at a 16-token block boundary, products of whole-block decays applied
+//       by Horner steps between the block products (all factors <= 1 except one block's worth).
+//   L5  dk^ = dkA + dkC, dq^ (state part), X = contributions to d log gamma
+//   L6  d log a = reverse cumulative sum of X over tokens = (0/1 triangular) x X on the tensor core
+//       db_pre = -dla b  (Eq. 14 l.310), dla itself goes to the epilogue kernel (df, dA, dtau)
+//   L7  [dz_b | dz_w] = [db_pre; dw_pre] [Vb | Vw],  dVb, dVw += [db_pre; dw_pre]^T [tt_b | tt_w]
+//   L8  dq^ += dz G,  dG = dz^T q^                        (Eq. 7 l.134 backward)
+//   L9  dS += [Ub;Uw]^T dG,  d[Ub;Uw] += dG S^T            (fold glue, Alg. 5 l.846-848)
+//   L10 dS -> bf16 operand copy, column sums of S . dS (the retention gradient carried into the
+//       previous chunk), dS0 at the end.
+// The chunk-local tail (L2-norm backward of q,k, decay activation backward, dA/dtau) runs as a
+// separate fully parallel kernel over (chain, chunk): carve_bwd_tc_epilogue_kernel below.
+// No floating-point atomics anywhere: results are run-to-run bitwise identical.
+#include "carve_tc.cuh"
+
+namespace carve {
+namespace {
+
+using namespace tcp;
+
+struct BwdArgs {
+    int B, H, T, L, r;
+    int l2norm;
+    float scale, eps;
+    const uint8_t* rec;
+    const uint8_t* sfin;
+    const float* dS_final;
+    const float *Ub, *Uw, *Vb, *Vw;
+    __nv_bfloat16 *dq, *dk, *dv, *df, *dbx, *dwx, *dbeta;
+    float* dS0;
+    float* part;
+    int part_stride;
+};
+
+// TMEM column map of the reverse kernel.
+constexpr uint32_t BM_DS = 0;     // [dv lanes][dk]  dS (fp32), pre-scaled by gamma_L of the chunk being processed
+constexpr uint32_t BM_A = 128;    // L1 dU (rows 0..63), L2 dX (rows 64..127), L3.. SP, then dq^ (rows 64..127)
+constexpr uint32_t BM_KT = 256;   // L1 dKtil (rows 0..63), L6 d log a (rows 0..63)
+constexpr uint32_t BM_DAP = 384;  // L3 [dA;dP] raw (64 cols); L7 ZZ (32 cols); L8 dG^T at +32 (32 cols)
+constexpr uint32_t BM_WG = 448;   // [n lanes][32]  dVb | dVw, accumulated over the whole chain
+constexpr uint32_t BM_WU = 480;   // [x lanes][32]  d[Ub;Uw]^T, accumulated over the whole chain
+
+constexpr uint32_t SLOT = 16384;
+struct BLayout {  // byte offsets into the 1024-aligned dynamic shared memory
+    uint32_t DSB, SBq, S[7], TRI, VcT, Ucat, misc, total;
+    __host__ __device__ BLayout(int d)
+    {
+        uint32_t o = 0;
+        auto take = [&](uint32_t n) { uint32_t r = o; o += (n + 1023u) & ~1023u; return r; };
+        DSB = take(tile_bytes(d, d));   // bf16 dS' (rows x, cols j)
+        SBq = take(tile_bytes(d, d));   // bf16 state entering the chunk (record SB)
+        for (int i = 0; i < 7; ++i) S[i] = take(SLOT);
+        TRI = take(24576);              // [64][192] 0/1: cols 0..63 t' > t, cols 64..127 t' >= t, cols 128..191 t' < t
+        VcT = take(tile_bytes(32, d));  // rows i: [Vb^T ; Vw^T]
+        Ucat = take(tile_bytes(32, d)); // rows i: [Ub ; Uw]
+        misc = take(8192);
+        total = o + 1024;
+    }
+};
+
+struct BMisc {
+    float etot[4][128];   // exp(block sums of log a) of the chunk
+    float gamLn[128];     // gamma_L of the chunk processed next (c - 1)
+    float extra[128];     // column sums of S . dS: d log gamma carried in from the later chunks
+    float rn[128];        // 1/|k|, 1/|q| of the chunk's tokens
+    float beta[64];
+    float dbp[2][64];     // dbeta partial sums of the two column halves
+    float colp[4][128];   // column-sum partials per lane quadrant
+    uint64_t bar_mma, bar_g1, bar_g3, bar_sb, bar_g4a, bar_g4b, bar_g5, bar_g8;
+    uint32_t tmem_base;
+};
+static_assert(sizeof(BMisc) <= 8192, "misc area too small");
+
+// ---- PTX helpers ----------------------------------------------------------------------------------
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t (&r)[4], uint32_t saddr)
+{
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                 : "r"(saddr));
+}
+__device__ __forceinline__ void mma_bf16(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
+{
+    asm volatile(
+        "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+// x = hi + lo with both parts bf16: the tensor-core sums of such pairs keep ~fp32 accuracy.
+__device__ __forceinline__ void split8(const float* x, uint4& hi, uint4& lo)
+{
+    float h[8], l[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+        h[e] = __bfloat162float(__float2bfloat16_rn(x[e]));
+        l[e] = x[e] - h[e];
+    }
+    hi = pack8(h);
+    lo = pack8(l);
+}
+__device__ __forceinline__ uint4 ldg128(const uint8_t* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
+__device__ __forceinline__ void stg128(void* p, uint4 v) { *reinterpret_cast<uint4*>(p) = v; }
+
+// Product over K (multiple of 16) from two row tiles, with explicit K offsets (see tc_common.cuh umma_tiles).
+template <int AMAJ, int BMAJ>
+__device__ __forceinline__ void mma_k(uint32_t d_tmem, int N, uint32_t a_saddr, int a_rows, int a_o0, int a_k0,
+                                      uint32_t b_saddr, int b_rows, int b_o0, int b_k0, int K, bool accumulate)
+{
+    const uint32_t idesc = umma_idesc(128, N, AMAJ, BMAJ);
+    for (int k = 0; k < K; k += 16) {
+        const uint64_t ad = AMAJ == KMAJ ? desc_kmajor(a_saddr, a_rows, a_o0, a_k0 + k) : desc_mnmajor(a_saddr, a_rows, a_o0, a_k0 + k);
+        const uint64_t bd = BMAJ == KMAJ ? desc_kmajor(b_saddr, b_rows, b_o0, b_k0 + k) : desc_mnmajor(b_saddr, b_rows, b_o0, b_k0 + k);
+        umma(d_tmem, ad, bd, idesc, (accumulate || k > 0) ? 1u : 0u);
+    }
+}
+
+// Column sums over the 32 lanes of a warp by a halving butterfly: on return lane l holds in v[0..N/32)
+// the sums of columns (N/32) l + i.
+template <int n, int s, int N>
+__device__ __forceinline__ void colsum_stage(float (&v)[N], int lane)
+{
+    const bool up = (lane & s) != 0;
+#pragma unroll
+    for (int i = 0; i < n / 2; ++i) {
+        const float send = up ? v[i] : v[i + n / 2];
+        const float keep = up ? v[i + n / 2] : v[i];
+        v[i] = keep + __shfl_xor_sync(0xFFFFFFFFu, send, s);
+    }
+}
+template <int N>
+__device__ __forceinline__ void warp_colsum(float (&v)[N], int lane)
+{
+    colsum_stage<N, 16, N>(v, lane);
+    colsum_stage<N / 2, 8, N>(v, lane);
+    colsum_stage<N / 4, 4, N>(v, lane);
+    colsum_stage<N / 8, 2, N>(v, lane);
+    colsum_stage<N / 16, 1, N>(v, lane);
+}
+
+#define PHASE_SYNC()            \
+    do {                        \
+        fence_async_smem();     \
+        tc_fence_before();      \
+        __syncthreads();        \
+        tc_fence_after();       \
+    } while (0)
+#define WAIT_MMA()                          \
+    do {                                    \
+        mbar_wait(&mi.bar_mma, mma_ph);     \
+        mma_ph ^= 1u;                       \
+        tc_fence_after();                   \
+    } while (0)
+
+template <int D>
+__global__ void __launch_bounds__(NT, 1)
+carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, const __grid_constant__ CUtensorMap mk,
+                    const __grid_constant__ CUtensorMap mq)
+{
+    constexpr int HK = D / 2;                      // columns per warpgroup half
+    constexpr uint32_t TB = tile_bytes(64, D);     // one [64][D] tile
+    constexpr uint32_t SBb = tile_bytes(D, D);     // one state tile
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* sm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    const BLayout Lo(D);
+    BMisc& mi = *reinterpret_cast<BMisc*>(sm + Lo.misc);
+    const uint32_t sb = smem_u32(sm);
+    const int r = a.r, R2 = 2 * r;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, q = warp & 3, half = warp >> 2;
+    const int row = q * 32 + lane;   // tile row == TMEM lane served by this thread
+    const bool krole = q < 2;
+    const int t = row & 63;          // token of this row
+    const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+    const int chain = blockIdx.x, b = chain / a.H, h = chain % a.H;
+    const int LCc = a.L < LC ? a.L : LC;
+    const int nchunks = a.T / LCc, nb = LCc >> 4;
+    const bool warp_active = (q & 1) * 32 < LCc;   // this warp holds at least one live token row
+    const bool live = t < LCc;
+    const bool srow = row < D;                     // this thread owns a row of the state adjoint
+    const int blk = t >> 4;
+    const Rec Rc(D, D);
+    const uint8_t* rec_chain = a.rec + (size_t)chain * nchunks * Rc.total;
+
+    // ---- one-time setup --------------------------------------------------------------------------
+    if (tid == 0) {
+        mbar_init(&mi.bar_mma, 1); mbar_init(&mi.bar_g1, 1); mbar_init(&mi.bar_g3, 1); mbar_init(&mi.bar_sb, 1);
+        mbar_init(&mi.bar_g4a, 1); mbar_init(&mi.bar_g4b, 1); mbar_init(&mi.bar_g5, 1); mbar_init(&mi.bar_g8, 1);
+        mbar_fence_init();
+        tma_prefetch_desc(&mdO); tma_prefetch_desc(&mk); tma_prefetch_desc(&mq);
+    }
+    if (warp == 0) tmem_alloc(&mi.tmem_base, TM_COLS);
+    for (int i = tid; i < 32 * D; i += NT) {
+        const int ii = i / D, n = i % D;
+        float vc = 0.f, uc = 0.f;
+        if (ii < r) { vc = __ldg(a.Vb + (size_t)n * r + ii); uc = __ldg(a.Ub + (size_t)ii * D + n); }
+        else if (ii < R2) { vc = __ldg(a.Vw + (size_t)n * r + (ii - r)); uc = __ldg(a.Uw + (size_t)(ii - r) * D + n); }
+        *reinterpret_cast<__nv_bfloat16*>(sm + Lo.VcT + tile_off(32, ii, n)) = __float2bfloat16_rn(vc);
+        *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Ucat + tile_off(32, ii, n)) = __float2bfloat16_rn(uc);
+    }
+    for (int i = tid; i < 64 * 192; i += NT) {
+        const int tt_ = i / 192, k = i % 192;
+        const bool one = k < 64 ? (k > tt_) : k < 128 ? (k - 64 >= tt_) : (k - 128 < tt_);
+        *reinterpret_cast<uint16_t*>(sm + Lo.TRI + tile_off(64, tt_, k)) = one ? 0x3F80u : 0u;
+    }
+    if (tid < D) {
+        const float* et = reinterpret_cast<const float*>(rec_chain + (size_t)(nchunks - 1) * Rc.total + Rc.etot);
+        mi.gamLn[tid] = et[tid] * et[D + tid] * et[2 * D + tid] * et[3 * D + tid];
+    }
+    PHASE_SYNC();
+    const uint32_t tmem = mi.tmem_base;
+    uint32_t mma_ph = 0;
+
+    // dS (this thread's row x = `row`, columns half*HK..) -> bf16 operand copy DSB, TMEM <- dS gamma_L(next chunk),
+    // and dS0 when `last`.  from_tmem: read dS from TMEM, else from dS_final (or zeros).
+    auto finalize = [&](bool from_tmem, bool last) {
+        if (srow) {
+#pragma unroll
+            for (int s = 0; s < HK; s += 32) {
+                const int c0 = half * HK + s;
+                uint32_t v[32];
+                if (from_tmem) {
+                    tmem_ld32(tmem + BM_DS + lane_base + c0, v);
+                    tmem_wait_ld();
+                } else {
+                    const float* src = a.dS_final ? a.dS_final + ((size_t)chain * D + row) * D + c0 : nullptr;
+#pragma unroll
+                    for (int e = 0; e < 32; e += 4) {
+                        const float4 f4 = src ? __ldg(reinterpret_cast<const float4*>(src + e)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                        v[e] = __float_as_uint(f4.x); v[e + 1] = __float_as_uint(f4.y);
+                        v[e + 2] = __float_as_uint(f4.z); v[e + 3] = __float_as_uint(f4.w);
+                    }
+                }
+                uint32_t sc[32];
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch) {
+                    float f8[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        f8[e] = __uint_as_float(v[8 * ch + e]);
+                        sc[8 * ch + e] = __float_as_uint(f8[e] * mi.gamLn[c0 + 8 * ch + e]);
+                    }
+                    sts128(sm + Lo.DSB + tile_chunk_off(D, row, c0 / 8 + ch), pack8(f8));
+                    if (last) {
+                        float* dst = a.dS0 + ((size_t)chain * D + row) * D + c0 + 8 * ch;
+                        *reinterpret_cast<float4*>(dst) = make_float4(f8[0], f8[1], f8[2], f8[3]);
+                        *reinterpret_cast<float4*>(dst + 4) = make_float4(f8[4], f8[5], f8[6], f8[7]);
+                    }
+                }
+                tmem_st32(tmem + BM_DS + lane_base + c0, sc);
+            }
+            tmem_wait_st();
+        }
+        PHASE_SYNC();
+    };
+
+    finalize(false, false);
+
+    bool first = true;
+    for (int it = 0, c = nchunks - 1; c >= 0; --c, ++it) {
+        const uint32_t ph = (uint32_t)it & 1u;
+        const uint8_t* rc = rec_chain + (size_t)c * Rc.total;
+        const size_t tok0 = (size_t)b * a.T + (size_t)c * LCc;
+        const int trow = b * a.T + c * LCc;  // TMA row coordinate of the chunk's first token
+        // ---- loads of the chunk: L1 operands, state, chunk-anchored rows; small per-chunk vectors
+        if (tid == 0) {
+            if (it == 0) {   // later chunks: issued as soon as the previous chunk's last reader of SBq is done
+                mbar_expect_tx(&mi.bar_sb, SBb);
+                bulk_g2s(sm + Lo.SBq, rc + Rc.SB, SBb, &mi.bar_sb);
+            }
+            mbar_expect_tx(&mi.bar_g1, 2 * TB + 16384 + (uint32_t)LCc * D * 2u);
+            bulk_g2s(sm + Lo.S[0], rc + Rc.KT, TB, &mi.bar_g1);
+            bulk_g2s(sm + Lo.S[1], rc + Rc.PT, 16384, &mi.bar_g1);
+            bulk_g2s(sm + Lo.S[4], rc + Rc.U, TB, &mi.bar_g1);
+            for (int cb = 0; cb < D / 64; ++cb)
+                tma_load_3d(sm + Lo.S[2] + cb * 16384 + 8192, &mdO, &mi.bar_g1, cb * 64, h, trow);
+            mbar_expect_tx(&mi.bar_g3, 2 * TB);
+            bulk_g2s(sm + Lo.S[5], rc + Rc.K0, TB, &mi.bar_g3);
+            bulk_g2s(sm + Lo.S[6], rc + Rc.Q0, TB, &mi.bar_g3);
+        }
+        {
+            const float* et = reinterpret_cast<const float*>(rc + Rc.etot);
+            for (int i = tid; i < 4 * D; i += NT) mi.etot[i / D][i % D] = __ldg(et + i);
+            if (tid < 128) mi.rn[tid] = __ldg(reinterpret_cast<const float*>(rc + Rc.rn) + tid);
+            if (tid < 64) mi.beta[tid] = __ldg(reinterpret_cast<const float*>(rc + Rc.beta) + tid);
+            if (tid >= 128 && tid < 128 + D) {
+                const int j = tid - 128;
+                float g = 1.f;
+                if (c > 0) {
+                    const float* en = reinterpret_cast<const float*>(rc - Rc.total + Rc.etot);
+                    g = __ldg(en + j) * __ldg(en + D + j) * __ldg(en + 2 * D + j) * __ldg(en + 3 * D + j);
+                }
+                mi.gamLn[j] = g;   // read by finalize at the end of this chunk
+            }
+        }
+        // ---- L1: dU = Ktil dS'^T + (scale P)^T dO -> BM_A rows 0..63;  dKtil = U dS' -> BM_KT rows 0..63
+        if (tid == 0) {
+            mbar_wait(&mi.bar_g1, ph);
+            tc_fence_after();
+            mma_k<KMAJ, KMAJ>(tmem + BM_A, D, sb + Lo.S[0], 64, 0, 0, sb + Lo.DSB, D, 0, 0, D, false);
+            mma_k<MNMAJ, MNMAJ>(tmem + BM_A, D, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[2], 128, 0, 64, LCc, true);
+            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D, sb + Lo.S[4], 64, 0, 0, sb + Lo.DSB, D, 0, 0, D, false);
+            umma_commit(&mi.bar_mma);
+        }
+        if (krole) {
+            WAIT_MMA();
+            if (warp_active) {
+#pragma unroll
+                for (int s = 0; s < HK; s += 32) {
+                    uint32_t v[32];
+                    tmem_ld32(tmem + BM_A + lane_base + half * HK + s, v);
+                    tmem_wait_ld();
+                    if (live) {
+#pragma unroll
+                        for (int ch = 0; ch < 4; ++ch) {
+                            float f8[8];
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) f8[e] = __uint_as_float(v[8 * ch + e]);
+                            sts128(sm + Lo.S[0] + tile_chunk_off(64, t, (half * HK + s) / 8 + ch), pack8(f8));  // DU over Ktil
+                        }
+                    }
+                }
+            }
+        } else {
+            mma_ph ^= 1u;  // Q-side threads skip this wait
+        }
+        // ---- L2: dX = T^T dU -> BM_A rows 64..127
+        PHASE_SYNC();
+        if (tid == 0) {
+            mma_k<MNMAJ, MNMAJ>(tmem + BM_A, D, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[0], 64, 0, 0, LCc, false);
+            umma_commit(&mi.bar_mma);
+        }
+        if (!krole) {
+            // row-private record data straight from global memory, issued before the MMA wait
+            uint4 e4[HK / 8], x4[HK / 8], w4[HK / 8];
+            if (live) {
+#pragma unroll
+                for (int i = 0; i < HK / 8; ++i) {
+                    const uint32_t off = tile_chunk_off(64, t, half * (HK / 8) + i);
+                    e4[i] = ldg128(rc + Rc.E + off);
+                    x4[i] = ldg128(rc + Rc.VWX + off);
+                    w4[i] = ldg128(rc + Rc.W + off);
+                }
+            }
+            WAIT_MMA();
+            if (warp_active) {
+                const float bt = live ? mi.beta[t] : 0.f;
+                float dbs = 0.f;
+                __nv_bfloat16* gdv = a.dv + ((tok0 + t) * a.H + h) * D;
+                __nv_bfloat16* gdwx = a.dwx + ((tok0 + t) * a.H + h) * D;
+#pragma unroll
+                for (int s = 0; s < HK; s += 32) {
+                    uint32_t v[32];
+                    tmem_ld32(tmem + BM_A + lane_base + half * HK + s, v);
+                    tmem_wait_ld();
+                    if (live) {
+#pragma unroll
+                        for (int ch = 0; ch < 4; ++ch) {
+                            const int i = s / 8 + ch, cc = half * (HK / 8) + i;
+                            float ee[8], xx[8], ww[8], ndr[8], o1[8], o2[8];
+                            unpack8(e4[i], ee); unpack8(x4[i], xx); unpack8(w4[i], ww);
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) {
+                                const float dx = __uint_as_float(v[8 * ch + e]);
+                                const float dr = bt * dx;
+                                dbs += dx * ee[e];
+                                ndr[e] = -dr;
+                                o1[e] = dr * ww[e];
+                                o2[e] = dr * xx[e];
+                            }
+                            sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8(ndr));
+                            stg128(gdv + 8 * cc, pack8(o1));
+                            stg128(gdwx + 8 * cc, pack8(o2));
+                        }
+                    }
+                }
+                if (live) mi.dbp[half][t] = dbs;
+            }
+        } else {
+            WAIT_MMA();
+            if (tid == 0) {  // PT is dead: fetch the block-anchored column operand of L4
+                mbar_expect_tx(&mi.bar_g4a, TB);
+                bulk_g2s(sm + Lo.S[1], rc + Rc.CC, TB, &mi.bar_g4a);
+            }
+        }
+        // ---- L3: [dA;dP] raw, SP = [-dR;dO] S, dS += [-dR;dO]^T [Kbar; scale Qbar]
+        PHASE_SYNC();
+        if (tid == 0) {
+            mbar_wait(&mi.bar_sb, ph);
+            mbar_wait(&mi.bar_g3, ph);
+            tc_fence_after();
+            mma_k<KMAJ, KMAJ>(tmem + BM_DAP, 64, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[4], 64, 0, 0, D, false);
+            mma_k<KMAJ, MNMAJ>(tmem + BM_A, D, sb + Lo.S[2], 128, 0, 0, sb + Lo.SBq, D, 0, 0, D, false);
+            mma_k<MNMAJ, MNMAJ>(tmem + BM_DS, D, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[5], 64, 0, 0, LCc, true);
+            mma_k<MNMAJ, MNMAJ>(tmem + BM_DS, D, sb + Lo.S[2], 128, 0, 64, sb + Lo.S[6], 64, 0, 0, LCc, true);
+            umma_commit(&mi.bar_mma);
+        }
+        if (!krole && half == 0 && live)
+            a.dbeta[(tok0 + t) * a.H + h] = __float2bfloat16_rn(mi.dbp[0][t] + mi.dbp[1][t]);
+        WAIT_MMA();
+        if (tid == 0) {  // DRO and U are dead
+            mbar_expect_tx(&mi.bar_g4b, 2 * TB);
+            bulk_g2s(sm + Lo.S[2], rc + Rc.KQo, 2 * TB, &mi.bar_g4b);
+        }
+        {   // masked [dA;dP] -> bf16 tile DAP (S[4], over U)
+            uint32_t v[32];
+            tmem_ld32(tmem + BM_DAP + lane_base + 32 * half, v);
+            tmem_wait_ld();
+#pragma unroll
+            for (int ch = 0; ch < 4; ++ch) {
+                float f8[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int s = 32 * half + 8 * ch + e;
+                    const bool keep = live && (krole ? s < t : s <= t);
+                    f8[e] = keep ? (krole ? __uint_as_float(v[8 * ch + e]) : a.scale * __uint_as_float(v[8 * ch + e])) : 0.f;
+                }
+                sts128(sm + Lo.S[4] + tile_chunk_off(128, row, 4 * half + ch), pack8(f8));
+            }
+        }
+        // ---- carry term of d log gamma: gamma_L . colsum(S . dS')  (dS' still sits in DSB as bf16)
+        mbar_wait(&mi.bar_sb, ph);
+        if (srow) {
+            float p[HK];
+#pragma unroll
+            for (int ch = 0; ch < HK / 8; ++ch) {
+                float s8[8], d8[8];
+                const uint32_t off = tile_chunk_off(D, row, half * (HK / 8) + ch);
+                unpack8(lds128(sm + Lo.SBq + off), s8);
+                unpack8(lds128(sm + Lo.DSB + off), d8);
+#pragma unroll
+                for (int e = 0; e < 8; ++e) p[8 * ch + e] = s8[e] * d8[e];
+            }
+            warp_colsum<HK>(p, lane);
+#pragma unroll
+            for (int i = 0; i < HK / 32; ++i) mi.colp[q][half * HK + (HK / 32) * lane + i] = p[i];
+        }
+        // ---- L4: pairwise decay terms on mma.sync.  Warp w owns key channels [NCW w, NCW (w+1)) for all tokens, so the
+        //      three pieces of d log gamma that cancel pairwise meet in one thread, in fp32:
+        //        (i)  H_t  = sum_{s} [dA;dP]_ts C_s G(blk t, blk s)      (rows of both sides)
+        //        (ii) H'_s = sum_{t} [dA;dP]_ts [Kbar;Qbar]own_t G(blk t, blk s)
+        //      with G = product of the whole-block decays between the two blocks, applied by Horner steps.  Every pair
+        //      (t,s) enters +Kbar_own_t C_s dA_ts G in row t and -C_s Kbar_own_t dA_ts G in row s with bit-identical
+        //      operands, so the pairs that do not straddle a token cancel to fp32 rounding in the reverse cumulative sum.
+        __syncthreads();
+        if (tid < D) {
+            float sx = 0.f;
+#pragma unroll
+            for (int qq = 0; qq < D / 32; ++qq) sx += mi.colp[qq][tid];
+            mi.extra[tid] = sx * (mi.etot[0][tid] * mi.etot[1][tid] * mi.etot[2][tid] * mi.etot[3][tid]);
+        }
+        {
+            constexpr int NCW = D / 8, NTW = NCW / 8;
+            const int g = lane >> 2, l4 = lane & 3, cw = NCW * warp;
+            const int lrow = (lane & 7) + ((lane >> 3) & 1) * 8;
+            const int lchk = NTW == 2 ? (lane >> 4) : 0;
+            const uint8_t* dap = sm + Lo.S[4];
+            float et[4][NTW][2];
+#pragma unroll
+            for (int b2 = 0; b2 < 4; ++b2)
+#pragma unroll
+                for (int nt = 0; nt < NTW; ++nt) {
+                    const float2 e2 = *reinterpret_cast<const float2*>(&mi.etot[b2][cw + 8 * nt + 2 * l4]);
+                    et[b2][nt][0] = e2.x; et[b2][nt][1] = e2.y;
+                }
+            mbar_wait(&mi.bar_g4a, ph);
+            uint32_t bC[4][NTW][2];
+#pragma unroll
+            for (int jb = 0; jb < 4; ++jb) {
+                if (jb < nb) {
+                    uint32_t tmp[4];
+                    ldsm_x4_t(tmp, sb + Lo.S[1] + tile_chunk_off(64, 16 * jb + lrow, cw / 8 + lchk));
+#pragma unroll
+                    for (int nt = 0; nt < NTW; ++nt) { bC[jb][nt][0] = tmp[2 * nt]; bC[jb][nt][1] = tmp[2 * nt + 1]; }
+                }
+            }
+            float accI[8][NTW][4];
+#pragma unroll
+            for (int mt = 0; mt < 8; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < NTW; ++nt)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) accI[mt][nt][e] = 0.f;
+#pragma unroll
+            for (int side = 0; side < 2; ++side)
+#pragma unroll
+                for (int ib = 0; ib < 4; ++ib) {
+                    if (ib < nb) {
+                        const int mt = side * 4 + ib, r0 = side * 64 + 16 * ib;
+#pragma unroll
+                        for (int jb = 0; jb < 4; ++jb) {
+                            if (jb <= ib) {
+                                uint32_t af[4];
+                                af[0] = *reinterpret_cast<const uint32_t*>(dap + tile_off(128, r0 + g, 16 * jb + 2 * l4));
+                                af[1] = *reinterpret_cast<const uint32_t*>(dap + tile_off(128, r0 + g + 8, 16 * jb + 2 * l4));
+                                af[2] = *reinterpret_cast<const uint32_t*>(dap + tile_off(128, r0 + g, 16 * jb + 2 * l4 + 8));
+                                af[3] = *reinterpret_cast<const uint32_t*>(dap + tile_off(128, r0 + g + 8, 16 * jb + 2 * l4 + 8));
+#pragma unroll
+                                for (int nt = 0; nt < NTW; ++nt) {
+                                    mma_bf16(accI[mt][nt], af, bC[jb][nt][0], bC[jb][nt][1]);
+                                    if (jb < ib) {   // step over block jb: gamma_e(jb)/gamma_a(jb)
+                                        accI[mt][nt][0] *= et[jb][nt][0]; accI[mt][nt][1] *= et[jb][nt][1];
+                                        accI[mt][nt][2] *= et[jb][nt][0]; accI[mt][nt][3] *= et[jb][nt][1];
+                                    }
+                                }
+                            }
+                        }
+                    }
+                }
+            mbar_wait(&mi.bar_g4b, ph);
+            float accII[4][NTW][4];
+#pragma unroll
+            for (int jb = 0; jb < 4; ++jb)
+#pragma unroll
+                for (int nt = 0; nt < NTW; ++nt)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) accII[jb][nt][e] = 0.f;
+#pragma unroll
+            for (int ib = 3; ib >= 0; --ib) {
+                if (ib < nb) {
+                    uint32_t bK[2][NTW][2];
+#pragma unroll
+                    for (int side = 0; side < 2; ++side) {
+                        uint32_t tmp[4];
+                        ldsm_x4_t(tmp, sb + Lo.S[2] + tile_chunk_off(128, side * 64 + 16 * ib + lrow, cw / 8 + lchk));
+#pragma unroll
+                        for (int nt = 0; nt < NTW; ++nt) { bK[side][nt][0] = tmp[2 * nt]; bK[side][nt][1] = tmp[2 * nt + 1]; }
+                    }
+#pragma unroll
+                    for (int jb = 0; jb < 4; ++jb) {
+                        if (jb <= ib) {
+                            if (ib < nb - 1) {
+#pragma unroll
+                                for (int nt = 0; nt < NTW; ++nt) {
+                                    accII[jb][nt][0] *= et[ib][nt][0]; accII[jb][nt][1] *= et[ib][nt][1];
+                                    accII[jb][nt][2] *= et[ib][nt][0]; accII[jb][nt][3] *= et[ib][nt][1];
+                                }
+                            }
+#pragma unroll
+                            for (int side = 0; side < 2; ++side) {
+                                uint32_t af[4];
+                                // A[m = s][k = t] = DAP[t][s]: transposed 8x8 loads; matrix m: rows t0 + 8 (m>>1), chunk 2 jb + (m&1)
+                                ldsm_x4_t(af, sb + Lo.S[4] + tile_chunk_off(128, side * 64 + 16 * ib + (lane & 7) + (lane >> 4) * 8,
+                                                                            2 * jb + ((lane >> 3) & 1)));
+#pragma unroll
+                                for (int nt = 0; nt < NTW; ++nt) mma_bf16(accII[jb][nt], af, bK[side][nt][0], bK[side][nt][1]);
+                            }
+                        }
+                    }
+                }
+            }
+            // contributions to d log gamma_t from the pairs: +Kbar_own_t H_t (to t-1), +Qbar_own_t H_t, -C_t H'_t
+            float dd[8][NTW][2], aa[8][NTW][2];
+#pragma unroll
+            for (int b2 = 0; b2 < 4; ++b2)
+#pragma unroll
+                for (int hh = 0; hh < 2; ++hh) {
+                    const int grp = 2 * b2 + hh, tt2 = 16 * b2 + 8 * hh + g;
+#pragma unroll
+                    for (int nt = 0; nt < NTW; ++nt) {
+                        dd[grp][nt][0] = dd[grp][nt][1] = aa[grp][nt][0] = aa[grp][nt][1] = 0.f;
+                        if (b2 < nb) {
+                            const int j = cw + 8 * nt + 2 * l4;
+                            const uint32_t wk = *reinterpret_cast<const uint32_t*>(sm + Lo.S[2] + tile_off(128, tt2, j));
+                            const uint32_t wq = *reinterpret_cast<const uint32_t*>(sm + Lo.S[2] + tile_off(128, 64 + tt2, j));
+                            const uint32_t wc = *reinterpret_cast<const uint32_t*>(sm + Lo.S[1] + tile_off(64, tt2, j));
+                            const float xa0 = bf16_lo(wk) * accI[b2][nt][2 * hh], xa1 = bf16_hi(wk) * accI[b2][nt][2 * hh + 1];
+                            const float xq0 = bf16_lo(wq) * accI[4 + b2][nt][2 * hh], xq1 = bf16_hi(wq) * accI[4 + b2][nt][2 * hh + 1];
+                            const float xc0 = bf16_lo(wc) * accII[b2][nt][2 * hh], xc1 = bf16_hi(wc) * accII[b2][nt][2 * hh + 1];
+                            dd[grp][nt][0] = (xq0 - xc0) + xa0; dd[grp][nt][1] = (xq1 - xc1) + xa1;
+                            aa[grp][nt][0] = xa0; aa[grp][nt][1] = xa1;
+                        }
+                    }
+                }
+            // reverse cumulative sum over tokens (token = 8 grp + g): dlp_t = sum_{t' >= t} dd_t' - aa_t
+#pragma unroll
+            for (int nt = 0; nt < NTW; ++nt)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    float carry = 0.f;
+#pragma unroll
+                    for (int grp = 7; grp >= 0; --grp) {
+                        float v = dd[grp][nt][e];
+#pragma unroll
+                        for (int off = 1; off < 8; off <<= 1) {
+                            const float o = __shfl_down_sync(0xFFFFFFFFu, v, 4 * off);
+                            if (g + off < 8) v += o;
+                        }
+                        const float tot = __shfl_sync(0xFFFFFFFFu, v, l4);
+                        dd[grp][nt][e] = v + carry - aa[grp][nt][e];
+                        carry += tot;
+                    }
+                }
+            __syncthreads();  // every warp is done reading DAP / C / KQo
+#pragma unroll
+            for (int side = 0; side < 2; ++side)       // H raw -> S[2..3] ([128][D] tile, over KQo): for dk^, dq^
+#pragma unroll
+                for (int ib = 0; ib < 4; ++ib) {
+                    if (ib < nb) {
+                        const int mt = side * 4 + ib, r0 = side * 64 + 16 * ib;
+#pragma unroll
+                        for (int nt = 0; nt < NTW; ++nt) {
+                            const int j = cw + 8 * nt + 2 * l4;
+                            *reinterpret_cast<uint32_t*>(sm + Lo.S[2] + tile_off(128, r0 + g, j)) = pack_bf16(accI[mt][nt][0], accI[mt][nt][1]);
+                            *reinterpret_cast<uint32_t*>(sm + Lo.S[2] + tile_off(128, r0 + g + 8, j)) = pack_bf16(accI[mt][nt][2], accI[mt][nt][3]);
+                        }
+                    }
+                }
+#pragma unroll
+            for (int jb = 0; jb < 4; ++jb) {           // H' raw -> S[4] ([64][D] tile, over DAP);  dlp -> S[0]
+                if (jb < nb) {
+#pragma unroll
+                    for (int nt = 0; nt < NTW; ++nt) {
+                        const int j = cw + 8 * nt + 2 * l4;
+                        *reinterpret_cast<uint32_t*>(sm + Lo.S[4] + tile_off(64, 16 * jb + g, j)) = pack_bf16(accII[jb][nt][0], accII[jb][nt][1]);
+                        *reinterpret_cast<uint32_t*>(sm + Lo.S[4] + tile_off(64, 16 * jb + g + 8, j)) = pack_bf16(accII[jb][nt][2], accII[jb][nt][3]);
+                        *reinterpret_cast<uint32_t*>(sm + Lo.S[0] + tile_off(64, 16 * jb + g, j)) = pack_bf16(dd[2 * jb][nt][0], dd[2 * jb][nt][1]);
+                        *reinterpret_cast<uint32_t*>(sm + Lo.S[0] + tile_off(64, 16 * jb + g + 8, j)) = pack_bf16(dd[2 * jb + 1][nt][0], dd[2 * jb + 1][nt][1]);
+                    }
+                }
+            }
+        }
+        // ---- L5: assemble dk^, dq^ (state part) and the state-read / state-write contributions to d log gamma
+        __syncthreads();
+        if (warp_active) {
+            if (krole) {
+                uint4 fq4[HK / 8], ic4[HK / 8];
+                const bool bstart = (t & 15) == 0;
+                if (live) {
+#pragma unroll
+                    for (int i = 0; i < HK / 8; ++i) {
+                        const int cc = half * (HK / 8) + i;
+                        fq4[i] = bstart ? make_uint4(0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u)
+                                        : ldg128(rc + Rc.FQ + tile_chunk_off(64, t - 1, cc));
+                        ic4[i] = ldg128(rc + Rc.IC + tile_chunk_off(64, t, cc));
+                    }
+                }
+                __nv_bfloat16* gdk = a.dk + ((tok0 + t) * a.H + h) * D;
+#pragma unroll
+                for (int s = 0; s < HK; s += 16) {
+                    uint32_t vs[16], vk[16];
+                    tmem_ld16(tmem + BM_A + lane_base + half * HK + s, vs);    // SP_K = (-dR) S
+                    tmem_ld16(tmem + BM_KT + lane_base + half * HK + s, vk);   // dKtil = U dS'
+                    tmem_wait_ld();
+                    if (live) {
+#pragma unroll
+                        for (int ch = 0; ch < 2; ++ch) {
+                            const int i = s / 8 + ch, cc = half * (HK / 8) + i, j0 = 8 * cc;
+                            float fp[8], ic[8], pk[8], pc[8], k0[8], c8[8], o[8], xa[8], zz[8];
+                            unpack8(fq4[i], fp); unpack8(ic4[i], ic);
+                            unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, t, cc)), pk);
+                            unpack8(lds128(sm + Lo.S[4] + tile_chunk_off(64, t, cc)), pc);
+                            unpack8(lds128(sm + Lo.S[5] + tile_chunk_off(64, t, cc)), k0);
+                            unpack8(lds128(sm + Lo.S[1] + tile_chunk_off(64, t, cc)), c8);
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) {
+                                const int j = j0 + e;
+                                float pre = 1.f, suf = 1.f;   // gamma_a(blk)/gamma_{-1} and gamma_L/gamma_a(blk)
+#pragma unroll
+                                for (int b2 = 0; b2 < 4; ++b2) {
+                                    const float etv = mi.etot[b2][j];
+                                    pre *= b2 < blk ? etv : 1.f;
+                                    suf *= b2 >= blk ? etv : 1.f;
+                                }
+                                const float sp = __uint_as_float(vs[8 * ch + e]), dkt = __uint_as_float(vk[8 * ch + e]);
+                                const float dkA = fp[e] * (pk[e] + pre * sp);
+                                const float dkC = ic[e] * (pc[e] + suf * dkt);
+                                o[e] = dkA + dkC;
+                                xa[e] = k0[e] * sp;                 // Kbar_t . dKbar_t (state read), to d log gamma_{t-1}
+                                zz[e] = (c8[e] * suf) * dkt;        // Ktil_t . dKtil_t (state write), to d log gamma_t' for t' > t
+                            }
+                            stg128(gdk + j0, pack8(o));
+                            sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8(xa));   // in place over H_t
+                            sts128(sm + Lo.S[4] + tile_chunk_off(64, t, cc), pack8(zz));    // in place over H'_t
+                        }
+                    }
+                }
+            } else {
+                uint4 fq4[HK / 8];
+                if (live) {
+#pragma unroll
+                    for (int i = 0; i < HK / 8; ++i) fq4[i] = ldg128(rc + Rc.FQ + tile_chunk_off(64, t, half * (HK / 8) + i));
+                }
+#pragma unroll
+                for (int s = 0; s < HK; s += 16) {
+                    uint32_t vs[16];
+                    tmem_ld16(tmem + BM_A + lane_base + half * HK + s, vs);    // SP_Q = dO S
+                    tmem_wait_ld();
+                    if (live) {
+#pragma unroll
+                        for (int ch = 0; ch < 2; ++ch) {
+                            const int i = s / 8 + ch, cc = half * (HK / 8) + i, j0 = 8 * cc;
+                            float fq[8], pq[8], q0[8], xq[8];
+                            unpack8(fq4[i], fq);
+                            unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc)), pq);
+                            unpack8(lds128(sm + Lo.S[6] + tile_chunk_off(64, t, cc)), q0);
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) {
+                                const int j = j0 + e;
+                                float pre = 1.f;
+#pragma unroll
+                                for (int b2 = 0; b2 < 4; ++b2) pre *= b2 < blk ? mi.etot[b2][j] : 1.f;
+                                const float sp = __uint_as_float(vs[8 * ch + e]);
+                                vs[8 * ch + e] = __float_as_uint(fq[e] * (pq[e] + pre * a.scale * sp));
+                                xq[e] = q0[e] * sp;                 // scale Qbar_t . (dO S)_t (state read)
+                            }
+                            sts128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc), pack8(xq));   // in place over H_t
+                        }
+                    }
+                    tmem_st16(tmem + BM_A + lane_base + half * HK + s, vs);   // dq^ state part, completed by the L8 MMA
+                }
+                tmem_wait_st();
+            }
+        }
+        // ---- L6: d log a_t = dlp_t + carry + sum_{t' > t} XA_t' + sum_{t' >= t} XQ_t' + sum_{t' < t} Z_t'  -> BM_KT rows 0..63
+        PHASE_SYNC();
+        if (tid == 0) {
+            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D, sb + Lo.TRI, 64, 0, 0, sb + Lo.S[2], 128, 0, 0, LCc, false);
+            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D, sb + Lo.TRI, 64, 0, 64, sb + Lo.S[2], 128, 0, 64, LCc, true);
+            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D, sb + Lo.TRI, 64, 0, 128, sb + Lo.S[4], 64, 0, 0, LCc, true);
+            umma_commit(&mi.bar_mma);
+            // K0, Q0 are dead: fetch G^T of the chunk and the raw q rows for L8
+            mbar_expect_tx(&mi.bar_g8, tile_bytes(D, 64));
+            bulk_g2s(sm + Lo.S[5], rc + Rc.GT, tile_bytes(D, 64), &mi.bar_g8);
+            mbar_expect_tx(&mi.bar_g5, (uint32_t)LCc * D * 2u);
+            for (int cb = 0; cb < D / 64; ++cb) tma_load_3d(sm + Lo.S[6] + cb * 8192, &mq, &mi.bar_g5, cb * 64, h, trow);
+        }
+        if (krole) {
+            uint4 b4[HK / 8];
+            if (live) {
+#pragma unroll
+                for (int i = 0; i < HK / 8; ++i) b4[i] = ldg128(rc + Rc.Bg + tile_chunk_off(64, t, half * (HK / 8) + i));
+            }
+            WAIT_MMA();
+            if (warp_active) {
+                __nv_bfloat16* gdf = a.df + ((tok0 + t) * a.H + h) * D;
+                __nv_bfloat16* gdbx = a.dbx + ((tok0 + t) * a.H + h) * D;
+#pragma unroll
+                for (int s = 0; s < HK; s += 32) {
+                    uint32_t v[32];
+                    tmem_ld32(tmem + BM_KT + lane_base + half * HK + s, v);
+                    tmem_wait_ld();
+                    if (live) {
+#pragma unroll
+                        for (int ch = 0; ch < 4; ++ch) {
+                            const int i = s / 8 + ch, cc = half * (HK / 8) + i;
+                            float bb[8], dp[8], dla[8], dbp[8];
+                            unpack8(b4[i], bb);
+                            unpack8(lds128(sm + Lo.S[0] + tile_chunk_off(64, t, cc)), dp);
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) {
+                                dla[e] = __uint_as_float(v[8 * ch + e]) + dp[e] + mi.extra[8 * cc + e];
+                                dbp[e] = -dla[e] * bb[e];
+                            }
+                            stg128(gdf + 8 * cc, pack8(dla));    // d log a; the epilogue kernel turns it into df
+                            const uint4 w = pack8(dbp);
+                            stg128(gdbx + 8 * cc, w);
+                            sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), w);   // GW rows 0..63 = db_pre
+                        }
+                    }
+                }
+            }
+        } else {
+            // Q side: dw_pre rows (this thread wrote them to dwx in L2) -> GW rows 64..127;  [tt_b|0 ; 0|tt_w] -> S[1]
+            uint4 d4[HK / 8], t4[4];
+            if (live) {
+                const __nv_bfloat16* gdwx = a.dwx + ((tok0 + t) * a.H + h) * D;
+#pragma unroll
+                for (int i = 0; i < HK / 8; ++i) d4[i] = *reinterpret_cast<const uint4*>(gdwx + 8 * (half * (HK / 8) + i));
+#pragma unroll
+                for (int i = 0; i < 4; ++i) t4[i] = ldg128(rc + Rc.tt + t * 64 + 16 * i);
+            }
+            WAIT_MMA();
+            if (live) {
+#pragma unroll
+                for (int i = 0; i < HK / 8; ++i) sts128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, half * (HK / 8) + i), d4[i]);
+                // TT2: row t = [tt_b | 0], row 64+t = [0 | tt_w] over 32 columns; half 0 writes the K-side row
+                const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
+                const int rc8 = r >> 3;  // 16-byte chunks per gate half
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const bool is_b = i < rc8, is_w = i >= rc8 && i < 2 * rc8;
+                    if (half == 0) sts128(sm + Lo.S[1] + tile_chunk_off(128, t, i), is_b ? t4[i] : z4);
+                    else sts128(sm + Lo.S[1] + tile_chunk_off(128, 64 + t, i), is_w ? t4[i] : z4);
+                }
+            }
+        }
+        // ---- L7: ZZ = [db_pre; dw_pre] [Vb | Vw] -> BM_DAP;  dVb | dVw += [db_pre; dw_pre]^T TT2 -> BM_WG
+        PHASE_SYNC();
+        if (tid == 0) {
+            mma_k<KMAJ, KMAJ>(tmem + BM_DAP, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.VcT, 32, 0, 0, D, false);
+            mma_k<MNMAJ, MNMAJ>(tmem + BM_WG, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[1], 128, 0, 0, LCc, !first);
+            mma_k<MNMAJ, MNMAJ>(tmem + BM_WG, 32, sb + Lo.S[2], 128, 0, 64, sb + Lo.S[1], 128, 0, 64, LCc, true);
+            umma_commit(&mi.bar_mma);
+        }
+        WAIT_MMA();
+        if (half == 0 && warp_active) {
+            // dz = ZZ (1 - tt^2): K side owns the erase half (cols 0..r), Q side the write half (cols r..2r)
+            const int c0 = krole ? 0 : r;
+            uint32_t v[16];
+            tmem_ld16(tmem + BM_DAP + lane_base + c0, v);
+            tmem_wait_ld();
+            if (live) {
+                const float rnq = a.l2norm ? mi.rn[64 + t] : 1.f;
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    if (i < (r >> 3)) {
+                        float tv[8], dz[8], dzq[8];
+                        unpack8(lds128(sm + Lo.S[1] + tile_chunk_off(128, krole ? t : 64 + t, c0 / 8 + i)), tv);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            dz[e] = __uint_as_float(v[8 * i + e]) * (1.f - tv[e] * tv[e]);
+                            dzq[e] = dz[e] * rnq;
+                        }
+                        sts128(sm + Lo.S[0] + tile_chunk_off(128, 64 + t, c0 / 8 + i), pack8(dz));    // DZ rows 64..127
+                        sts128(sm + Lo.S[4] + tile_chunk_off(64, t, c0 / 8 + i), pack8(dzq));          // DZQ = dz / |q|
+                    }
+                }
+                if (!krole) {  // zero the unused columns [2r, 32) of DZQ (the dG product has N = 32)
+                    const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
+                    for (int i = 2 * (r >> 3); i < 4; ++i) sts128(sm + Lo.S[4] + tile_chunk_off(64, t, i), z4);
+                }
+            }
+        }
+        // ---- L8: dq^ += dz G -> BM_A rows 64..127;  dG^T = q^T (dz/|q|) -> BM_DAP + 32
+        PHASE_SYNC();
+        if (tid == 0) {
+            mbar_wait(&mi.bar_g8, ph);
+            mbar_wait(&mi.bar_g5, ph);
+            tc_fence_after();
+            mma_k<KMAJ, KMAJ>(tmem + BM_A, D, sb + Lo.S[0], 128, 0, 0, sb + Lo.S[5], D, 0, 0, R2, true);
+            mma_k<MNMAJ, MNMAJ>(tmem + BM_DAP + 32, 32, sb + Lo.S[6], 64, 0, 0, sb + Lo.S[4], 64, 0, 0, LCc, false);
+            umma_commit(&mi.bar_mma);
+        }
+        WAIT_MMA();
+        if (!krole && warp_active) {
+            __nv_bfloat16* gdq = a.dq + ((tok0 + t) * a.H + h) * D;
+#pragma unroll
+            for (int s = 0; s < HK; s += 32) {
+                uint32_t v[32];
+                tmem_ld32(tmem + BM_A + lane_base + half * HK + s, v);
+                tmem_wait_ld();
+                if (live) {
+#pragma unroll
+                    for (int ch = 0; ch < 4; ++ch) {
+                        float f8[8];
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) f8[e] = __uint_as_float(v[8 * ch + e]);
+                        stg128(gdq + half * HK + s + 8 * ch, pack8(f8));
+                    }
+                }
+            }
+        }
+        if (half == 1 && srow) {   // dG^T rows j -> bf16 tile DGT (S[1], over TT2)
+            uint32_t v[32];
+            tmem_ld32(tmem + BM_DAP + 32 + lane_base, v);
+            tmem_wait_ld();
+#pragma unroll
+            for (int ch = 0; ch < 4; ++ch) {
+                float f8[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) f8[e] = __uint_as_float(v[8 * ch + e]);
+                sts128(sm + Lo.S[1] + tile_chunk_off(D, row, ch), pack8(f8));
+            }
+        }
+        // ---- L9: fold glue: dS += [Ub;Uw]^T dG;  d[Ub;Uw]^T += S dG^T -> BM_WU
+        PHASE_SYNC();
+        if (tid == 0) {
+            mma_k<MNMAJ, KMAJ>(tmem + BM_DS, D, sb + Lo.Ucat, 32, 0, 0, sb + Lo.S[1], D, 0, 0, R2, true);
+            mma_k<KMAJ, MNMAJ>(tmem + BM_WU, 32, sb + Lo.SBq, D, 0, 0, sb + Lo.S[1], D, 0, 0, D, !first);
+            umma_commit(&mi.bar_mma);
+        }
+        WAIT_MMA();
+        if (tid == 0 && c > 0) {   // SBq is free: the state entering the next chunk to be processed
+            mbar_expect_tx(&mi.bar_sb, SBb);
+            bulk_g2s(sm + Lo.SBq, rc - Rc.total + Rc.SB, SBb, &mi.bar_sb);
+        }
+        // ---- L10: the adjoint of the state entering the chunk
+        finalize(true, c == 0);
+        first = false;
+    }
+
+    // ---- per-chain partial weight gradients: [dUb|dUw][dVb][dVw] (dA, dtau come from the epilogue kernel)
+    if (half == 0 && srow) {
+        float* part = a.part + (size_t)chain * a.part_stride;
+        float* partVb = part + 2 * r * D;
+        float* partVw = partVb + D * r;
+        uint32_t wg[32], wu[32];
+        tmem_ld32(tmem + BM_WG + lane_base, wg);
+        tmem_ld32(tmem + BM_WU + lane_base, wu);
+        tmem_wait_ld();
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+            if (i < r) partVb[row * r + i] = __uint_as_float(wg[i]);
+            else if (i < R2) partVw[row * r + (i - r)] = __uint_as_float(wg[i]);
+            if (i < R2) part[i * D + row] = __uint_as_float(wu[i]);
+        }
+    }
+    PHASE_SYNC();
+    if (warp == 0) tmem_dealloc(tmem, TM_COLS);
+}
+
+// ---- chunk-local tail, fully parallel over (chain, chunk) -----------------------------------------
+// dq, dk hold the gradients w.r.t. the normalised q^, k^ and df holds d log a; in place:
+//   dq = (dq^ - q^ <q^, dq^>) / sqrt(|q|^2 + eps)   (L2-norm backward, Alg. 5 step 14 l.857-860), same for k
+//   df = dla . (-exp A) sigmoid(f + tau)            (Eq. 9 l.151), and the per-chunk partial sums of
+//   dtau = sum df,  dA = sum dla . g  with g = -exp(A) softplus(f + tau).
+template <int D>
+__global__ void __launch_bounds__(256)
+carve_bwd_tc_epilogue_kernel(const __nv_bfloat16* __restrict__ gq, const __nv_bfloat16* __restrict__ gk,
+                             const __nv_bfloat16* __restrict__ gf, const float* __restrict__ A,
+                             const float* __restrict__ tau, __nv_bfloat16* dq, __nv_bfloat16* dk, __nv_bfloat16* df,
+                             float* __restrict__ partAT, int T, int H, int LCc, int l2norm, float eps)
+{
+    constexpr int V = D / 32;   // channels per lane
+    __shared__ float red[8][2][D];
+    const int nchunks = T / LCc;
+    const int chain = blockIdx.x / nchunks, c = blockIdx.x % nchunks, b = chain / H, h = chain % H;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float eA[V], ta[V], accA[V], accT[V];
+#pragma unroll
+    for (int e = 0; e < V; ++e) {
+        const int j = lane * V + e;
+        eA[e] = A ? __expf(__ldg(A + h * D + j)) : 1.f;
+        ta[e] = tau ? __ldg(tau + h * D + j) : 0.f;
+        accA[e] = accT[e] = 0.f;
+    }
+    auto load = [&](const __nv_bfloat16* p, float (&o)[V]) {
+        if constexpr (V == 4) {
+            const uint2 w = *reinterpret_cast<const uint2*>(p);
+            o[0] = bf16_lo(w.x); o[1] = bf16_hi(w.x); o[2] = bf16_lo(w.y); o[3] = bf16_hi(w.y);
+        } else {
+            const uint32_t w = *reinterpret_cast<const uint32_t*>(p);
+            o[0] = bf16_lo(w); o[1] = bf16_hi(w);
+        }
+    };
+    auto store = [&](__nv_bfloat16* p, const float (&o)[V]) {
+        if constexpr (V == 4) *reinterpret_cast<uint2*>(p) = make_uint2(pack_bf16(o[0], o[1]), pack_bf16(o[2], o[3]));
+        else *reinterpret_cast<uint32_t*>(p) = pack_bf16(o[0], o[1]);
+    };
+    auto wsum = [](float x) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xFFFFFFFFu, x, o);
+        return x;
+    };
+    for (int tt_ = warp; tt_ < LCc; tt_ += 8) {
+        const size_t ro = (((size_t)b * T + (size_t)c * LCc + tt_) * H + h) * D + lane * V;
+        if (l2norm) {
+            float x[V], dx[V];
+#pragma unroll
+            for (int which = 0; which < 2; ++which) {
+                const __nv_bfloat16* src = which ? gk : gq;
+                __nv_bfloat16* dst = which ? dk : dq;
+                load(src + ro, x);
+                load(dst + ro, dx);
+                float ss = 0.f;
+#pragma unroll
+                for (int e = 0; e < V; ++e) ss += x[e] * x[e];
+                const float rn = rsqrtf(wsum(ss) + eps);
+                float dot = 0.f;
+#pragma unroll
+                for (int e = 0; e < V; ++e) { x[e] *= rn; dot += x[e] * dx[e]; }
+                dot = wsum(dot);
+#pragma unroll
+                for (int e = 0; e < V; ++e) dx[e] = (dx[e] - x[e] * dot) * rn;
+                store(dst + ro, dx);
+            }
+        }
+        float fv[V], dla[V];
+        load(gf + ro, fv);
+        load(df + ro, dla);
+#pragma unroll
+        for (int e = 0; e < V; ++e) {
+            const float z = fv[e] + ta[e];
+            const float sg = sigmoid_fast(z), sp = softplus_fast(z);
+            const float d = dla[e] * (-eA[e]) * sg;
+            accT[e] += d;
+            accA[e] += dla[e] * (-eA[e] * sp);
+            dla[e] = d;
+        }
+        store(df + ro, dla);
+    }
+#pragma unroll
+    for (int e = 0; e < V; ++e) { red[warp][0][lane * V + e] = accA[e]; red[warp][1][lane * V + e] = accT[e]; }
+    __syncthreads();
+    for (int i = threadIdx.x; i < 2 * D; i += 256) {
+        float s = 0.f;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) s += red[w][i / D][i % D];
+        partAT[(size_t)blockIdx.x * 2 * D + i] = s;
+    }
+}
+
+// part[chain][nW + which*dk + j] = sum over the chain's chunks of partAT (fixed order: deterministic).
+__global__ void carve_reduce_at_kernel(const float* __restrict__ partAT, float* part, int nchunks, int stride, int nW, int D)
+{
+    const int chain = blockIdx.x, i = threadIdx.x;
+    if (i >= 2 * D) return;
+    float s = 0.f;
+    for (int c = 0; c < nchunks; ++c) s += partAT[((size_t)chain * nchunks + c) * 2 * D + i];
+    part[(size_t)chain * stride + nW + i] = s;
+}
+
+template <int D>
+cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float* dA, float* dtau, float* dUb, float* dUw,
+                          float* dVb, float* dVw, cudaStream_t st)
+{
+    const int LCc = a.L < tcp::LC ? a.L : tcp::LC;
+    CUtensorMap mdO, mk, mq;
+    if (!tc_make_token_map(&mdO, a.dO, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mk, a.k, a.B, a.T, a.H, D, LCc) ||
+        !tc_make_token_map(&mq, a.q, a.B, a.T, a.H, D, LCc))
+        return cudaErrorInvalidValue;
+    BwdArgs t{};
+    t.B = a.B; t.H = a.H; t.T = a.T; t.L = a.L; t.r = a.r; t.l2norm = a.l2norm; t.scale = a.scale; t.eps = a.eps;
+    t.rec = ws + w.rec; t.sfin = ws + w.sfin; t.dS_final = a.dS_final;
+    t.Ub = a.Ub; t.Uw = a.Uw; t.Vb = a.Vb; t.Vw = a.Vw;
+    t.dq = static_cast<__nv_bfloat16*>(a.dq); t.dk = static_cast<__nv_bfloat16*>(a.dk_);
+    t.dv = static_cast<__nv_bfloat16*>(a.dv_); t.df = static_cast<__nv_bfloat16*>(a.df);
+    t.dbx = static_cast<__nv_bfloat16*>(a.dbx); t.dwx = static_cast<__nv_bfloat16*>(a.dwx);
+    t.dbeta = static_cast<__nv_bfloat16*>(a.dbeta); t.dS0 = a.dS0;
+    t.part = reinterpret_cast<float*>(ws + w.part); t.part_stride = w.part_stride;
+    const size_t smem = BLayout(D).total;
+    auto kern = carve_bwd_tc_kernel<D>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int chains = a.B * a.H, nchunks = a.T / LCc;
+    kern<<<chains, tcp::NT, smem, st>>>(t, mdO, mk, mq);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    float* partAT = reinterpret_cast<float*>(ws + w.partAT);
+    carve_bwd_tc_epilogue_kernel<D><<<chains * nchunks, 256, 0, st>>>(
+        static_cast<const __nv_bfloat16*>(a.q), static_cast<const __nv_bfloat16*>(a.k),
+        static_cast<const __nv_bfloat16*>(a.f), a.A, a.tau, t.dq, t.dk, t.df, partAT, a.T, a.H, LCc, a.l2norm, a.eps);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    const int nW = 2 * a.r * D + 2 * D * a.r;
+    carve_reduce_at_kernel<<<chains, 2 * D, 0, st>>>(partAT, t.part, nchunks, w.part_stride, nW, D);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    return reduce_weights_launch(t.part, chains, w.part_stride, a.H, D, D, a.r, dUb, dUw, dVb, dVw, dA, dtau, st);
+}
+
+}  // namespace
+
+bool tc_bwd_supported(const carve_params_t& p) { return tc_fwd_supported(p) && p.L <= 64; }
+
+cudaError_t tc_bwd_launch(const Args& a, uint8_t* ws, const TcWsLayout& w, float* dA, float* dtau, float* dUb, float* dUw,
+                          float* dVb, float* dVw, cudaStream_t st)
+{
+    if (a.dk == 128) return launch_tc_bwd<128>(a, ws, w, dA, dtau, dUb, dUw, dVb, dVw, st);
+    if (a.dk == 64) return launch_tc_bwd<64>(a, ws, w, dA, dtau, dUb, dUw, dVb, dVw, st);
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace carve

@@ -36,7 +36,8 @@ struct TcArgs {
     const float *A, *tau, *Ub, *Uw, *Vb, *Vw, *S0;
     __nv_bfloat16* O;
     float* S_final;
-    uint8_t* ws_S;  // bf16 row tiles of the state entering every solve chunk, or nullptr
+    uint8_t* rec;   // [chains][T/LC] chunk records (carve_tc.cuh Rec) for the reverse kernel, or nullptr
+    uint8_t* sfin;  // [chains] bf16 row tile of the final state (the reverse kernel's first "next state")
 };
 
 // Runtime-shaped product from two row tiles (see tc_common.cuh umma_tiles); M fixed at compile time.
@@ -228,7 +229,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     PHASE_SYNC();
     const uint32_t tmem = mi.tmem_base;
     const size_t state_tile = tile_bytes(DV, DK);
-    uint8_t* ws_chain = a.ws_S ? a.ws_S + (size_t)chain * nchunks * state_tile : nullptr;
+    const Rec Rc(DK, DV);
+    uint8_t* rec_chain = a.rec ? a.rec + (size_t)chain * nchunks * Rc.total : nullptr;
+    uint8_t* ws_chain = rec_chain ? rec_chain + Rc.SB : nullptr;  // state tile of chunk 0
 
     // initial state: fp32 -> TMEM, bf16 -> Sb (and the workspace slot of chunk 0)
     if (row < DV) {
@@ -288,6 +291,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     for (int c = 0; c < nchunks; ++c) {
         const bool fold_now = (c % gate_every) == 0;
         const size_t tok0 = (size_t)b * a.T + (size_t)c * LCc;  // first token of the chunk
+        uint8_t* rc = rec_chain ? rec_chain + (size_t)c * Rc.total : nullptr;  // this chunk's record
         // ---- P0: fold G^T = S^T Ucat^T -> TM_X2[0, R2)
         PHASE_SYNC();
         if (fold_now && tid == 0) {
@@ -306,7 +310,12 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 for (int e = 0; e < 8; ++e) ss += f8[e] * f8[e];
             }
             mi.nrm[row][half] = ss;
-            if (krole && half == 0) sBeta[t] = __bfloat162float(a.beta[(tok0 + t) * a.H + h]);
+            if (krole && half == 0) {
+                // clamped away from 0 so that e_t = u_t / beta_t exists (u_t changes by < 1e-30 |e_t|)
+                const float bt = fmaxf(__bfloat162float(a.beta[(tok0 + t) * a.H + h]), 1e-30f);
+                sBeta[t] = bt;
+                if (rc) reinterpret_cast<float*>(rc + Rc.beta)[t] = bt;
+            }
         }
         if (fold_now) {
             WAIT_MMA();
@@ -321,6 +330,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     for (int e = 0; e < 16; ++e) f[e] = __uint_as_float(v[e]);
                     sts128(sm + Lo.Vcat + tile_chunk_off(DM, row, (32 + c0) / 8), pack8(f));
                     sts128(sm + Lo.Vcat + tile_chunk_off(DM, row, (32 + c0) / 8 + 1), pack8(f + 8));
+                    if (rc) {
+                        *reinterpret_cast<uint4*>(rc + Rc.GT + tile_chunk_off(DK, row, c0 / 8)) = pack8(f);
+                        *reinterpret_cast<uint4*>(rc + Rc.GT + tile_chunk_off(DK, row, c0 / 8 + 1)) = pack8(f + 8);
+                    }
                 }
             }
         }
@@ -343,6 +356,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     float f[16];
 #pragma unroll
                     for (int e = 0; e < 16; ++e) f[e] = tanh_fast(__uint_as_float(v[e]) * rnq);
+                    if (rc) {
+                        *reinterpret_cast<uint4*>(rc + Rc.tt + t * 64 + c0 * 2) = pack8(f);
+                        *reinterpret_cast<uint4*>(rc + Rc.tt + t * 64 + c0 * 2 + 16) = pack8(f + 8);
+                    }
 #pragma unroll
                     for (int k8 = 0; k8 < 2; ++k8) {
                         const int col = c0 + 8 * k8;       // tt columns [col, col+8)
@@ -387,7 +404,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     tmem_ld8(tmem + TM_X1 + lane_base + 8 * cc, pr);
                     tmem_wait_ld();
                     if (live) {
-                        float fb[8], ff[8], hi[8], lo[8];
+                        float fb[8], ff[8], hi[8], lo[8], bg[8];
                         const uint32_t off = tile_chunk_off(64, t, cc);
                         unpack8(lds128(sm + Lo.BX + off), fb);
                         unpack8(lds128(sm + Lo.F + off), ff);
@@ -395,6 +412,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         for (int e = 0; e < 8; ++e) {
                             const int j = 8 * cc + e;
                             const float pre = fb[e] + __uint_as_float(pr[e]);
+                            bg[e] = sigmoid_fast(pre);
                             const float g = -mi.eA[j] * softplus_fast(ff[e] + mi.tau[j]);
                             const float la = g - softplus_fast(pre);
                             const float h16 = __bfloat162float(__float2bfloat16_rn(la));
@@ -403,6 +421,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         }
                         sts128(sm + Lo.Y0 + off, pack8(hi));
                         sts128(sm + Lo.Y1 + off, pack8(lo));
+                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.Bg + off) = pack8(bg);
                     }
                 }
             } else {
@@ -417,8 +436,17 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         unpack8(lds128(sm + Lo.WX + off), fw);
                         unpack8(lds128(sm + Lo.V + off), fv);
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) fv[e] *= sigmoid_fast(fw[e] + __uint_as_float(pr[e]));
+                        for (int e = 0; e < 8; ++e) {
+                            fw[e] = sigmoid_fast(fw[e] + __uint_as_float(pr[e]));
+                            fv[e] *= fw[e];
+                        }
                         sts128(sm + Lo.V + off, pack8(fv));
+                        if (rc) {
+                            *reinterpret_cast<uint4*>(rc + Rc.W + off) = pack8(fw);
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) fv[e] *= 1.f - fw[e];
+                            *reinterpret_cast<uint4*>(rc + Rc.VWX + off) = pack8(fv);
+                        }
                     }
                 }
             }
@@ -456,6 +484,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 if (b2 < nb) p *= mi.etot[b2][tid];
             }
             mi.gamL[tid] = p;
+            if (rc) {
+#pragma unroll
+                for (int b2 = 0; b2 < 4; ++b2) reinterpret_cast<float*>(rc + Rc.etot)[b2 * DK + tid] = b2 < nb ? mi.etot[b2][tid] : 1.f;
+            }
         }
         __syncthreads();
         // ---- P7b: decayed operands.  Row operands exist in up to four anchorings: version 0 relative to the chunk
@@ -478,6 +510,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 const bool has_next = tn < LCc;
                 const int bn = tn >> 4, krow = has_next ? tn : 0;
                 const float rnk = a.l2norm ? rsqrtf(mi.nrm[krow][0] + mi.nrm[krow][1] + a.eps) : 1.f;
+                if (rc && live && half == 0) reinterpret_cast<float*>(rc + Rc.rn)[64 + t] = rnq;
 #pragma unroll 1
                 for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
                     uint32_t v[8];
@@ -491,17 +524,32 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, krow, cc)), kv);
 #pragma unroll
                         for (int e = 0; e < 8; ++e) { qv[e] *= rnq; kv[e] *= rnk; }
-                        if (has_next && bn > blk) sts128(ver_row(bn, false, tn, cc), pack8(kv));  // first row of its block
+                        if (has_next && bn > blk) {  // first row of its block
+                            sts128(ver_row(bn, false, tn, cc), pack8(kv));
+                            if (rc) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = pack8(kv);
+                        }
+                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.FQ + tile_chunk_off(64, t, cc)) = pack8(Fp);
 #pragma unroll
                         for (int jb = 3; jb >= 0; --jb) {
                             if (jb <= blk) {
 #pragma unroll
                                 for (int e = 0; e < 8; ++e) o[e] = qv[e] * Fp[e];
-                                sts128(ver_row(jb, true, t, cc), pack8(o));
+                                const uint4 wq = pack8(o);
+                                sts128(ver_row(jb, true, t, cc), wq);
+                                if (rc && jb == blk) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, 64 + t, cc)) = wq;
+                                if (rc && jb == 0) {
+#pragma unroll
+                                    for (int e = 0; e < 8; ++e) o[e] *= a.scale;
+                                    *reinterpret_cast<uint4*>(rc + Rc.Q0 + tile_chunk_off(64, t, cc)) = pack8(o);
+                                }
                                 if (has_next) {
 #pragma unroll
                                     for (int e = 0; e < 8; ++e) o[e] = kv[e] * Fp[e];
-                                    sts128(ver_row(jb, false, tn, cc), pack8(o));
+                                    const uint4 wk = pack8(o);
+                                    sts128(ver_row(jb, false, tn, cc), wk);
+                                    if (rc && jb == blk && bn == blk)
+                                        *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = wk;
+                                    if (rc && jb == 0) *reinterpret_cast<uint4*>(rc + Rc.K0 + tile_chunk_off(64, tn, cc)) = wk;
                                 }
                                 if (jb > 0) {
                                     const float4 e0 = *reinterpret_cast<const float4*>(&mi.etot[jb - 1][8 * cc]);
@@ -511,18 +559,25 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                                 }
                             }
                         }
-                        if (!has_next) sts128(sm + Lo.KQbar + tile_chunk_off(128, 0, cc), pack8(kv));  // Kbar_0 = k^_0
+                        if (!has_next) {  // Kbar_0 = k^_0
+                            sts128(sm + Lo.KQbar + tile_chunk_off(128, 0, cc), pack8(kv));
+                            if (rc) {
+                                *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, 0, cc)) = pack8(kv);
+                                *reinterpret_cast<uint4*>(rc + Rc.K0 + tile_chunk_off(64, 0, cc)) = pack8(kv);
+                            }
+                        }
                     }
                 }
             } else {
                 const float rnk = a.l2norm ? rsqrtf(mi.nrm[row][0] + mi.nrm[row][1] + a.eps) : 1.f;
+                if (rc && live && half == 0) reinterpret_cast<float*>(rc + Rc.rn)[t] = rnk;
 #pragma unroll 1
                 for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
                     uint32_t v[8];
                     tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, v);
                     tmem_wait_ld();
                     if (live) {
-                        float kv[8], o1[8], o2[8], et[8], sf[8];
+                        float kv[8], o1[8], o2[8], ic[8], et[8], sf[8];
                         unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, t, cc)), kv);
                         *reinterpret_cast<float4*>(et) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc]);
                         *reinterpret_cast<float4*>(et + 4) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc + 4]);
@@ -532,11 +587,18 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         for (int e = 0; e < 8; ++e) {
                             const float cx = __expf(__uint_as_float(v[e]));   // gamma_{a_blk} / gamma_t >= 1
                             const float kh = kv[e] * rnk;
+                            ic[e] = cx;
                             o1[e] = kh * cx;
                             o2[e] = kh * ((cx * et[e]) * sf[e]);              // k^ gamma_L / gamma_t, every factor <= 1
                         }
-                        sts128(sm + Lo.Y1 + tile_chunk_off(64, t, cc), pack8(o1));      // C_t
-                        sts128(sm + Lo.Ktil + tile_chunk_off(64, t, cc), pack8(o2));    // Ktil_t
+                        const uint32_t off = tile_chunk_off(64, t, cc);
+                        sts128(sm + Lo.Y1 + off, pack8(o1));      // C_t
+                        sts128(sm + Lo.Ktil + off, pack8(o2));    // Ktil_t
+                        if (rc) {
+                            *reinterpret_cast<uint4*>(rc + Rc.CC + off) = pack8(o1);
+                            *reinterpret_cast<uint4*>(rc + Rc.KT + off) = pack8(o2);
+                            *reinterpret_cast<uint4*>(rc + Rc.IC + off) = pack8(ic);
+                        }
                     }
                 }
             }
@@ -567,6 +629,12 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     for (int e = 0; e < 16; ++e) f[e] = (16 * jb + e <= tok) ? __uint_as_float(v[e]) : 0.f;
                     sts128(sm + Lo.TP + tile_chunk_off(128, 64 + tok, 2 * jb), pack8(f));
                     sts128(sm + Lo.TP + tile_chunk_off(128, 64 + tok, 2 * jb + 1), pack8(f + 8));
+                    if (rc) {  // the record keeps scale.P in rows 0..63
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) f[e] *= a.scale;
+                        *reinterpret_cast<uint4*>(rc + Rc.PT + tile_chunk_off(128, tok, 2 * jb)) = pack8(f);
+                        *reinterpret_cast<uint4*>(rc + Rc.PT + tile_chunk_off(128, tok, 2 * jb + 1)) = pack8(f + 8);
+                    }
                 }
             };
             const int nb = LCc >> 4;
@@ -582,6 +650,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         for (int jb = (t >> 4) + 1; jb < 4; ++jb) {
                             sts128(sm + Lo.TP + tile_chunk_off(128, 64 + t, 2 * jb), z4);
                             sts128(sm + Lo.TP + tile_chunk_off(128, 64 + t, 2 * jb + 1), z4);
+                            if (rc) {
+                                *reinterpret_cast<uint4*>(rc + Rc.PT + tile_chunk_off(128, t, 2 * jb)) = z4;
+                                *reinterpret_cast<uint4*>(rc + Rc.PT + tile_chunk_off(128, t, 2 * jb + 1)) = z4;
+                            }
                         }
                     }
                 }
@@ -646,6 +718,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         f[e] = s <= tr_ ? Tm[mm_idx(tr_, s)] : 0.f;
                     }
                     sts128(sm + Lo.TP + tile_chunk_off(128, tr_, 2 * qq + k8), pack8(f));
+                    if (rc) *reinterpret_cast<uint4*>(rc + Rc.PT + tile_chunk_off(128, 64 + tr_, 2 * qq + k8)) = pack8(f);
                 }
             }
         }
@@ -659,6 +732,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         WAIT_MMA();
         // ---- P11: U -> bf16 rows (over V')
         if (krole && warp_active) {
+            const float rbt = live ? __fdividef(1.f, sBeta[t]) : 0.f;
 #pragma unroll 1
             for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
                 uint32_t v[8];
@@ -668,7 +742,14 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     float f[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[e]);
-                    sts128(sm + Lo.Us + tile_chunk_off(64, t, cc), pack8(f));
+                    const uint32_t off = tile_chunk_off(64, t, cc);
+                    sts128(sm + Lo.Us + off, pack8(f));
+                    if (rc) {
+                        *reinterpret_cast<uint4*>(rc + Rc.U + off) = pack8(f);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) f[e] *= rbt;  // e_t = u_t / beta_t (Alg. 2 step 7)
+                        *reinterpret_cast<uint4*>(rc + Rc.E + off) = pack8(f);
+                    }
                 }
             }
         }
@@ -699,7 +780,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         if (q * 32 < DV) {
             const bool last_chunk = c + 1 == nchunks;
-            uint8_t* ws_next = (ws_chain && !last_chunk) ? ws_chain + (size_t)(c + 1) * state_tile : nullptr;
+            uint8_t* ws_next = !ws_chain ? nullptr
+                               : last_chunk ? a.sfin + (size_t)chain * state_tile : ws_chain + (size_t)(c + 1) * Rc.total;
 #pragma unroll 1
             for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
                 uint32_t sv[8], wv[8];
@@ -772,9 +854,10 @@ bool tc_fwd_supported(const carve_params_t& p)
 }
 
 size_t tc_state_tile_bytes(const carve_params_t& p) { return tc::tile_bytes(p.dv, p.dk); }
+size_t tc_record_bytes(const carve_params_t& p) { return tcp::Rec(p.dk, p.dv).total; }
 
 template <int D>
-static cudaError_t launch_tc_fwd(const Args& a, uint8_t* ws_S, cudaStream_t st)
+static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, uint8_t* sfin, cudaStream_t st)
 {
     const int LCc = a.L < tcp::LC ? a.L : tcp::LC;
     CUtensorMap mq, mk, mv, mf, mbx, mwx;
@@ -786,7 +869,7 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* ws_S, cudaStream_t st)
     t.B = a.B; t.H = a.H; t.T = a.T; t.L = a.L; t.r = a.r; t.l2norm = a.l2norm; t.scale = a.scale; t.eps = a.eps;
     t.beta = static_cast<const __nv_bfloat16*>(a.beta);
     t.A = a.A; t.tau = a.tau; t.Ub = a.Ub; t.Uw = a.Uw; t.Vb = a.Vb; t.Vw = a.Vw; t.S0 = a.S0;
-    t.O = static_cast<__nv_bfloat16*>(a.O); t.S_final = a.S_final; t.ws_S = ws_S;
+    t.O = static_cast<__nv_bfloat16*>(a.O); t.S_final = a.S_final; t.rec = rec; t.sfin = sfin;
     const size_t smem = tcp::Layout(D, D, 2 * a.r).total;
     auto kern = carve_fwd_tc_kernel<D, D>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -795,10 +878,10 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* ws_S, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t tc_fwd_launch(const Args& a, uint8_t* ws_S, cudaStream_t st)
+cudaError_t tc_fwd_launch(const Args& a, uint8_t* rec, uint8_t* sfin, cudaStream_t st)
 {
-    if (a.dk == 128) return launch_tc_fwd<128>(a, ws_S, st);
-    if (a.dk == 64) return launch_tc_fwd<64>(a, ws_S, st);
+    if (a.dk == 128) return launch_tc_fwd<128>(a, rec, sfin, st);
+    if (a.dk == 64) return launch_tc_fwd<64>(a, rec, sfin, st);
     return cudaErrorInvalidValue;
 }
 
