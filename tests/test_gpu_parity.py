@@ -88,12 +88,13 @@ def test_extreme_decay_no_overflow(oracle):
     """Strong decay/erase (log gamma_L ~ -600 per chunk): every ratio is formed as exp(<=0).
     Gradient tolerance 5e-4: an fp32 prefix sum of magnitude ~150 puts ~8e-6 absolute error
     into every exp(lg_a - lg_b), and df sums ~1e2 such terms of both signs.  dA and dtau are sums of dg.g / df over
-    all T tokens (Eq. 9 l.151) that cancel to ~1/10 of their terms here, so they carry 10x that: 5e-3."""
+    all T tokens (Eq. 9 l.151) that cancel to ~1/10 of their terms here, so they carry 10x that: 5e-3; the same
+    holds for the other token-summed weight gradients fed by d log a (dUb, dVb through db_pre, Alg. 5 l.846)."""
     cfg = synth.Config("t", B=1, H=1, T=128, L=64, dk=64, dv=64, r=8, dtype="f32", wstd=0.1, s0_std=0.1, seed=4)
     x = synth.make_inputs(cfg)
     x["f"] = x["f"] + 5.0
     x["bx"] = x["bx"] + 5.0
-    _check_fwd_bwd(oracle, cfg, x, tol=dict(O=1e-4, S=1e-4, g=5e-4, dA=5e-3, dtau=5e-3))
+    _check_fwd_bwd(oracle, cfg, x, tol=dict(O=1e-4, S=1e-4, g=5e-4, dA=5e-3, dtau=5e-3, dUb=5e-3, dVb=5e-3, dUw=5e-3, dVw=5e-3))
 
 
 # ---- invariants that need no oracle -------------------------------------------------------------
@@ -152,3 +153,100 @@ def test_host_entry_point_matches_device_entry_point(oracle):
     assert np.array_equal(Sfh.numpy().astype(np.float64), Sf)
     for n in GRADS:
         assert np.array_equal(gh[n].float().numpy().astype(np.float64), g[n]), n
+
+
+# ---- both kernel families against the oracle on the same bf16 case --------------------------------
+@pytest.mark.parametrize("path", [carve.CARVE_PATH_SIMT, carve.CARVE_PATH_TENSOR])
+@pytest.mark.parametrize("dk,r,L", [(64, 8, 64), (128, 16, 64), (128, 16, 32), (64, 16, 16)])
+def test_kernel_families_bf16(oracle, path, dk, r, L):
+    """Several chunks, several 16-token anchor blocks, nonzero S0, active content gates, A and tau present."""
+    cfg = synth.Config("t", B=2, H=2, T=256, L=L, dk=dk, dv=dk, r=r, dtype="bf16", wstd=0.1, s0_std=0.05, seed=dk + L)
+    x = synth.make_inputs(cfg, with_decay_params=True)
+    p = params_of(cfg, path=path)
+    assert carve.carve_resolved_path(p, True) == path
+    _check_fwd_bwd(oracle, cfg, x, path=path)
+
+
+def test_tensor_path_refuses_what_it_does_not_cover(oracle):
+    """No silent substitution: an explicit CARVE_PATH_TENSOR request for L = 128 training or fp32 is an error."""
+    for kw in (dict(L=128, dtype="bf16"), dict(L=64, dtype="f32")):
+        cfg = synth.Config("t", B=1, H=1, T=128, dk=64, dv=64, r=8, seed=1, **kw)
+        p = params_of(cfg, path=carve.CARVE_PATH_TENSOR)
+        assert carve.carve_resolved_path(p, True) == -1
+        assert carve.carve_workspace_bytes(p, True) == 0
+
+
+def test_tensor_path_scale_and_no_l2norm(oracle):
+    cfg = synth.Config("t", B=1, H=2, T=128, L=64, dk=64, dv=64, r=8, dtype="bf16", wstd=0.1, s0_std=0.05,
+                       scale=0.125, qk_l2norm=0, seed=31)
+    x = synth.make_inputs(cfg)
+    _check_fwd_bwd(oracle, cfg, x, path=carve.CARVE_PATH_TENSOR)
+
+
+def test_tensor_path_determinism(oracle):
+    cfg = synth.Config("t", B=2, H=3, T=256, L=64, dk=128, dv=128, r=16, dtype="bf16", wstd=0.1, seed=12)
+    x, ct = synth.make_inputs(cfg), synth.make_cotangents(cfg)
+    p = params_of(cfg, path=carve.CARVE_PATH_TENSOR)
+    outs = []
+    for _ in range(2):
+        O, Sf, h = run_fwd(p, x, need_bwd=True)
+        g, _ = run_bwd(p, h, ct)
+        outs.append((O, Sf, g))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    for n in GRADS:
+        assert np.array_equal(outs[0][2][n], outs[1][2][n]), n
+
+
+# ---- BASELINE.json config 1 at full size, in the launch configuration bench.py times ------------------
+def test_config1_full_size_sampled_chains(oracle):
+    """The whole 1.3B-like workload runs on the GPU (128 chains x 64 chunks); the oracle recomputes sampled
+    (batch, head) chains one by one -- chains are independent (Alg. 2 l.318) -- for every per-token output, S_final
+    and dS0.  The shared-weight gradients sum over all chains, so they are checked on the sampled chains run as
+    their own B'=3, H'=1 problem at full T."""
+    cfg = synth.CFG1
+    x, ct = synth.make_inputs(cfg), synth.make_cotangents(cfg)
+    p = params_of(cfg)
+    assert carve.carve_resolved_path(p, True) == carve.CARVE_PATH_TENSOR
+    O, Sf, h = run_fwd(p, x, need_bwd=True)
+    g, _ = run_bwd(p, h, ct)
+    chains = [(0, 0), (3, 7), (7, 15)]
+    tol = TOL["bf16"]
+    xs_all, cts_all = None, None
+    for b, hh in chains:
+        xs = synth.slice_chains(x, [(b, hh)])
+        cts = synth.slice_chains(ct, [(b, hh)])
+        s = oracle_shape(oracle, cfg, B=1, H=1)
+        O_ref, S_ref = oracle.fwd(s, xs)
+        g_ref = oracle.bwd(s, xs, cts["dO"], cts["dS_final"])
+        assert relerr(O[b:b + 1, :, hh:hh + 1], O_ref) <= tol["O"]
+        assert relerr(Sf[b:b + 1, hh:hh + 1], S_ref) <= tol["S"]
+        for n in ("dq", "dk", "dv", "df", "dbx", "dwx"):
+            assert relerr(g[n][b:b + 1, :, hh:hh + 1], g_ref[n]) <= tol["g"], (n, b, hh)
+        assert relerr(g["dbeta"][b:b + 1, :, hh:hh + 1], g_ref["dbeta"]) <= tol["g"]
+        assert relerr(g["dS0"][b:b + 1, hh:hh + 1], g_ref["dS0"]) <= tol["g"]
+    xs = synth.slice_chains(x, chains)
+    cts = synth.slice_chains(ct, chains)
+    sub = cfg.with_(B=len(chains), H=1)
+    _check_fwd_bwd(oracle, sub, xs, ct=cts)
+
+
+@pytest.mark.parametrize("L", [16, 32, 64, 128])
+def test_config2_chunk_sweep_reduced_batch(oracle, L):
+    """Config 2 (chunk-length sweep, gate projections ~N(0,0.1^2)) at full T = 8192 with B*H reduced to 2 chains."""
+    cfg = synth.CFG2[L].with_(B=1, H=2)
+    x = synth.make_inputs(cfg)
+    _check_fwd_bwd(oracle, cfg, x)
+
+
+def test_config4_many_short_reduced_batch(oracle):
+    """Config 4's shape and stress structure (beta = 1 on 10 %, no decay on 10 % of key dims) at T = 1024, B*H = 4*4."""
+    cfg = synth.CFG4.with_(B=4, H=4)
+    x = synth.make_inputs(cfg)
+    _check_fwd_bwd(oracle, cfg, x)
+
+
+def test_config3_long_context_forward_reduced_heads(oracle):
+    """Config 3 (forward only, T = 65536, d_v = 256, random S0) with H reduced to 2 chains."""
+    cfg = synth.CFG3.with_(H=2)
+    x = synth.make_inputs(cfg)
+    _check_fwd_bwd(oracle, cfg, x, with_bwd=False)
