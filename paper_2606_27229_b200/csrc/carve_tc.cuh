@@ -53,7 +53,7 @@ struct Layout {  // byte offsets into the 1024-aligned dynamic shared memory
         TP = take(16384);                   // rows 0..63 T = (I + beta A)^-1, rows 64..127 P
         if (tile_bytes(128, dk) >= 32768) { Mm = KQraw; Tm = KQraw + 16384; }
         else { Mm = take(16384); Tm = take(16384); }  // fp32 scratch of the triangular inverse
-        misc = take(7168);
+        misc = take(8192);
         total = o + 1024;                   // slack for the manual 1024-byte alignment
     }
 };
@@ -106,13 +106,13 @@ struct Misc {
     float etot[4][128];         // exp(sum of log a over 16-token anchor block b)
     float suf[4][128];          // product of etot[b'] over b' > b
     float gamL[128];            // gamma_{L-1} of the chunk
-    float nrm[128][2];          // partial sums of squares: rows 0..63 k, 64..127 q; [half]
+    float nrm[128][4];          // partial sums of squares: rows 0..63 k, 64..127 q; [column part]
     float beta[64];             // write strength of the chunk's tokens
     uint64_t bar_mma, bar_kq, bar_fb, bar_wv;
     uint32_t tmem_base;
 };
 
-static_assert(sizeof(Misc) <= 7168, "misc area too small");
+static_assert(sizeof(Misc) <= 8192, "misc area too small");
 
 __device__ __forceinline__ float softplus_fast(float x) { return fmaxf(x, 0.f) + __logf(1.f + __expf(-fabsf(x))); }
 __device__ __forceinline__ float sigmoid_fast(float x) { return __fdividef(1.f, 1.f + __expf(-x)); }

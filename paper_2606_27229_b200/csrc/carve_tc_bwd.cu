@@ -33,6 +33,7 @@ namespace carve {
 namespace {
 
 using namespace tcp;
+PROF_DECL(g_prof_bwd)
 
 struct BwdArgs {
     int B, H, T, L, r;
@@ -69,7 +70,7 @@ struct BLayout {  // byte offsets into the 1024-aligned dynamic shared memory
         TRI = take(24576);              // [64][192] 0/1: cols 0..63 t' > t, cols 64..127 t' >= t, cols 128..191 t' < t
         VcT = take(tile_bytes(32, d));  // rows i: [Vb^T ; Vw^T]
         Ucat = take(tile_bytes(32, d)); // rows i: [Ub ; Uw]
-        misc = take(8192);
+        misc = take(9216);
         total = o + 1024;
     }
 };
@@ -81,11 +82,15 @@ struct BMisc {
     float rn[128];        // 1/|k|, 1/|q| of the chunk's tokens
     float beta[64];
     float dbp[2][64];     // dbeta partial sums of the two column halves
-    float colp[4][128];   // column-sum partials per lane quadrant
+    float pre[4][128];    // gamma_a(b)/gamma_{-1}: product of etot[b'] over b' < b
+    union {               // thread j turns its four column-sum partials into suf[.][j]: same addresses, no hazard
+        float colp[4][128];   // column-sum partials per lane quadrant
+        float suf[4][128];    // gamma_L/gamma_a(b): product of etot[b'] over b' >= b
+    };
     uint64_t bar_mma, bar_g1, bar_g3, bar_sb, bar_g4a, bar_g4b, bar_g5, bar_g8;
     uint32_t tmem_base;
 };
-static_assert(sizeof(BMisc) <= 8192, "misc area too small");
+static_assert(sizeof(BMisc) <= 9216, "misc area too small");
 
 // ---- PTX helpers ----------------------------------------------------------------------------------
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
@@ -97,6 +102,12 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 __device__ __forceinline__ void ldsm_x4_t(uint32_t (&r)[4], uint32_t saddr)
 {
     asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                 : "r"(saddr));
+}
+__device__ __forceinline__ void ldsm_x4(uint32_t (&r)[4], uint32_t saddr)
+{
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
                  : "r"(saddr));
 }
@@ -277,6 +288,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     finalize(false, false);
 
     bool first = true;
+    PROF_INIT();
     for (int it = 0, c = nchunks - 1; c >= 0; --c, ++it) {
         const uint32_t ph = (uint32_t)it & 1u;
         const uint8_t* rc = rec_chain + (size_t)c * Rc.total;
@@ -313,6 +325,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 mi.gamLn[j] = g;   // read by finalize at the end of this chunk
             }
         }
+        PROF(g_prof_bwd, 0);
         // ---- L1: dU = Ktil dS'^T + (scale P)^T dO -> BM_A rows 0..63;  dKtil = U dS' -> BM_KT rows 0..63
         if (tid == 0) {
             mbar_wait(&mi.bar_g1, ph);
@@ -344,6 +357,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         } else {
             mma_ph ^= 1u;  // Q-side threads skip this wait
         }
+        PROF(g_prof_bwd, 1);
         // ---- L2: dX = T^T dU -> BM_A rows 64..127
         PHASE_SYNC();
         if (tid == 0) {
@@ -403,6 +417,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 bulk_g2s(sm + Lo.S[1], rc + Rc.CC, TB, &mi.bar_g4a);
             }
         }
+        PROF(g_prof_bwd, 2);
         // ---- L3: [dA;dP] raw, SP = [-dR;dO] S, dS += [-dR;dO]^T [Kbar; scale Qbar]
         PHASE_SYNC();
         if (tid == 0) {
@@ -438,6 +453,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 sts128(sm + Lo.S[4] + tile_chunk_off(128, row, 4 * half + ch), pack8(f8));
             }
         }
+        PROF(g_prof_bwd, 3);
         // ---- carry term of d log gamma: gamma_L . colsum(S . dS')  (dS' still sits in DSB as bf16)
         mbar_wait(&mi.bar_sb, ph);
         if (srow) {
@@ -455,6 +471,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
 #pragma unroll
             for (int i = 0; i < HK / 32; ++i) mi.colp[q][half * HK + (HK / 32) * lane + i] = p[i];
         }
+        PROF(g_prof_bwd, 4);
         // ---- L4: pairwise decay terms on mma.sync.  Warp w owns key channels [NCW w, NCW (w+1)) for all tokens, so the
         //      three pieces of d log gamma that cancel pairwise meet in one thread, in fp32:
         //        (i)  H_t  = sum_{s} [dA;dP]_ts C_s G(blk t, blk s)      (rows of both sides)
@@ -467,14 +484,16 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             float sx = 0.f;
 #pragma unroll
             for (int qq = 0; qq < D / 32; ++qq) sx += mi.colp[qq][tid];
-            mi.extra[tid] = sx * (mi.etot[0][tid] * mi.etot[1][tid] * mi.etot[2][tid] * mi.etot[3][tid]);
+            const float e0 = mi.etot[0][tid], e1 = mi.etot[1][tid], e2 = mi.etot[2][tid], e3 = mi.etot[3][tid];
+            mi.extra[tid] = sx * (e0 * e1 * e2 * e3);
+            mi.pre[0][tid] = 1.f; mi.pre[1][tid] = e0; mi.pre[2][tid] = e0 * e1; mi.pre[3][tid] = e0 * e1 * e2;
+            mi.suf[3][tid] = e3; mi.suf[2][tid] = e2 * e3; mi.suf[1][tid] = e1 * e2 * e3; mi.suf[0][tid] = e0 * e1 * e2 * e3;
         }
         {
             constexpr int NCW = D / 8, NTW = NCW / 8;
             const int g = lane >> 2, l4 = lane & 3, cw = NCW * warp;
             const int lrow = (lane & 7) + ((lane >> 3) & 1) * 8;
             const int lchk = NTW == 2 ? (lane >> 4) : 0;
-            const uint8_t* dap = sm + Lo.S[4];
             float et[4][NTW][2];
 #pragma unroll
             for (int b2 = 0; b2 < 4; ++b2)
@@ -510,11 +529,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
 #pragma unroll
                         for (int jb = 0; jb < 4; ++jb) {
                             if (jb <= ib) {
-                                uint32_t af[4];
-                                af[0] = *reinterpret_cast<const uint32_t*>(dap + tile_off(128, r0 + g, 16 * jb + 2 * l4));
-                                af[1] = *reinterpret_cast<const uint32_t*>(dap + tile_off(128, r0 + g + 8, 16 * jb + 2 * l4));
-                                af[2] = *reinterpret_cast<const uint32_t*>(dap + tile_off(128, r0 + g, 16 * jb + 2 * l4 + 8));
-                                af[3] = *reinterpret_cast<const uint32_t*>(dap + tile_off(128, r0 + g + 8, 16 * jb + 2 * l4 + 8));
+                                uint32_t af[4];   // A[m = t][k = s] = DAP[t][s]: matrix m: rows r0 + 8 (m&1), chunk 2 jb + (m>>1)
+                                ldsm_x4(af, sb + Lo.S[4] + tile_chunk_off(128, r0 + lrow, 2 * jb + (lane >> 4)));
 #pragma unroll
                                 for (int nt = 0; nt < NTW; ++nt) {
                                     mma_bf16(accI[mt][nt], af, bC[jb][nt][0], bC[jb][nt][1]);
@@ -640,6 +656,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 }
             }
         }
+        PROF(g_prof_bwd, 5);
         // ---- L5: assemble dk^, dq^ (state part) and the state-read / state-write contributions to d log gamma
         __syncthreads();
         if (warp_active) {
@@ -672,22 +689,19 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                             unpack8(lds128(sm + Lo.S[4] + tile_chunk_off(64, t, cc)), pc);
                             unpack8(lds128(sm + Lo.S[5] + tile_chunk_off(64, t, cc)), k0);
                             unpack8(lds128(sm + Lo.S[1] + tile_chunk_off(64, t, cc)), c8);
+                            float pre[8], suf[8];   // gamma_a(blk)/gamma_{-1} and gamma_L/gamma_a(blk)
+                            *reinterpret_cast<float4*>(pre) = *reinterpret_cast<const float4*>(&mi.pre[blk][j0]);
+                            *reinterpret_cast<float4*>(pre + 4) = *reinterpret_cast<const float4*>(&mi.pre[blk][j0 + 4]);
+                            *reinterpret_cast<float4*>(suf) = *reinterpret_cast<const float4*>(&mi.suf[blk][j0]);
+                            *reinterpret_cast<float4*>(suf + 4) = *reinterpret_cast<const float4*>(&mi.suf[blk][j0 + 4]);
 #pragma unroll
                             for (int e = 0; e < 8; ++e) {
-                                const int j = j0 + e;
-                                float pre = 1.f, suf = 1.f;   // gamma_a(blk)/gamma_{-1} and gamma_L/gamma_a(blk)
-#pragma unroll
-                                for (int b2 = 0; b2 < 4; ++b2) {
-                                    const float etv = mi.etot[b2][j];
-                                    pre *= b2 < blk ? etv : 1.f;
-                                    suf *= b2 >= blk ? etv : 1.f;
-                                }
                                 const float sp = __uint_as_float(vs[8 * ch + e]), dkt = __uint_as_float(vk[8 * ch + e]);
-                                const float dkA = fp[e] * (pk[e] + pre * sp);
-                                const float dkC = ic[e] * (pc[e] + suf * dkt);
+                                const float dkA = fp[e] * (pk[e] + pre[e] * sp);
+                                const float dkC = ic[e] * (pc[e] + suf[e] * dkt);
                                 o[e] = dkA + dkC;
                                 xa[e] = k0[e] * sp;                 // Kbar_t . dKbar_t (state read), to d log gamma_{t-1}
-                                zz[e] = (c8[e] * suf) * dkt;        // Ktil_t . dKtil_t (state write), to d log gamma_t' for t' > t
+                                zz[e] = (c8[e] * suf[e]) * dkt;     // Ktil_t . dKtil_t (state write), to d log gamma_t' for t' > t
                             }
                             stg128(gdk + j0, pack8(o));
                             sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8(xa));   // in place over H_t
@@ -714,14 +728,13 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                             unpack8(fq4[i], fq);
                             unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc)), pq);
                             unpack8(lds128(sm + Lo.S[6] + tile_chunk_off(64, t, cc)), q0);
+                            float pre[8];
+                            *reinterpret_cast<float4*>(pre) = *reinterpret_cast<const float4*>(&mi.pre[blk][j0]);
+                            *reinterpret_cast<float4*>(pre + 4) = *reinterpret_cast<const float4*>(&mi.pre[blk][j0 + 4]);
 #pragma unroll
                             for (int e = 0; e < 8; ++e) {
-                                const int j = j0 + e;
-                                float pre = 1.f;
-#pragma unroll
-                                for (int b2 = 0; b2 < 4; ++b2) pre *= b2 < blk ? mi.etot[b2][j] : 1.f;
                                 const float sp = __uint_as_float(vs[8 * ch + e]);
-                                vs[8 * ch + e] = __float_as_uint(fq[e] * (pq[e] + pre * a.scale * sp));
+                                vs[8 * ch + e] = __float_as_uint(fq[e] * (pq[e] + pre[e] * a.scale * sp));
                                 xq[e] = q0[e] * sp;                 // scale Qbar_t . (dO S)_t (state read)
                             }
                             sts128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc), pack8(xq));   // in place over H_t
@@ -732,6 +745,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 tmem_wait_st();
             }
         }
+        PROF(g_prof_bwd, 6);
         // ---- L6: d log a_t = dlp_t + carry + sum_{t' > t} XA_t' + sum_{t' >= t} XQ_t' + sum_{t' < t} Z_t'  -> BM_KT rows 0..63
         PHASE_SYNC();
         if (tid == 0) {
@@ -805,6 +819,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 }
             }
         }
+        PROF(g_prof_bwd, 7);
         // ---- L7: ZZ = [db_pre; dw_pre] [Vb | Vw] -> BM_DAP;  dVb | dVw += [db_pre; dw_pre]^T TT2 -> BM_WG
         PHASE_SYNC();
         if (tid == 0) {
@@ -842,6 +857,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 }
             }
         }
+        PROF(g_prof_bwd, 8);
         // ---- L8: dq^ += dz G -> BM_A rows 64..127;  dG^T = q^T (dz/|q|) -> BM_DAP + 32
         PHASE_SYNC();
         if (tid == 0) {
@@ -883,6 +899,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 sts128(sm + Lo.S[1] + tile_chunk_off(D, row, ch), pack8(f8));
             }
         }
+        PROF(g_prof_bwd, 9);
         // ---- L9: fold glue: dS += [Ub;Uw]^T dG;  d[Ub;Uw]^T += S dG^T -> BM_WU
         PHASE_SYNC();
         if (tid == 0) {
@@ -895,8 +912,11 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mbar_expect_tx(&mi.bar_sb, SBb);
             bulk_g2s(sm + Lo.SBq, rc - Rc.total + Rc.SB, SBb, &mi.bar_sb);
         }
+        PROF(g_prof_bwd, 10);
         // ---- L10: the adjoint of the state entering the chunk
+        PROF(g_prof_bwd, 11);
         finalize(true, c == 0);
+        PROF(g_prof_bwd, 12);
         first = false;
     }
 
@@ -1058,6 +1078,15 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
 }
 
 }  // namespace
+
+#ifdef CARVE_PROFILE
+extern "C" void carve_debug_prof_bwd(unsigned long long* out)
+{
+    cudaMemcpyFromSymbol(out, g_prof_bwd, sizeof(g_prof_bwd));
+    unsigned long long z[40] = {};
+    cudaMemcpyToSymbol(g_prof_bwd, z, sizeof(z));
+}
+#endif
 
 bool tc_bwd_supported(const carve_params_t& p) { return tc_fwd_supported(p) && p.L <= 64; }
 

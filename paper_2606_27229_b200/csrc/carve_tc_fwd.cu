@@ -27,6 +27,7 @@ namespace carve {
 namespace {
 
 using namespace tcp;
+PROF_DECL(g_prof_fwd)
 
 struct TcArgs {
     int B, H, T, L, r;
@@ -106,7 +107,7 @@ __device__ __forceinline__ void warp_store(float* Q, int qr, int qc, const float
 // Tm <- (I + Mm)^-1 for the leading n x n block (n in {16,32,64}); Mm strictly lower (only that part is read).
 // Blocked forward substitution (Alg. 2 step 7): 16x16 diagonal blocks by substitution, then
 // T_ij = -T_ii (M_ij T_jj) one level at a time, the block products on tensor cores (tf32 mma.sync).
-__device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid)
+__device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid, int nthreads)
 {
     const int warp = tid >> 5, lane = tid & 31;
     if (tid < n) {
@@ -122,7 +123,7 @@ __device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid)
         }
     } else if (n >= 64) {
         // blocks (0,1) and (2,3) of T are zero; the level-64 products read them
-        for (int i = tid - 64; i < 512; i += NT - 64) {
+        for (int i = tid - 64; i < 512; i += nthreads - 64) {
             const int blk = i >> 8, rr = (i >> 4) & 15, cc = i & 15;
             Tm[mm_idx(32 * blk + rr, 32 * blk + 16 + cc)] = 0.f;
         }
@@ -172,15 +173,18 @@ __device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid)
         tc_fence_after();                   \
     } while (0)
 
-template <int DK, int DV>
-__global__ void __launch_bounds__(NT, 1)
+// NP = number of column parts a tile row is split into = warpgroups per CTA (threads = 128 NP); every thread
+// serves one TMEM lane (tile row) and DK/NP columns.
+template <int DK, int DV, int NP>
+__global__ void __launch_bounds__(128 * NP, 1)
 carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, const __grid_constant__ CUtensorMap mk,
                     const __grid_constant__ CUtensorMap mv, const __grid_constant__ CUtensorMap mf,
                     const __grid_constant__ CUtensorMap mbx, const __grid_constant__ CUtensorMap mwx)
 {
     static_assert(DK == DV, "the shared-memory map assumes dk == dv");
     constexpr int DM = DK > DV ? DK : DV;
-    constexpr int HK = DK / 2, HV = DV / 2;  // columns per warpgroup half
+    constexpr int NTH = 128 * NP;
+    constexpr int HK = DK / NP, HV = DV / NP;  // columns per warpgroup ("half" = part index 0..NP-1)
     extern __shared__ uint8_t smem_raw[];
     uint8_t* sm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     const int r = a.r, R2 = 2 * r;
@@ -210,19 +214,19 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         tma_prefetch_desc(&mf); tma_prefetch_desc(&mbx); tma_prefetch_desc(&mwx);
     }
     if (warp == 0) tmem_alloc(&mi.tmem_base, TM_COLS);
-    for (int i = tid; i < R2 * DV; i += NT) {
+    for (int i = tid; i < R2 * DV; i += NTH) {
         const int ii = i / DV, x = i % DV;
         const float v = ii < r ? __ldg(a.Ub + (size_t)ii * DV + x) : __ldg(a.Uw + (size_t)(ii - r) * DV + x);
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Ucat + tile_off(R2, ii, x)) = __float2bfloat16_rn(v);
     }
-    for (int i = tid; i < DM * 64; i += NT) {
+    for (int i = tid; i < DM * 64; i += NTH) {
         const int n = i / 64, c = i % 64;
         float v = 0.f;
         if (c < r) { if (n < DK) v = __ldg(a.Vb + (size_t)n * r + c); }
         else if (c < R2) { if (n < DV) v = __ldg(a.Vw + (size_t)n * r + (c - r)); }
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Vcat + tile_off(DM, n, c)) = __float2bfloat16_rn(v);
     }
-    for (int j = tid; j < DK; j += NT) {
+    for (int j = tid; j < DK; j += NTH) {
         mi.eA[j] = a.A ? __expf(__ldg(a.A + h * DK + j)) : 1.f;
         mi.tau[j] = a.tau ? __ldg(a.tau + h * DK + j) : 0.f;
     }
@@ -261,6 +265,12 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         tmem_wait_st();
     }
 
+    auto sumsq = [&](int rw) {
+        float ss = 0.f;
+#pragma unroll
+        for (int pp = 0; pp < NP; ++pp) ss += mi.nrm[rw][pp];
+        return ss;
+    };
     auto issue_kq = [&](int c) {
         mbar_expect_tx(&mi.bar_kq, 2u * LCc * DK * 2u);
         const int tr = b * a.T + c * LCc;
@@ -288,10 +298,12 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     if (tid == 0) { fence_async_smem(); issue_kq(0); issue_fb(0); issue_wv(0); }
 
     uint32_t mma_ph = 0, tma_ph = 0;
+    PROF_INIT();
     for (int c = 0; c < nchunks; ++c) {
         const bool fold_now = (c % gate_every) == 0;
         const size_t tok0 = (size_t)b * a.T + (size_t)c * LCc;  // first token of the chunk
         uint8_t* rc = rec_chain ? rec_chain + (size_t)c * Rc.total : nullptr;  // this chunk's record
+        PROF(g_prof_fwd, 0);
         // ---- P0: fold G^T = S^T Ucat^T -> TM_X2[0, R2)
         PHASE_SYNC();
         if (fold_now && tid == 0) {
@@ -319,6 +331,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         if (fold_now) {
             WAIT_MMA();
+            PROF(g_prof_fwd, 1);
             // ---- P1: G^T (lanes j) -> bf16 into the spare columns [32, 32+R2) of the Vcat tile
             if (half == 0 && q * 32 < DK) {
                 for (int c0 = 0; c0 < R2; c0 += 16) {
@@ -337,6 +350,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
+        PROF(g_prof_fwd, 2);
         // ---- P2: Z = [k;q] G^T -> TM_X2[32, 32+R2)
         PHASE_SYNC();
         if (tid == 0) {
@@ -344,9 +358,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             umma_commit(&mi.bar_mma);
         }
         WAIT_MMA();
+        PROF(g_prof_fwd, 3);
         // ---- P3: tt = tanh(Z rnorm_q) -> [0 tt_w; tt_b 0];  block-triangular +-1 matrix
         if (!krole && half == 0 && warp_active) {
-            const float rnq = a.l2norm ? rsqrtf(mi.nrm[row][0] + mi.nrm[row][1] + a.eps) : 1.f;
+            const float rnq = a.l2norm ? rsqrtf(sumsq(row) + a.eps) : 1.f;
             const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
             for (int c0 = 0; c0 < R2; c0 += 16) {
                 uint32_t v[16];
@@ -386,6 +401,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 sts128(sm + Lo.Y2 + tile_chunk_off(128, row, ch), make_uint4(w[0], w[1], w[2], w[3]));
             }
         }
+        PROF(g_prof_fwd, 4);
         // ---- P4: [w_proj; b_proj] = Ablk Vcat^T -> TM_X1
         PHASE_SYNC();
         if (tid == 0) {
@@ -395,6 +411,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         mbar_wait(&mi.bar_fb, tma_ph);
         mbar_wait(&mi.bar_wv, tma_ph);
         WAIT_MMA();
+        PROF(g_prof_fwd, 5);
         // ---- P5: gates (8 columns per step; cc = 16-byte chunk index inside the row)
         if (warp_active) {
             if (!krole) {
@@ -451,6 +468,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
+        PROF(g_prof_fwd, 6);
         // ---- P6: block-local prefix sums -> TM_X2[0, DK): rows 0..63 a_b - lg_t, rows 64..127 lg_t - a_b
         PHASE_SYNC();
         if (tid == 0) {
@@ -459,6 +477,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             umma_commit(&mi.bar_mma);
         }
         WAIT_MMA();
+        PROF(g_prof_fwd, 7);
         // ---- P7a: exp of the block totals (last token of each 16-token anchor block), then their suffix products
         if (!krole && warp_active) {
             const int blk = t >> 4;
@@ -490,6 +509,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             }
         }
         __syncthreads();
+        PROF(g_prof_fwd, 8);
         // ---- P7b: decayed operands.  Row operands exist in up to four anchorings: version 0 relative to the chunk
         //      start (Kbar, Qbar: also the operand of the state products), version jb relative to the start of
         //      anchor block jb (only rows at or after that block).  Column operand C_s is relative to its own block.
@@ -505,11 +525,11 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             };
             if (!krole) {
-                const float rnq = a.l2norm ? rsqrtf(mi.nrm[row][0] + mi.nrm[row][1] + a.eps) : 1.f;
+                const float rnq = a.l2norm ? rsqrtf(sumsq(row) + a.eps) : 1.f;
                 const int tn = t + 1;  // the key row that shares this token's retention (Kbar_{t+1} = k^_{t+1} gamma_t)
                 const bool has_next = tn < LCc;
                 const int bn = tn >> 4, krow = has_next ? tn : 0;
-                const float rnk = a.l2norm ? rsqrtf(mi.nrm[krow][0] + mi.nrm[krow][1] + a.eps) : 1.f;
+                const float rnk = a.l2norm ? rsqrtf(sumsq(krow) + a.eps) : 1.f;
                 if (rc && live && half == 0) reinterpret_cast<float*>(rc + Rc.rn)[64 + t] = rnq;
 #pragma unroll 1
                 for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
@@ -569,7 +589,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     }
                 }
             } else {
-                const float rnk = a.l2norm ? rsqrtf(mi.nrm[row][0] + mi.nrm[row][1] + a.eps) : 1.f;
+                const float rnk = a.l2norm ? rsqrtf(sumsq(row) + a.eps) : 1.f;
                 if (rc && live && half == 0) reinterpret_cast<float*>(rc + Rc.rn)[t] = rnk;
 #pragma unroll 1
                 for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
@@ -603,6 +623,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
+        PROF(g_prof_fwd, 9);
         // ---- P8: A|P blocks (one 16-column block per anchoring) and the state products
         PHASE_SYNC();
         if (tid == 0) {
@@ -615,6 +636,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             umma_commit(&mi.bar_mma);
         }
         WAIT_MMA();
+        PROF(g_prof_fwd, 10);
         // ---- P9a: beta A -> Mm (fp32, only the strictly lower part is ever read), P -> TP rows 64.. (bf16, masked s <= t)
         {
             // one 16-column piece [16 jb, 16 jb + 16) of row `tok`
@@ -657,6 +679,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         }
                     }
                 }
+            }
+            if (half == 2 % NP) {
                 if (nb > 2) {
                     // version 2 (M = 64): compact row m = 16 q + lane sits in lane < 16 of warp q; m < 32: K token 32+m, else Q token m
                     tmem_ld16(tmem + TM_X2 + 32 + lane_base, v);
@@ -666,7 +690,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         if (tok < LCc) put_piece(q >= 2, tok, 2, v);
                     }
                 }
-            } else {
+            }
+            if (half == 1) {
                 if (nb > 1) {
                     // version 1 (M = 128 over a 96-row tile): lanes 0..47 K tokens 16.., lanes 48..95 Q tokens 16..
                     tmem_ld16(tmem + TM_X2 + 16 + lane_base, v);
@@ -677,6 +702,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         if (tok < LCc) put_piece(qr, tok, 1, v);
                     }
                 }
+            }
+            if (half == 3 % NP) {
                 if (nb > 3) {
                     // version 3 (M = 64 over a 32-row tile): m < 16: K token 48+m (warp 0), 16 <= m < 32: Q token 32+m (warp 1)
                     tmem_ld16(tmem + TM_X2 + 48 + lane_base, v);
@@ -685,6 +712,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
+        PROF(g_prof_fwd, 11);
         // ---- P9b: beta R = beta (V' - Kbar S^T) -> Y2 (rows t)
         if (krole && warp_active) {
             const float bt = live ? sBeta[t] : 0.f;
@@ -704,8 +732,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             }
         }
         __syncthreads();
+        PROF(g_prof_fwd, 12);
         // ---- P9c: T = (I + beta A)^-1 -> TP rows 0..63 (bf16, zero above the diagonal)
-        tri_inverse(Mm, Tm, LCc, tid);
+        tri_inverse(Mm, Tm, LCc, tid, NTH);
         {
             const int tr_ = tid >> 2, qq = tid & 3;  // row, 16-column quarter
             if (tr_ < LCc) {
@@ -722,6 +751,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
+        PROF(g_prof_fwd, 13);
         // ---- P10: U = T (beta R) -> TM_X1
         PHASE_SYNC();
         if (tid == 0) {
@@ -730,6 +760,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             if (c + 1 < nchunks) issue_kq(c + 1);
         }
         WAIT_MMA();
+        PROF(g_prof_fwd, 14);
         // ---- P11: U -> bf16 rows (over V')
         if (krole && warp_active) {
             const float rbt = live ? __fdividef(1.f, sBeta[t]) : 0.f;
@@ -753,6 +784,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
+        PROF(g_prof_fwd, 15);
         // ---- P12: O += P U;  W = U^T Ktil -> TM_X2
         PHASE_SYNC();
         if (tid == 0) {
@@ -762,6 +794,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         WAIT_MMA();
         if (tid == 0 && c + 1 < nchunks) { fence_async_smem(); issue_fb(c + 1); issue_wv(c + 1); }
+        PROF(g_prof_fwd, 16);
         // ---- P13: outputs and the state carry
         if (!krole && warp_active) {
             __nv_bfloat16* dst = a.O + ((tok0 + t) * a.H + h) * DV;
@@ -808,6 +841,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             tmem_wait_st();
         }
         tma_ph ^= 1u;
+        PROF(g_prof_fwd, 17);
     }
     PHASE_SYNC();
     if (warp == 0) tmem_dealloc(tmem, TM_COLS);
@@ -848,6 +882,15 @@ bool tc_make_token_map(CUtensorMap* map, const void* base, int B, int T, int H, 
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+#ifdef CARVE_PROFILE
+extern "C" void carve_debug_prof_fwd(unsigned long long* out)
+{
+    cudaMemcpyFromSymbol(out, g_prof_fwd, sizeof(g_prof_fwd));
+    unsigned long long z[40] = {};
+    cudaMemcpyToSymbol(g_prof_fwd, z, sizeof(z));
+}
+#endif
+
 bool tc_fwd_supported(const carve_params_t& p)
 {
     return p.dtype == CARVE_BF16 && p.dk == p.dv && (p.dk == 64 || p.dk == 128) && p.r <= 16;
@@ -871,10 +914,11 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, uint8_t* sfin, cud
     t.A = a.A; t.tau = a.tau; t.Ub = a.Ub; t.Uw = a.Uw; t.Vb = a.Vb; t.Vw = a.Vw; t.S0 = a.S0;
     t.O = static_cast<__nv_bfloat16*>(a.O); t.S_final = a.S_final; t.rec = rec; t.sfin = sfin;
     const size_t smem = tcp::Layout(D, D, 2 * a.r).total;
-    auto kern = carve_fwd_tc_kernel<D, D>;
+    constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
+    auto kern = carve_fwd_tc_kernel<D, D, NP>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<a.B * a.H, tcp::NT, smem, st>>>(t, mq, mk, mv, mf, mbx, mwx);
+    kern<<<a.B * a.H, 128 * NP, smem, st>>>(t, mq, mk, mv, mf, mbx, mwx);
     return cudaGetLastError();
 }
 

@@ -15,6 +15,22 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// Optional per-phase cycle counters (build with -DCARVE_PROFILE; block 0, thread 0 = the MMA-issuing thread).
+#ifdef CARVE_PROFILE
+#define PROF_DECL(name) static __device__ unsigned long long name[40];
+#define PROF_INIT() long long prof_t_ = clock64();
+#define PROF(name, i)                                        \
+    if (blockIdx.x == 0 && threadIdx.x == 0) {               \
+        const long long prof_n_ = clock64();                 \
+        name[i] += (unsigned long long)(prof_n_ - prof_t_);  \
+        prof_t_ = prof_n_;                                   \
+    }
+#else
+#define PROF_DECL(name)
+#define PROF_INIT()
+#define PROF(name, i)
+#endif
+
 namespace carve {
 namespace tc {
 
