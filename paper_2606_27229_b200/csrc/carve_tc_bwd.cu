@@ -59,7 +59,7 @@ constexpr uint32_t BM_WU = 480;   // [x lanes][32]  d[Ub;Uw]^T, accumulated over
 
 constexpr uint32_t SLOT = 16384;
 struct BLayout {  // byte offsets into the 1024-aligned dynamic shared memory
-    uint32_t DSB, SBq, S[7], TRI, VcT, Ucat, misc, total;
+    uint32_t DSB, SBq, S[7], TRI, VcT, Ucat, FI, misc, total;
     __host__ __device__ BLayout(int d)
     {
         uint32_t o = 0;
@@ -70,6 +70,8 @@ struct BLayout {  // byte offsets into the 1024-aligned dynamic shared memory
         TRI = take(24576);              // [64][192] 0/1: cols 0..63 t' > t, cols 64..127 t' >= t, cols 128..191 t' < t
         VcT = take(tile_bytes(32, d));  // rows i: [Vb^T ; Vw^T]
         Ucat = take(tile_bytes(32, d)); // rows i: [Ub ; Uw]
+        // staging of row-private record tiles (FQ | IC, later b): over DSB once dS' is consumed when it fits (d = 128)
+        FI = tile_bytes(d, d) >= 2 * tile_bytes(64, d) ? DSB : take(2 * tile_bytes(64, d));
         misc = take(9216);
         total = o + 1024;
     }
@@ -87,7 +89,7 @@ struct BMisc {
         float colp[4][128];   // column-sum partials per lane quadrant
         float suf[4][128];    // gamma_L/gamma_a(b): product of etot[b'] over b' >= b
     };
-    uint64_t bar_mma, bar_g1, bar_g3, bar_sb, bar_g4a, bar_g4b, bar_g5, bar_g8;
+    uint64_t bar_mma, bar_g1, bar_g3, bar_sb, bar_g4a, bar_g4b, bar_g5, bar_g8, bar_fi, bar_bg;
     uint32_t tmem_base;
 };
 static_assert(sizeof(BMisc) <= 9216, "misc area too small");
@@ -133,17 +135,12 @@ __device__ __forceinline__ void split8(const float* x, uint4& hi, uint4& lo)
 __device__ __forceinline__ uint4 ldg128(const uint8_t* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
 __device__ __forceinline__ void stg128(void* p, uint4 v) { *reinterpret_cast<uint4*>(p) = v; }
 
-// Product over K (multiple of 16) from two row tiles, with explicit K offsets (see tc_common.cuh umma_tiles).
+// Product over K (multiple of 16) from two row tiles, with explicit K offsets (tc_common.cuh umma_tiles_rt), M = 128.
 template <int AMAJ, int BMAJ>
 __device__ __forceinline__ void mma_k(uint32_t d_tmem, int N, uint32_t a_saddr, int a_rows, int a_o0, int a_k0,
                                       uint32_t b_saddr, int b_rows, int b_o0, int b_k0, int K, bool accumulate)
 {
-    const uint32_t idesc = umma_idesc(128, N, AMAJ, BMAJ);
-    for (int k = 0; k < K; k += 16) {
-        const uint64_t ad = AMAJ == KMAJ ? desc_kmajor(a_saddr, a_rows, a_o0, a_k0 + k) : desc_mnmajor(a_saddr, a_rows, a_o0, a_k0 + k);
-        const uint64_t bd = BMAJ == KMAJ ? desc_kmajor(b_saddr, b_rows, b_o0, b_k0 + k) : desc_mnmajor(b_saddr, b_rows, b_o0, b_k0 + k);
-        umma(d_tmem, ad, bd, idesc, (accumulate || k > 0) ? 1u : 0u);
-    }
+    umma_tiles_rt<AMAJ, BMAJ>(d_tmem, 128, N, a_saddr, a_rows, a_o0, a_k0, b_saddr, b_rows, b_o0, b_k0, K, accumulate);
 }
 
 // Column sums over the 32 lanes of a warp by a halving butterfly: on return lane l holds in v[0..N/32)
@@ -217,6 +214,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     if (tid == 0) {
         mbar_init(&mi.bar_mma, 1); mbar_init(&mi.bar_g1, 1); mbar_init(&mi.bar_g3, 1); mbar_init(&mi.bar_sb, 1);
         mbar_init(&mi.bar_g4a, 1); mbar_init(&mi.bar_g4b, 1); mbar_init(&mi.bar_g5, 1); mbar_init(&mi.bar_g8, 1);
+        mbar_init(&mi.bar_fi, 1); mbar_init(&mi.bar_bg, 1);
         mbar_fence_init();
         tma_prefetch_desc(&mdO); tma_prefetch_desc(&mk); tma_prefetch_desc(&mq);
     }
@@ -326,6 +324,18 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             }
         }
         PROF(g_prof_bwd, 0);
+        // row-private record data of L2 straight from global memory: the Q-side threads, idle through L1, issue the
+        // loads now so that their latency hides behind L1
+        uint4 e4[HK / 8], x4[HK / 8], w4[HK / 8];
+        if (!krole && live) {
+#pragma unroll
+            for (int i = 0; i < HK / 8; ++i) {
+                const uint32_t off = tile_chunk_off(64, t, half * (HK / 8) + i);
+                e4[i] = ldg128(rc + Rc.E + off);
+                x4[i] = ldg128(rc + Rc.VWX + off);
+                w4[i] = ldg128(rc + Rc.W + off);
+            }
+        }
         // ---- L1: dU = Ktil dS'^T + (scale P)^T dO -> BM_A rows 0..63;  dKtil = U dS' -> BM_KT rows 0..63
         if (tid == 0) {
             mbar_wait(&mi.bar_g1, ph);
@@ -365,17 +375,6 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             umma_commit(&mi.bar_mma);
         }
         if (!krole) {
-            // row-private record data straight from global memory, issued before the MMA wait
-            uint4 e4[HK / 8], x4[HK / 8], w4[HK / 8];
-            if (live) {
-#pragma unroll
-                for (int i = 0; i < HK / 8; ++i) {
-                    const uint32_t off = tile_chunk_off(64, t, half * (HK / 8) + i);
-                    e4[i] = ldg128(rc + Rc.E + off);
-                    x4[i] = ldg128(rc + Rc.VWX + off);
-                    w4[i] = ldg128(rc + Rc.W + off);
-                }
-            }
             WAIT_MMA();
             if (warp_active) {
                 const float bt = live ? mi.beta[t] : 0.f;
@@ -480,6 +479,11 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         //      (t,s) enters +Kbar_own_t C_s dA_ts G in row t and -C_s Kbar_own_t dA_ts G in row s with bit-identical
         //      operands, so the pairs that do not straddle a token cancel to fp32 rounding in the reverse cumulative sum.
         __syncthreads();
+        if (tid == 0) {   // dS' (DSB) is consumed: stage gamma_t/gamma_a and its inverse there for L5
+            mbar_expect_tx(&mi.bar_fi, 2 * TB);
+            bulk_g2s(sm + Lo.FI, rc + Rc.FQ, TB, &mi.bar_fi);
+            bulk_g2s(sm + Lo.FI + TB, rc + Rc.IC, TB, &mi.bar_fi);
+        }
         if (tid < D) {
             float sx = 0.f;
 #pragma unroll
@@ -659,19 +663,11 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROF(g_prof_bwd, 5);
         // ---- L5: assemble dk^, dq^ (state part) and the state-read / state-write contributions to d log gamma
         __syncthreads();
+        mbar_wait(&mi.bar_fi, ph);
         if (warp_active) {
             if (krole) {
-                uint4 fq4[HK / 8], ic4[HK / 8];
                 const bool bstart = (t & 15) == 0;
-                if (live) {
-#pragma unroll
-                    for (int i = 0; i < HK / 8; ++i) {
-                        const int cc = half * (HK / 8) + i;
-                        fq4[i] = bstart ? make_uint4(0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u)
-                                        : ldg128(rc + Rc.FQ + tile_chunk_off(64, t - 1, cc));
-                        ic4[i] = ldg128(rc + Rc.IC + tile_chunk_off(64, t, cc));
-                    }
-                }
+                const uint4 ones4 = make_uint4(0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u);
                 __nv_bfloat16* gdk = a.dk + ((tok0 + t) * a.H + h) * D;
 #pragma unroll
                 for (int s = 0; s < HK; s += 16) {
@@ -684,7 +680,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         for (int ch = 0; ch < 2; ++ch) {
                             const int i = s / 8 + ch, cc = half * (HK / 8) + i, j0 = 8 * cc;
                             float fp[8], ic[8], pk[8], pc[8], k0[8], c8[8], o[8], xa[8], zz[8];
-                            unpack8(fq4[i], fp); unpack8(ic4[i], ic);
+                            unpack8(bstart ? ones4 : lds128(sm + Lo.FI + tile_chunk_off(64, t - 1, cc)), fp);
+                            unpack8(lds128(sm + Lo.FI + TB + tile_chunk_off(64, t, cc)), ic);
                             unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, t, cc)), pk);
                             unpack8(lds128(sm + Lo.S[4] + tile_chunk_off(64, t, cc)), pc);
                             unpack8(lds128(sm + Lo.S[5] + tile_chunk_off(64, t, cc)), k0);
@@ -710,11 +707,6 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                     }
                 }
             } else {
-                uint4 fq4[HK / 8];
-                if (live) {
-#pragma unroll
-                    for (int i = 0; i < HK / 8; ++i) fq4[i] = ldg128(rc + Rc.FQ + tile_chunk_off(64, t, half * (HK / 8) + i));
-                }
 #pragma unroll
                 for (int s = 0; s < HK; s += 16) {
                     uint32_t vs[16];
@@ -725,7 +717,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         for (int ch = 0; ch < 2; ++ch) {
                             const int i = s / 8 + ch, cc = half * (HK / 8) + i, j0 = 8 * cc;
                             float fq[8], pq[8], q0[8], xq[8];
-                            unpack8(fq4[i], fq);
+                            unpack8(lds128(sm + Lo.FI + tile_chunk_off(64, t, cc)), fq);
                             unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc)), pq);
                             unpack8(lds128(sm + Lo.S[6] + tile_chunk_off(64, t, cc)), q0);
                             float pre[8];
@@ -758,14 +750,12 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             bulk_g2s(sm + Lo.S[5], rc + Rc.GT, tile_bytes(D, 64), &mi.bar_g8);
             mbar_expect_tx(&mi.bar_g5, (uint32_t)LCc * D * 2u);
             for (int cb = 0; cb < D / 64; ++cb) tma_load_3d(sm + Lo.S[6] + cb * 8192, &mq, &mi.bar_g5, cb * 64, h, trow);
+            mbar_expect_tx(&mi.bar_bg, TB);   // the erase gate b over gamma_t/gamma_a (dead after L5)
+            bulk_g2s(sm + Lo.FI, rc + Rc.Bg, TB, &mi.bar_bg);
         }
         if (krole) {
-            uint4 b4[HK / 8];
-            if (live) {
-#pragma unroll
-                for (int i = 0; i < HK / 8; ++i) b4[i] = ldg128(rc + Rc.Bg + tile_chunk_off(64, t, half * (HK / 8) + i));
-            }
             WAIT_MMA();
+            mbar_wait(&mi.bar_bg, ph);
             if (warp_active) {
                 __nv_bfloat16* gdf = a.df + ((tok0 + t) * a.H + h) * D;
                 __nv_bfloat16* gdbx = a.dbx + ((tok0 + t) * a.H + h) * D;
@@ -779,7 +769,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         for (int ch = 0; ch < 4; ++ch) {
                             const int i = s / 8 + ch, cc = half * (HK / 8) + i;
                             float bb[8], dp[8], dla[8], dbp[8];
-                            unpack8(b4[i], bb);
+                            unpack8(lds128(sm + Lo.FI + tile_chunk_off(64, t, cc)), bb);
                             unpack8(lds128(sm + Lo.S[0] + tile_chunk_off(64, t, cc)), dp);
 #pragma unroll
                             for (int e = 0; e < 8; ++e) {

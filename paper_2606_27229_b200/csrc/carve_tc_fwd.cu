@@ -41,17 +41,12 @@ struct TcArgs {
     uint8_t* sfin;  // [chains] bf16 row tile of the final state (the reverse kernel's first "next state")
 };
 
-// Runtime-shaped product from two row tiles (see tc_common.cuh umma_tiles); M fixed at compile time.
+// Runtime-shaped product from two row tiles (see tc_common.cuh umma_tiles_rt); M fixed at compile time.
 template <int M, int AMAJ, int BMAJ>
 __device__ __forceinline__ void mma_rt(uint32_t d_tmem, int N, uint32_t a_saddr, int a_rows, int a_o0, uint32_t b_saddr,
                                        int b_rows, int b_o0, int K, bool accumulate)
 {
-    const uint32_t idesc = umma_idesc(M, N, AMAJ, BMAJ);
-    for (int k = 0; k < K; k += 16) {
-        const uint64_t ad = AMAJ == KMAJ ? desc_kmajor(a_saddr, a_rows, a_o0, k) : desc_mnmajor(a_saddr, a_rows, a_o0, k);
-        const uint64_t bd = BMAJ == KMAJ ? desc_kmajor(b_saddr, b_rows, b_o0, k) : desc_mnmajor(b_saddr, b_rows, b_o0, k);
-        umma(d_tmem, ad, bd, idesc, (accumulate || k > 0) ? 1u : 0u);
-    }
+    umma_tiles_rt<AMAJ, BMAJ>(d_tmem, M, N, a_saddr, a_rows, a_o0, 0, b_saddr, b_rows, b_o0, 0, K, accumulate);
 }
 
 // fp32 scratch matrices of the triangular inverse: [64][64], columns XOR-swizzled by the row.

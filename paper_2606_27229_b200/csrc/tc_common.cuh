@@ -15,15 +15,16 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-// Optional per-phase cycle counters (build with -DCARVE_PROFILE; block 0, thread 0 = the MMA-issuing thread).
+// Optional per-phase cycle counters (build with -DCARVE_PROFILE; block 0: thread 0 = the MMA-issuing, K-side
+// thread in slots 0.., thread 64 = a Q-side thread in slots 20..).
 #ifdef CARVE_PROFILE
 #define PROF_DECL(name) static __device__ unsigned long long name[40];
 #define PROF_INIT() long long prof_t_ = clock64();
-#define PROF(name, i)                                        \
-    if (blockIdx.x == 0 && threadIdx.x == 0) {               \
-        const long long prof_n_ = clock64();                 \
-        name[i] += (unsigned long long)(prof_n_ - prof_t_);  \
-        prof_t_ = prof_n_;                                   \
+#define PROF(name, i)                                                              \
+    if (blockIdx.x == 0 && (threadIdx.x == 0 || threadIdx.x == 64)) {              \
+        const long long prof_n_ = clock64();                                       \
+        name[(threadIdx.x ? 20 : 0) + i] += (unsigned long long)(prof_n_ - prof_t_); \
+        prof_t_ = prof_n_;                                                         \
     }
 #else
 #define PROF_DECL(name)
@@ -224,20 +225,31 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar)
 // Which operand view an MMA uses.
 enum : int { KMAJ = 0, MNMAJ = 1 };
 
+// Descriptor of the next K = 16 slice, given the descriptor of the slice that starts at K index `k` (relative
+// to the tile): K-major operands advance 32 bytes inside a 64-column block and jump to the next block
+// (rows*128 bytes further) after four slices; MN-major operands advance two 8-row groups (2048 bytes).
+template <int MAJ>
+__device__ __forceinline__ uint64_t desc_next(uint64_t d, int rows, int k)
+{
+    if (MAJ == 0) return d + ((((k + 16) & 63) == 0) ? (uint64_t)(rows * 8 - 6) : 2ull);
+    return d + 128ull;
+}
+
 // Full product over K (multiple of 16) from two row tiles.  For a K-major operand `o0` is its first
 // MN row and K runs over columns from `k0`; for an MN-major operand `o0` is its first MN column and
-// K runs over rows from `k0`.
-template <int M, int N, int AMAJ, int BMAJ>
-__device__ __forceinline__ void umma_tiles(uint32_t d_tmem, uint32_t a_saddr, int a_rows, int a_o0, int a_k0,
-                                           uint32_t b_saddr, int b_rows, int b_o0, int b_k0, int K, bool accumulate)
+// K runs over rows from `k0`.  M = 128; N at run time.  Issued by ONE thread.
+template <int AMAJ, int BMAJ>
+__device__ __forceinline__ void umma_tiles_rt(uint32_t d_tmem, int M, int N, uint32_t a_saddr, int a_rows, int a_o0,
+                                              int a_k0, uint32_t b_saddr, int b_rows, int b_o0, int b_k0, int K,
+                                              bool accumulate)
 {
-    constexpr uint32_t idesc = umma_idesc(M, N, AMAJ, BMAJ);
+    const uint32_t idesc = umma_idesc(M, N, AMAJ, BMAJ);
+    uint64_t ad = AMAJ == KMAJ ? desc_kmajor(a_saddr, a_rows, a_o0, a_k0) : desc_mnmajor(a_saddr, a_rows, a_o0, a_k0);
+    uint64_t bd = BMAJ == KMAJ ? desc_kmajor(b_saddr, b_rows, b_o0, b_k0) : desc_mnmajor(b_saddr, b_rows, b_o0, b_k0);
     for (int k = 0; k < K; k += 16) {
-        const uint64_t ad = AMAJ == KMAJ ? desc_kmajor(a_saddr, a_rows, a_o0, a_k0 + k)
-                                         : desc_mnmajor(a_saddr, a_rows, a_o0, a_k0 + k);
-        const uint64_t bd = BMAJ == KMAJ ? desc_kmajor(b_saddr, b_rows, b_o0, b_k0 + k)
-                                         : desc_mnmajor(b_saddr, b_rows, b_o0, b_k0 + k);
         umma(d_tmem, ad, bd, idesc, (accumulate || k > 0) ? 1u : 0u);
+        ad = desc_next<AMAJ>(ad, a_rows, a_k0 + k);
+        bd = desc_next<BMAJ>(bd, b_rows, b_k0 + k);
     }
 }
 
