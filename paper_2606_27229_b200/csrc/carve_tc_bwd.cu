@@ -83,7 +83,7 @@ struct BMisc {
     float extra[128];     // column sums of S . dS: d log gamma carried in from the later chunks
     float rn[128];        // 1/|k|, 1/|q| of the chunk's tokens
     float beta[64];
-    float dbp[2][64];     // dbeta partial sums of the two column halves
+    float dbp[4][64];     // dbeta partial sums of the column parts
     float pre[4][128];    // gamma_a(b)/gamma_{-1}: product of etot[b'] over b' < b
     union {               // thread j turns its four column-sum partials into suf[.][j]: same addresses, no hazard
         float colp[4][128];   // column-sum partials per lane quadrant
@@ -180,12 +180,14 @@ __device__ __forceinline__ void warp_colsum(float (&v)[N], int lane)
         tc_fence_after();                   \
     } while (0)
 
-template <int D>
-__global__ void __launch_bounds__(NT, 1)
+// NP = column parts per tile row = warpgroups per CTA (threads = 128 NP): 32 columns per thread.
+template <int D, int NP>
+__global__ void __launch_bounds__(128 * NP, 1)
 carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, const __grid_constant__ CUtensorMap mk,
                     const __grid_constant__ CUtensorMap mq)
 {
-    constexpr int HK = D / 2;                      // columns per warpgroup half
+    constexpr int NTH = 128 * NP;
+    constexpr int HK = D / NP;                     // columns per warpgroup ("half" = part index 0..NP-1)
     constexpr uint32_t TB = tile_bytes(64, D);     // one [64][D] tile
     constexpr uint32_t SBb = tile_bytes(D, D);     // one state tile
     extern __shared__ uint8_t smem_raw[];
@@ -219,7 +221,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         tma_prefetch_desc(&mdO); tma_prefetch_desc(&mk); tma_prefetch_desc(&mq);
     }
     if (warp == 0) tmem_alloc(&mi.tmem_base, TM_COLS);
-    for (int i = tid; i < 32 * D; i += NT) {
+    for (int i = tid; i < 32 * D; i += NTH) {
         const int ii = i / D, n = i % D;
         float vc = 0.f, uc = 0.f;
         if (ii < r) { vc = __ldg(a.Vb + (size_t)n * r + ii); uc = __ldg(a.Ub + (size_t)ii * D + n); }
@@ -227,7 +229,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.VcT + tile_off(32, ii, n)) = __float2bfloat16_rn(vc);
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Ucat + tile_off(32, ii, n)) = __float2bfloat16_rn(uc);
     }
-    for (int i = tid; i < 64 * 192; i += NT) {
+    for (int i = tid; i < 64 * 192; i += NTH) {
         const int tt_ = i / 192, k = i % 192;
         const bool one = k < 64 ? (k > tt_) : k < 128 ? (k - 64 >= tt_) : (k - 128 < tt_);
         *reinterpret_cast<uint16_t*>(sm + Lo.TRI + tile_off(64, tt_, k)) = one ? 0x3F80u : 0u;
@@ -310,7 +312,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         }
         {
             const float* et = reinterpret_cast<const float*>(rc + Rc.etot);
-            for (int i = tid; i < 4 * D; i += NT) mi.etot[i / D][i % D] = __ldg(et + i);
+            for (int i = tid; i < 4 * D; i += NTH) mi.etot[i / D][i % D] = __ldg(et + i);
             if (tid < 128) mi.rn[tid] = __ldg(reinterpret_cast<const float*>(rc + Rc.rn) + tid);
             if (tid < 64) mi.beta[tid] = __ldg(reinterpret_cast<const float*>(rc + Rc.beta) + tid);
             if (tid >= 128 && tid < 128 + D) {
@@ -430,26 +432,33 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             umma_commit(&mi.bar_mma);
         }
         if (!krole && half == 0 && live)
-            a.dbeta[(tok0 + t) * a.H + h] = __float2bfloat16_rn(mi.dbp[0][t] + mi.dbp[1][t]);
+        {
+            float sdb = 0.f;
+#pragma unroll
+            for (int pp = 0; pp < NP; ++pp) sdb += mi.dbp[pp][t];
+            a.dbeta[(tok0 + t) * a.H + h] = __float2bfloat16_rn(sdb);
+        }
         WAIT_MMA();
         if (tid == 0) {  // DRO and U are dead
             mbar_expect_tx(&mi.bar_g4b, 2 * TB);
             bulk_g2s(sm + Lo.S[2], rc + Rc.KQo, 2 * TB, &mi.bar_g4b);
         }
         {   // masked [dA;dP] -> bf16 tile DAP (S[4], over U)
-            uint32_t v[32];
-            tmem_ld32(tmem + BM_DAP + lane_base + 32 * half, v);
+            constexpr int DW = 64 / NP;   // columns of the 64-wide block handled by this thread
+            uint32_t v[DW];
+            if constexpr (DW == 32) tmem_ld32(tmem + BM_DAP + lane_base + DW * half, v);
+            else tmem_ld16(tmem + BM_DAP + lane_base + DW * half, v);
             tmem_wait_ld();
 #pragma unroll
-            for (int ch = 0; ch < 4; ++ch) {
+            for (int ch = 0; ch < DW / 8; ++ch) {
                 float f8[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    const int s = 32 * half + 8 * ch + e;
+                    const int s = DW * half + 8 * ch + e;
                     const bool keep = live && (krole ? s < t : s <= t);
                     f8[e] = keep ? (krole ? __uint_as_float(v[8 * ch + e]) : a.scale * __uint_as_float(v[8 * ch + e])) : 0.f;
                 }
-                sts128(sm + Lo.S[4] + tile_chunk_off(128, row, 4 * half + ch), pack8(f8));
+                sts128(sm + Lo.S[4] + tile_chunk_off(128, row, (DW / 8) * half + ch), pack8(f8));
             }
         }
         PROF(g_prof_bwd, 3);
@@ -494,7 +503,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mi.suf[3][tid] = e3; mi.suf[2][tid] = e2 * e3; mi.suf[1][tid] = e1 * e2 * e3; mi.suf[0][tid] = e0 * e1 * e2 * e3;
         }
         {
-            constexpr int NCW = D / 8, NTW = NCW / 8;
+            constexpr int NCW = D / (4 * NP), NTW = NCW / 8;   // key channels per warp, n-tiles
             const int g = lane >> 2, l4 = lane & 3, cw = NCW * warp;
             const int lrow = (lane & 7) + ((lane >> 3) & 1) * 8;
             const int lchk = NTW == 2 ? (lane >> 4) : 0;
@@ -805,7 +814,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 for (int i = 0; i < 4; ++i) {
                     const bool is_b = i < rc8, is_w = i >= rc8 && i < 2 * rc8;
                     if (half == 0) sts128(sm + Lo.S[1] + tile_chunk_off(128, t, i), is_b ? t4[i] : z4);
-                    else sts128(sm + Lo.S[1] + tile_chunk_off(128, 64 + t, i), is_w ? t4[i] : z4);
+                    else if (half == 1) sts128(sm + Lo.S[1] + tile_chunk_off(128, 64 + t, i), is_w ? t4[i] : z4);
                 }
             }
         }
@@ -1050,11 +1059,12 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
     t.dbeta = static_cast<__nv_bfloat16*>(a.dbeta); t.dS0 = a.dS0;
     t.part = reinterpret_cast<float*>(ws + w.part); t.part_stride = w.part_stride;
     const size_t smem = BLayout(D).total;
-    auto kern = carve_bwd_tc_kernel<D>;
+    constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
+    auto kern = carve_bwd_tc_kernel<D, NP>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int chains = a.B * a.H, nchunks = a.T / LCc;
-    kern<<<chains, tcp::NT, smem, st>>>(t, mdO, mk, mq);
+    kern<<<chains, 128 * NP, smem, st>>>(t, mdO, mk, mq);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     float* partAT = reinterpret_cast<float*>(ws + w.partAT);
     carve_bwd_tc_epilogue_kernel<D><<<chains * nchunks, 256, 0, st>>>(
