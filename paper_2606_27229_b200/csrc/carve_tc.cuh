@@ -100,6 +100,11 @@ struct Rec {
     }
 };
 
+// Byte offset of 16-byte piece `cc` of row `row` in a row-private record array ([64 rows][d] bf16, only ever
+// read by the thread that owns the row): piece-major, so a warp (32 consecutive rows, one piece) moves 512
+// contiguous bytes both when the forward stores it and when the reverse kernel loads it.
+__host__ __device__ __forceinline__ uint32_t rp_off(int row, int cc) { return (uint32_t)((cc * 64 + row) * 16); }
+
 // misc area (floats unless noted)
 struct Misc {
     float eA[128], tau[128];    // exp(A_h), tau_h

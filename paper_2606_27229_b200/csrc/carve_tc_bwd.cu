@@ -332,7 +332,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         if (!krole && live) {
 #pragma unroll
             for (int i = 0; i < HK / 8; ++i) {
-                const uint32_t off = tile_chunk_off(64, t, half * (HK / 8) + i);
+                const uint32_t off = rp_off(t, half * (HK / 8) + i);
                 e4[i] = ldg128(rc + Rc.E + off);
                 x4[i] = ldg128(rc + Rc.VWX + off);
                 w4[i] = ldg128(rc + Rc.W + off);
@@ -689,8 +689,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         for (int ch = 0; ch < 2; ++ch) {
                             const int i = s / 8 + ch, cc = half * (HK / 8) + i, j0 = 8 * cc;
                             float fp[8], ic[8], pk[8], pc[8], k0[8], c8[8], o[8], xa[8], zz[8];
-                            unpack8(bstart ? ones4 : lds128(sm + Lo.FI + tile_chunk_off(64, t - 1, cc)), fp);
-                            unpack8(lds128(sm + Lo.FI + TB + tile_chunk_off(64, t, cc)), ic);
+                            unpack8(bstart ? ones4 : lds128(sm + Lo.FI + rp_off(t - 1, cc)), fp);
+                            unpack8(lds128(sm + Lo.FI + TB + rp_off(t, cc)), ic);
                             unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, t, cc)), pk);
                             unpack8(lds128(sm + Lo.S[4] + tile_chunk_off(64, t, cc)), pc);
                             unpack8(lds128(sm + Lo.S[5] + tile_chunk_off(64, t, cc)), k0);
@@ -726,7 +726,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         for (int ch = 0; ch < 2; ++ch) {
                             const int i = s / 8 + ch, cc = half * (HK / 8) + i, j0 = 8 * cc;
                             float fq[8], pq[8], q0[8], xq[8];
-                            unpack8(lds128(sm + Lo.FI + tile_chunk_off(64, t, cc)), fq);
+                            unpack8(lds128(sm + Lo.FI + rp_off(t, cc)), fq);
                             unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc)), pq);
                             unpack8(lds128(sm + Lo.S[6] + tile_chunk_off(64, t, cc)), q0);
                             float pre[8];
@@ -778,7 +778,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         for (int ch = 0; ch < 4; ++ch) {
                             const int i = s / 8 + ch, cc = half * (HK / 8) + i;
                             float bb[8], dp[8], dla[8], dbp[8];
-                            unpack8(lds128(sm + Lo.FI + tile_chunk_off(64, t, cc)), bb);
+                            unpack8(lds128(sm + Lo.FI + rp_off(t, cc)), bb);
                             unpack8(lds128(sm + Lo.S[0] + tile_chunk_off(64, t, cc)), dp);
 #pragma unroll
                             for (int e = 0; e < 8; ++e) {

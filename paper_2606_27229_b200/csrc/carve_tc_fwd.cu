@@ -433,7 +433,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         }
                         sts128(sm + Lo.Y0 + off, pack8(hi));
                         sts128(sm + Lo.Y1 + off, pack8(lo));
-                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.Bg + off) = pack8(bg);
+                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.Bg + rp_off(t, cc)) = pack8(bg);
                     }
                 }
             } else {
@@ -454,10 +454,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         }
                         sts128(sm + Lo.V + off, pack8(fv));
                         if (rc) {
-                            *reinterpret_cast<uint4*>(rc + Rc.W + off) = pack8(fw);
+                            *reinterpret_cast<uint4*>(rc + Rc.W + rp_off(t, cc)) = pack8(fw);
 #pragma unroll
                             for (int e = 0; e < 8; ++e) fv[e] *= 1.f - fw[e];
-                            *reinterpret_cast<uint4*>(rc + Rc.VWX + off) = pack8(fv);
+                            *reinterpret_cast<uint4*>(rc + Rc.VWX + rp_off(t, cc)) = pack8(fv);
                         }
                     }
                 }
@@ -543,7 +543,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                             sts128(ver_row(bn, false, tn, cc), pack8(kv));
                             if (rc) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = pack8(kv);
                         }
-                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.FQ + tile_chunk_off(64, t, cc)) = pack8(Fp);
+                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.FQ + rp_off(t, cc)) = pack8(Fp);
 #pragma unroll
                         for (int jb = 3; jb >= 0; --jb) {
                             if (jb <= blk) {
@@ -612,7 +612,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         if (rc) {
                             *reinterpret_cast<uint4*>(rc + Rc.CC + off) = pack8(o1);
                             *reinterpret_cast<uint4*>(rc + Rc.KT + off) = pack8(o2);
-                            *reinterpret_cast<uint4*>(rc + Rc.IC + off) = pack8(ic);
+                            *reinterpret_cast<uint4*>(rc + Rc.IC + rp_off(t, cc)) = pack8(ic);
                         }
                     }
                 }
@@ -774,7 +774,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         *reinterpret_cast<uint4*>(rc + Rc.U + off) = pack8(f);
 #pragma unroll
                         for (int e = 0; e < 8; ++e) f[e] *= rbt;  // e_t = u_t / beta_t (Alg. 2 step 7)
-                        *reinterpret_cast<uint4*>(rc + Rc.E + off) = pack8(f);
+                        *reinterpret_cast<uint4*>(rc + Rc.E + rp_off(t, cc)) = pack8(f);
                     }
                 }
             }
