@@ -89,7 +89,7 @@ struct BMisc {
         float colp[4][128];   // column-sum partials per lane quadrant
         float suf[4][128];    // gamma_L/gamma_a(b): product of etot[b'] over b' >= b
     };
-    uint64_t bar_mma, bar_g1, bar_g3, bar_sb, bar_g4a, bar_g4b, bar_g5, bar_g8, bar_fi, bar_bg;
+    uint64_t bar_mma, bar_g1, bar_g3, bar_sb, bar_g4a, bar_g4b, bar_g5, bar_g8, bar_fi, bar_bg, bar_pt;
     uint32_t tmem_base;
 };
 static_assert(sizeof(BMisc) <= 9216, "misc area too small");
@@ -216,7 +216,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     if (tid == 0) {
         mbar_init(&mi.bar_mma, 1); mbar_init(&mi.bar_g1, 1); mbar_init(&mi.bar_g3, 1); mbar_init(&mi.bar_sb, 1);
         mbar_init(&mi.bar_g4a, 1); mbar_init(&mi.bar_g4b, 1); mbar_init(&mi.bar_g5, 1); mbar_init(&mi.bar_g8, 1);
-        mbar_init(&mi.bar_fi, 1); mbar_init(&mi.bar_bg, 1);
+        mbar_init(&mi.bar_fi, 1); mbar_init(&mi.bar_bg, 1); mbar_init(&mi.bar_pt, 1);
         mbar_fence_init();
         tma_prefetch_desc(&mdO); tma_prefetch_desc(&mk); tma_prefetch_desc(&mq);
     }
@@ -287,6 +287,26 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
 
     finalize(false, false);
 
+    // L1 / L3 operands of chunk c2 (thread 0): issued at the top for the first chunk, afterwards as soon as the
+    // previous chunk's last readers of the slots are done, so that the fetch hides behind its last phases.
+    auto issue_l1 = [&](int c2) {
+        const uint8_t* r2 = rec_chain + (size_t)c2 * Rc.total;
+        mbar_expect_tx(&mi.bar_g1, 2 * TB + (uint32_t)LCc * D * 2u + 16u * D + 512u + 256u);
+        for (int b2 = 0; b2 < 4; ++b2) bulk_g2s(mi.etot[b2], r2 + Rc.etot + b2 * 4 * D, 4u * D, &mi.bar_g1);
+        bulk_g2s(mi.rn, r2 + Rc.rn, 512, &mi.bar_g1);
+        bulk_g2s(mi.beta, r2 + Rc.beta, 256, &mi.bar_g1);
+        bulk_g2s(sm + Lo.S[0], r2 + Rc.KT, TB, &mi.bar_g1);
+        bulk_g2s(sm + Lo.S[4], r2 + Rc.U, TB, &mi.bar_g1);
+        for (int cb = 0; cb < D / 64; ++cb)
+            tma_load_3d(sm + Lo.S[2] + cb * 16384 + 8192, &mdO, &mi.bar_g1, cb * 64, h, b * a.T + c2 * LCc);
+        mbar_expect_tx(&mi.bar_g3, 2 * TB);
+        bulk_g2s(sm + Lo.S[5], r2 + Rc.K0, TB, &mi.bar_g3);
+        bulk_g2s(sm + Lo.S[6], r2 + Rc.Q0, TB, &mi.bar_g3);
+    };
+    auto issue_pt = [&](int c2) {
+        mbar_expect_tx(&mi.bar_pt, 16384);
+        bulk_g2s(sm + Lo.S[1], rec_chain + (size_t)c2 * Rc.total + Rc.PT, 16384, &mi.bar_pt);
+    };
     bool first = true;
     PROF_INIT();
     for (int it = 0, c = nchunks - 1; c >= 0; --c, ++it) {
@@ -300,21 +320,9 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 mbar_expect_tx(&mi.bar_sb, SBb);
                 bulk_g2s(sm + Lo.SBq, rc + Rc.SB, SBb, &mi.bar_sb);
             }
-            mbar_expect_tx(&mi.bar_g1, 2 * TB + 16384 + (uint32_t)LCc * D * 2u);
-            bulk_g2s(sm + Lo.S[0], rc + Rc.KT, TB, &mi.bar_g1);
-            bulk_g2s(sm + Lo.S[1], rc + Rc.PT, 16384, &mi.bar_g1);
-            bulk_g2s(sm + Lo.S[4], rc + Rc.U, TB, &mi.bar_g1);
-            for (int cb = 0; cb < D / 64; ++cb)
-                tma_load_3d(sm + Lo.S[2] + cb * 16384 + 8192, &mdO, &mi.bar_g1, cb * 64, h, trow);
-            mbar_expect_tx(&mi.bar_g3, 2 * TB);
-            bulk_g2s(sm + Lo.S[5], rc + Rc.K0, TB, &mi.bar_g3);
-            bulk_g2s(sm + Lo.S[6], rc + Rc.Q0, TB, &mi.bar_g3);
+            if (it == 0) { issue_l1(c); issue_pt(c); }
         }
         {
-            const float* et = reinterpret_cast<const float*>(rc + Rc.etot);
-            for (int i = tid; i < 4 * D; i += NTH) mi.etot[i / D][i % D] = __ldg(et + i);
-            if (tid < 128) mi.rn[tid] = __ldg(reinterpret_cast<const float*>(rc + Rc.rn) + tid);
-            if (tid < 64) mi.beta[tid] = __ldg(reinterpret_cast<const float*>(rc + Rc.beta) + tid);
             if (tid >= 128 && tid < 128 + D) {
                 const int j = tid - 128;
                 float g = 1.f;
@@ -341,6 +349,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         // ---- L1: dU = Ktil dS'^T + (scale P)^T dO -> BM_A rows 0..63;  dKtil = U dS' -> BM_KT rows 0..63
         if (tid == 0) {
             mbar_wait(&mi.bar_g1, ph);
+            mbar_wait(&mi.bar_pt, ph);
             tc_fence_after();
             mma_k<KMAJ, KMAJ>(tmem + BM_A, D, sb + Lo.S[0], 64, 0, 0, sb + Lo.DSB, D, 0, 0, D, false);
             mma_k<MNMAJ, MNMAJ>(tmem + BM_A, D, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[2], 128, 0, 64, LCc, true);
@@ -868,6 +877,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             umma_commit(&mi.bar_mma);
         }
         WAIT_MMA();
+        if (tid == 0 && c > 0) issue_l1(c - 1);   // DZ, DZQ, GW, G^T, q are dead
         if (!krole && warp_active) {
             __nv_bfloat16* gdq = a.dq + ((tok0 + t) * a.H + h) * D;
 #pragma unroll
@@ -907,9 +917,10 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             umma_commit(&mi.bar_mma);
         }
         WAIT_MMA();
-        if (tid == 0 && c > 0) {   // SBq is free: the state entering the next chunk to be processed
+        if (tid == 0 && c > 0) {   // SBq and the dG tile are free: the state entering the next chunk, its [P;T]
             mbar_expect_tx(&mi.bar_sb, SBb);
             bulk_g2s(sm + Lo.SBq, rc - Rc.total + Rc.SB, SBb, &mi.bar_sb);
+            issue_pt(c - 1);
         }
         PROF(g_prof_bwd, 10);
         // ---- L10: the adjoint of the state entering the chunk
