@@ -69,14 +69,14 @@ cudaError_t simt_bwd_launch(const Args& a, int dtype, float* dA, float* dtau, fl
 
 // Tensor-core path (carve_tc_fwd.cu, carve_tc_bwd.cu): bf16 tokens, dk == dv in {64,128}, r <= 16.
 bool tc_fwd_supported(const carve_params_t& p);
-bool tc_bwd_supported(const carve_params_t& p);   // additionally L <= 64
+bool tc_bwd_supported(const carve_params_t& p);
 size_t tc_state_tile_bytes(const carve_params_t& p);
 size_t tc_record_bytes(const carve_params_t& p);
 
 // Workspace of the tensor path (byte offsets): chunk records, final-state tiles, per-chain weight-gradient
 // partials (layout of part_stride_of) and per-chunk dA/dtau partials.
 struct TcWsLayout {
-    size_t rec, sfin, part, partAT, total_bytes;
+    size_t rec, sfin, part, partAT, dgs, total_bytes;
     int part_stride;
 };
 inline TcWsLayout tc_ws_layout(const carve_params_t& p)
@@ -92,6 +92,7 @@ inline TcWsLayout tc_ws_layout(const carve_params_t& p)
     w.part_stride = part_stride_of(p.dk, p.dv, p.r);
     w.part = take(chains * (size_t)w.part_stride * sizeof(float));
     w.partAT = take(chains * nchunks * 2 * p.dk * sizeof(float));
+    w.dgs = take(chains * (size_t)p.dk * 32 * sizeof(float));
     w.total_bytes = off;
     return w;
 }

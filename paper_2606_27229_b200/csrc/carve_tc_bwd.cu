@@ -47,6 +47,7 @@ struct BwdArgs {
     float* dS0;
     float* part;
     int part_stride;
+    float* dgs;   // [chains][dk][32] dG^T of the later solve chunk of a gate chunk (L = 128)
 };
 
 // TMEM column map of the reverse kernel.
@@ -204,7 +205,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
     const int chain = blockIdx.x, b = chain / a.H, h = chain % a.H;
     const int LCc = a.L < LC ? a.L : LC;
-    const int nchunks = a.T / LCc, nb = LCc >> 4;
+    const int nchunks = a.T / LCc, nb = LCc >> 4, gate_every = a.L / LCc;
     const bool warp_active = (q & 1) * 32 < LCc;   // this warp holds at least one live token row
     const bool live = t < LCc;
     const bool srow = row < D;                     // this thread owns a row of the state adjoint
@@ -307,13 +308,14 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         mbar_expect_tx(&mi.bar_pt, 16384);
         bulk_g2s(sm + Lo.S[1], rec_chain + (size_t)c2 * Rc.total + Rc.PT, 16384, &mi.bar_pt);
     };
-    bool first = true;
+    bool first = true, first_glue = true;
     PROF_INIT();
     for (int it = 0, c = nchunks - 1; c >= 0; --c, ++it) {
         const uint32_t ph = (uint32_t)it & 1u;
         const uint8_t* rc = rec_chain + (size_t)c * Rc.total;
         const size_t tok0 = (size_t)b * a.T + (size_t)c * LCc;
         const int trow = b * a.T + c * LCc;  // TMA row coordinate of the chunk's first token
+        const bool gate_start = (c % gate_every) == 0;   // the fold G of this solve chunk read the state entering it
         // ---- loads of the chunk: L1 operands, state, chunk-anchored rows; small per-chunk vectors
         if (tid == 0) {
             if (it == 0) {   // later chunks: issued as soon as the previous chunk's last reader of SBq is done
@@ -900,23 +902,44 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             uint32_t v[32];
             tmem_ld32(tmem + BM_DAP + 32 + lane_base, v);
             tmem_wait_ld();
+            if (gate_every > 1) {   // L = 128: both solve chunks of a gate chunk share G; their dG add up (same thread, same row)
+                float4* st = reinterpret_cast<float4*>(a.dgs + ((size_t)chain * D + row) * 32);
 #pragma unroll
-            for (int ch = 0; ch < 4; ++ch) {
-                float f8[8];
+                for (int e = 0; e < 8; ++e) {
+                    if (!gate_start) {
+                        st[e] = make_float4(__uint_as_float(v[4 * e]), __uint_as_float(v[4 * e + 1]), __uint_as_float(v[4 * e + 2]),
+                                            __uint_as_float(v[4 * e + 3]));
+                    } else {
+                        const float4 o = st[e];
+                        v[4 * e] = __float_as_uint(__uint_as_float(v[4 * e]) + o.x);
+                        v[4 * e + 1] = __float_as_uint(__uint_as_float(v[4 * e + 1]) + o.y);
+                        v[4 * e + 2] = __float_as_uint(__uint_as_float(v[4 * e + 2]) + o.z);
+                        v[4 * e + 3] = __float_as_uint(__uint_as_float(v[4 * e + 3]) + o.w);
+                    }
+                }
+            }
+            if (gate_start) {   // (otherwise S[1] is already being refilled for the next chunk)
 #pragma unroll
-                for (int e = 0; e < 8; ++e) f8[e] = __uint_as_float(v[8 * ch + e]);
-                sts128(sm + Lo.S[1] + tile_chunk_off(D, row, ch), pack8(f8));
+                for (int ch = 0; ch < 4; ++ch) {
+                    float f8[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) f8[e] = __uint_as_float(v[8 * ch + e]);
+                    sts128(sm + Lo.S[1] + tile_chunk_off(D, row, ch), pack8(f8));
+                }
             }
         }
         PROF(g_prof_bwd, 9);
         // ---- L9: fold glue: dS += [Ub;Uw]^T dG;  d[Ub;Uw]^T += S dG^T -> BM_WU
-        PHASE_SYNC();
-        if (tid == 0) {
-            mma_k<MNMAJ, KMAJ>(tmem + BM_DS, D, sb + Lo.Ucat, 32, 0, 0, sb + Lo.S[1], D, 0, 0, R2, true);
-            mma_k<KMAJ, MNMAJ>(tmem + BM_WU, 32, sb + Lo.SBq, D, 0, 0, sb + Lo.S[1], D, 0, 0, D, !first);
-            umma_commit(&mi.bar_mma);
+        if (gate_start) {
+            PHASE_SYNC();
+            if (tid == 0) {
+                mma_k<MNMAJ, KMAJ>(tmem + BM_DS, D, sb + Lo.Ucat, 32, 0, 0, sb + Lo.S[1], D, 0, 0, R2, true);
+                mma_k<KMAJ, MNMAJ>(tmem + BM_WU, 32, sb + Lo.SBq, D, 0, 0, sb + Lo.S[1], D, 0, 0, D, !first_glue);
+                umma_commit(&mi.bar_mma);
+            }
+            WAIT_MMA();
+            first_glue = false;
         }
-        WAIT_MMA();
         if (tid == 0 && c > 0) {   // SBq and the dG tile are free: the state entering the next chunk, its [P;T]
             mbar_expect_tx(&mi.bar_sb, SBb);
             bulk_g2s(sm + Lo.SBq, rc - Rc.total + Rc.SB, SBb, &mi.bar_sb);
@@ -1069,6 +1092,7 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
     t.dbx = static_cast<__nv_bfloat16*>(a.dbx); t.dwx = static_cast<__nv_bfloat16*>(a.dwx);
     t.dbeta = static_cast<__nv_bfloat16*>(a.dbeta); t.dS0 = a.dS0;
     t.part = reinterpret_cast<float*>(ws + w.part); t.part_stride = w.part_stride;
+    t.dgs = reinterpret_cast<float*>(ws + w.dgs);
     const size_t smem = BLayout(D).total;
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
     auto kern = carve_bwd_tc_kernel<D, NP>;
@@ -1099,7 +1123,7 @@ extern "C" void carve_debug_prof_bwd(unsigned long long* out)
 }
 #endif
 
-bool tc_bwd_supported(const carve_params_t& p) { return tc_fwd_supported(p) && p.L <= 64; }
+bool tc_bwd_supported(const carve_params_t& p) { return tc_fwd_supported(p); }
 
 cudaError_t tc_bwd_launch(const Args& a, uint8_t* ws, const TcWsLayout& w, float* dA, float* dtau, float* dUb, float* dUw,
                           float* dVb, float* dVw, cudaStream_t st)

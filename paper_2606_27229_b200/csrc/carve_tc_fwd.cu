@@ -344,6 +344,11 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     }
                 }
             }
+        } else if (rc && half == 0 && q * 32 < DK) {
+            // second solve chunk of a gate chunk (L = 128): same G, copied into this chunk's record
+            for (int c0 = 0; c0 < R2; c0 += 8)
+                *reinterpret_cast<uint4*>(rc + Rc.GT + tile_chunk_off(DK, row, c0 / 8)) =
+                    lds128(sm + Lo.Vcat + tile_chunk_off(DM, row, (32 + c0) / 8));
         }
         PROF(g_prof_fwd, 2);
         // ---- P2: Z = [k;q] G^T -> TM_X2[32, 32+R2)

@@ -157,7 +157,7 @@ def test_host_entry_point_matches_device_entry_point(oracle):
 
 # ---- both kernel families against the oracle on the same bf16 case --------------------------------
 @pytest.mark.parametrize("path", [carve.CARVE_PATH_SIMT, carve.CARVE_PATH_TENSOR])
-@pytest.mark.parametrize("dk,r,L", [(64, 8, 64), (128, 16, 64), (128, 16, 32), (64, 16, 16)])
+@pytest.mark.parametrize("dk,r,L", [(64, 8, 64), (128, 16, 64), (128, 16, 32), (64, 16, 16), (128, 16, 128), (64, 8, 128)])
 def test_kernel_families_bf16(oracle, path, dk, r, L):
     """Several chunks, several 16-token anchor blocks, nonzero S0, active content gates, A and tau present."""
     cfg = synth.Config("t", B=2, H=2, T=256, L=L, dk=dk, dv=dk, r=r, dtype="bf16", wstd=0.1, s0_std=0.05, seed=dk + L)
@@ -168,9 +168,10 @@ def test_kernel_families_bf16(oracle, path, dk, r, L):
 
 
 def test_tensor_path_refuses_what_it_does_not_cover(oracle):
-    """No silent substitution: an explicit CARVE_PATH_TENSOR request for L = 128 training or fp32 is an error."""
-    for kw in (dict(L=128, dtype="bf16"), dict(L=64, dtype="f32")):
-        cfg = synth.Config("t", B=1, H=1, T=128, dk=64, dv=64, r=8, seed=1, **kw)
+    """No silent substitution: an explicit CARVE_PATH_TENSOR request for fp32 tokens, d_k != d_v or r = 32 is an error."""
+    for kw in (dict(dk=64, dv=64, r=8, dtype="f32"), dict(dk=64, dv=128, r=8, dtype="bf16"),
+               dict(dk=128, dv=128, r=32, dtype="bf16")):
+        cfg = synth.Config("t", B=1, H=1, T=128, L=64, seed=1, **kw)
         p = params_of(cfg, path=carve.CARVE_PATH_TENSOR)
         assert carve.carve_resolved_path(p, True) == -1
         assert carve.carve_workspace_bytes(p, True) == 0
