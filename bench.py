@@ -317,6 +317,13 @@ def run_ours(args):
         dom_ms = bwd_ms if dom == "bwd" else fwd_ms
         dom_bytes = alg[f"{dom}_bytes"]
         achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
+        traffic = None      # DRAM bytes of that call from the committed ncu capture (config 1, tensor path only)
+        tpath = os.path.join(ROOT, "profiles", "r1_tc_traffic.csv")
+        if cfg.name == synth.CFG1.name and not args.fwd_only and os.path.exists(tpath):
+            for ln in open(tpath).read().splitlines()[1:]:
+                f = ln.split(",")
+                if f[0] == f"carve_{dom}":
+                    traffic = int(f[2]) + int(f[3])
         t_hbm = (alg["fwd_bytes"] + alg["bwd_bytes"]) / (peaks["hbm_gbs"] * 1e9)
         t_tc = (alg["fwd_flops"] + alg["bwd_flops"]) / (peaks["bf16_tflops"] * 1e12)
         path = carve.carve_resolved_path(p, with_bwd)
@@ -329,8 +336,11 @@ def run_ours(args):
                                           (carve.carve_num_launches(p, True) if with_bwd else 0)),
             "kernel_path": {1: "simt-fp32", 2: "tensor-tcgen05"}.get(path, str(path)),
             "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
-            "roofline": {"bound": "hbm", "kernel": f"carve_{dom}", "achieved": achieved, "peak": peaks["hbm_gbs"],
-                         "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"], "traffic": None,
+            "roofline": {"bound": "hbm",
+                         "kernel": (f"carve_{dom} call" + (" (reverse kernel + chunk-local epilogue + 2 reductions)"
+                                                           if dom == "bwd" and path == 2 else "")),
+                         "achieved": achieved, "peak": peaks["hbm_gbs"],
+                         "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"], "traffic": traffic,
                          "peak_source": f"{peaks['source']} (MEASURED_PEAKS.json hbm_gbs)" if peaks["source"] == "measured"
                          else "fallback 6650 GB/s",
                          "algorithmic_bytes_per_launch": dom_bytes},
