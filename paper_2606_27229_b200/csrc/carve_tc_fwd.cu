@@ -524,26 +524,54 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     default: return sm + Lo.Y2 + tile_bytes(96, DK) + tile_chunk_off(32, (qrole ? 16 : 0) + tok - 48, cc);
                 }
             };
-            if (!krole) {
-                const float rnq = a.l2norm ? rsqrtf(sumsq(row) + a.eps) : 1.f;
+            // Both threads of a token (K-side lane t, Q-side lane 64+t) hold +-(lg_t - lg_a) of the same columns: each
+            // takes half of them and produces every decayed operand of the token for those columns.
+            {
+                const float rnq = a.l2norm ? rsqrtf(sumsq(64 + t) + a.eps) : 1.f;
+                const float rnk = a.l2norm ? rsqrtf(sumsq(t) + a.eps) : 1.f;
                 const int tn = t + 1;  // the key row that shares this token's retention (Kbar_{t+1} = k^_{t+1} gamma_t)
                 const bool has_next = tn < LCc;
                 const int bn = tn >> 4, krow = has_next ? tn : 0;
-                const float rnk = a.l2norm ? rsqrtf(sumsq(krow) + a.eps) : 1.f;
-                if (rc && live && half == 0) reinterpret_cast<float*>(rc + Rc.rn)[64 + t] = rnq;
+                const float rnkn = a.l2norm ? rsqrtf(sumsq(krow) + a.eps) : 1.f;
+                if (rc && live && half == 0) reinterpret_cast<float*>(rc + Rc.rn)[row] = krole ? rnk : rnq;
+                const int cc0 = half * (HK / 8) + (krole ? 0 : HK / 16);
 #pragma unroll 1
-                for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
+                for (int cc = cc0; cc < cc0 + HK / 16; ++cc) {
                     uint32_t v[8];
                     tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, v);
                     tmem_wait_ld();
                     if (live) {
                         float Fp[8], qv[8], kv[8], o[8];
+                        {   // column operand C_t, Ktil_t (own anchor), gamma_a/gamma_t >= 1
+                            float kt[8], o1[8], o2[8], ic[8], et[8], sf[8];
+                            unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, t, cc)), kt);
+                            *reinterpret_cast<float4*>(et) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc]);
+                            *reinterpret_cast<float4*>(et + 4) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc + 4]);
+                            *reinterpret_cast<float4*>(sf) = *reinterpret_cast<const float4*>(&mi.suf[blk][8 * cc]);
+                            *reinterpret_cast<float4*>(sf + 4) = *reinterpret_cast<const float4*>(&mi.suf[blk][8 * cc + 4]);
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) Fp[e] = __expf(__uint_as_float(v[e]));  // gamma_t / gamma_{a_blk}
+                            for (int e = 0; e < 8; ++e) {
+                                const float lgl = krole ? -__uint_as_float(v[e]) : __uint_as_float(v[e]);  // lg_t - lg_a <= 0
+                                Fp[e] = __expf(lgl);                              // gamma_t / gamma_{a_blk}
+                                const float cx = __expf(-lgl);                    // gamma_{a_blk} / gamma_t >= 1
+                                const float kh = kt[e] * rnk;
+                                ic[e] = cx;
+                                o1[e] = kh * cx;
+                                o2[e] = kh * ((cx * et[e]) * sf[e]);              // k^ gamma_L / gamma_t, every factor <= 1
+                            }
+                            const uint32_t off = tile_chunk_off(64, t, cc);
+                            sts128(sm + Lo.Y1 + off, pack8(o1));      // C_t
+                            sts128(sm + Lo.Ktil + off, pack8(o2));    // Ktil_t
+                            if (rc) {
+                                *reinterpret_cast<uint4*>(rc + Rc.CC + off) = pack8(o1);
+                                *reinterpret_cast<uint4*>(rc + Rc.KT + off) = pack8(o2);
+                                *reinterpret_cast<uint4*>(rc + Rc.IC + rp_off(t, cc)) = pack8(ic);
+                            }
+                        }
                         unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, 64 + t, cc)), qv);
                         unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, krow, cc)), kv);
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) { qv[e] *= rnq; kv[e] *= rnk; }
+                        for (int e = 0; e < 8; ++e) { qv[e] *= rnq; kv[e] *= rnkn; }
                         if (has_next && bn > blk) {  // first row of its block
                             sts128(ver_row(bn, false, tn, cc), pack8(kv));
                             if (rc) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = pack8(kv);
@@ -585,39 +613,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                                 *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, 0, cc)) = pack8(kv);
                                 *reinterpret_cast<uint4*>(rc + Rc.K0 + tile_chunk_off(64, 0, cc)) = pack8(kv);
                             }
-                        }
-                    }
-                }
-            } else {
-                const float rnk = a.l2norm ? rsqrtf(sumsq(row) + a.eps) : 1.f;
-                if (rc && live && half == 0) reinterpret_cast<float*>(rc + Rc.rn)[t] = rnk;
-#pragma unroll 1
-                for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
-                    uint32_t v[8];
-                    tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, v);
-                    tmem_wait_ld();
-                    if (live) {
-                        float kv[8], o1[8], o2[8], ic[8], et[8], sf[8];
-                        unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, t, cc)), kv);
-                        *reinterpret_cast<float4*>(et) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc]);
-                        *reinterpret_cast<float4*>(et + 4) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc + 4]);
-                        *reinterpret_cast<float4*>(sf) = *reinterpret_cast<const float4*>(&mi.suf[blk][8 * cc]);
-                        *reinterpret_cast<float4*>(sf + 4) = *reinterpret_cast<const float4*>(&mi.suf[blk][8 * cc + 4]);
-#pragma unroll
-                        for (int e = 0; e < 8; ++e) {
-                            const float cx = __expf(__uint_as_float(v[e]));   // gamma_{a_blk} / gamma_t >= 1
-                            const float kh = kv[e] * rnk;
-                            ic[e] = cx;
-                            o1[e] = kh * cx;
-                            o2[e] = kh * ((cx * et[e]) * sf[e]);              // k^ gamma_L / gamma_t, every factor <= 1
-                        }
-                        const uint32_t off = tile_chunk_off(64, t, cc);
-                        sts128(sm + Lo.Y1 + off, pack8(o1));      // C_t
-                        sts128(sm + Lo.Ktil + off, pack8(o2));    // Ktil_t
-                        if (rc) {
-                            *reinterpret_cast<uint4*>(rc + Rc.CC + off) = pack8(o1);
-                            *reinterpret_cast<uint4*>(rc + Rc.KT + off) = pack8(o2);
-                            *reinterpret_cast<uint4*>(rc + Rc.IC + rp_off(t, cc)) = pack8(ic);
                         }
                     }
                 }
