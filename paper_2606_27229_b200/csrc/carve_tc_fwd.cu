@@ -217,8 +217,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     for (int i = tid; i < DM * 64; i += NTH) {
         const int n = i / 64, c = i % 64;
         float v = 0.f;
-        if (c < r) { if (n < DK) v = __ldg(a.Vb + (size_t)n * r + c); }
-        else if (c < R2) { if (n < DV) v = __ldg(a.Vw + (size_t)n * r + (c - r)); }
+        // each gate half padded to 16 columns, so that the two up-projections are separate K = 16 slices
+        if (c < 16) { if (c < r && n < DK) v = __ldg(a.Vb + (size_t)n * r + c); }
+        else if (c < 32) { if (c - 16 < r && n < DV) v = __ldg(a.Vw + (size_t)n * r + (c - 16)); }
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Vcat + tile_off(DM, n, c)) = __float2bfloat16_rn(v);
     }
     for (int j = tid; j < DK; j += NTH) {
@@ -380,8 +381,13 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         const int col = c0 + 8 * k8;       // tt columns [col, col+8)
                         const uint4 w = pack8(f + 8 * k8);
                         const bool is_b = col < r;         // erase-gate half of the bottleneck
-                        sts128(sm + Lo.Y1 + tile_chunk_off(128, 64 + t, col / 8), is_b ? w : z4);
-                        sts128(sm + Lo.Y1 + tile_chunk_off(128, t, col / 8), is_b ? z4 : w);
+                        const int dst = is_b ? col / 8 : 2 + (col - r) / 8;   // [tt_b pad 16 | tt_w pad 16], both row halves
+                        sts128(sm + Lo.Y1 + tile_chunk_off(128, 64 + t, dst), w);
+                        sts128(sm + Lo.Y1 + tile_chunk_off(128, t, dst), w);
+                    }
+                    if (r < 16) {
+                        sts128(sm + Lo.Y1 + tile_chunk_off(128, 64 + t, 1), z4); sts128(sm + Lo.Y1 + tile_chunk_off(128, t, 1), z4);
+                        sts128(sm + Lo.Y1 + tile_chunk_off(128, 64 + t, 3), z4); sts128(sm + Lo.Y1 + tile_chunk_off(128, t, 3), z4);
                     }
                 }
             }
@@ -402,27 +408,31 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             }
         }
         PROF(g_prof_fwd, 4);
-        // ---- P4: [w_proj; b_proj] = Ablk Vcat^T -> TM_X1
+        // ---- P4: b_proj = [tt_b;tt_b] Vb^T -> TM_X1, w_proj = [tt_w;tt_w] Vw^T -> TM_X2 (both row halves get both)
         PHASE_SYNC();
         if (tid == 0) {
-            mma_rt<128, KMAJ, KMAJ>(tmem + TM_X1, DM, sb + Lo.Y1, 128, 0, sb + Lo.Vcat, DM, 0, R2, false);
+            umma_tiles_rt<KMAJ, KMAJ>(tmem + TM_X1, 128, DK, sb + Lo.Y1, 128, 0, 0, sb + Lo.Vcat, DM, 0, 0, 16, false);
+            umma_tiles_rt<KMAJ, KMAJ>(tmem + TM_X2, 128, DV, sb + Lo.Y1, 128, 0, 16, sb + Lo.Vcat, DM, 0, 16, 16, false);
             umma_commit(&mi.bar_mma);
         }
         mbar_wait(&mi.bar_fb, tma_ph);
         mbar_wait(&mi.bar_wv, tma_ph);
         WAIT_MMA();
         PROF(g_prof_fwd, 5);
-        // ---- P5: gates (8 columns per step; cc = 16-byte chunk index inside the row)
+        // ---- P5: gates (8 columns per step; cc = 16-byte chunk index inside the row).  Both threads of a token take
+        //      half of the part's columns and do the erase side (log a) and the write side (V' = w v) for them.
         if (warp_active) {
-            if (!krole) {
+            const int cc0 = half * (HK / 8) + (krole ? 0 : HK / 16);
 #pragma unroll 1
-                for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
-                    uint32_t pr[8];
-                    tmem_ld8(tmem + TM_X1 + lane_base + 8 * cc, pr);
-                    tmem_wait_ld();
-                    if (live) {
+            for (int cc = cc0; cc < cc0 + HK / 16; ++cc) {
+                uint32_t pr[8], pw[8];
+                tmem_ld8(tmem + TM_X1 + lane_base + 8 * cc, pr);
+                tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, pw);
+                tmem_wait_ld();
+                if (live) {
+                    const uint32_t off = tile_chunk_off(64, t, cc);
+                    {
                         float fb[8], ff[8], hi[8], lo[8], bg[8];
-                        const uint32_t off = tile_chunk_off(64, t, cc);
                         unpack8(lds128(sm + Lo.BX + off), fb);
                         unpack8(lds128(sm + Lo.F + off), ff);
 #pragma unroll
@@ -440,21 +450,13 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         sts128(sm + Lo.Y1 + off, pack8(lo));
                         if (rc) *reinterpret_cast<uint4*>(rc + Rc.Bg + rp_off(t, cc)) = pack8(bg);
                     }
-                }
-            } else {
-#pragma unroll 1
-                for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
-                    uint32_t pr[8];
-                    tmem_ld8(tmem + TM_X1 + lane_base + 8 * cc, pr);
-                    tmem_wait_ld();
-                    if (live) {
+                    {
                         float fw[8], fv[8];
-                        const uint32_t off = tile_chunk_off(64, t, cc);
                         unpack8(lds128(sm + Lo.WX + off), fw);
                         unpack8(lds128(sm + Lo.V + off), fv);
 #pragma unroll
                         for (int e = 0; e < 8; ++e) {
-                            fw[e] = sigmoid_fast(fw[e] + __uint_as_float(pr[e]));
+                            fw[e] = sigmoid_fast(fw[e] + __uint_as_float(pw[e]));
                             fv[e] *= fw[e];
                         }
                         sts128(sm + Lo.V + off, pack8(fv));
