@@ -84,8 +84,10 @@ struct BMisc {
     float extra[128];     // column sums of S . dS: d log gamma carried in from the later chunks
     float rn[128];        // 1/|k|, 1/|q| of the chunk's tokens
     float beta[64];
-    float dbp[4][64];     // dbeta partial sums of the column parts
-    float pre[4][128];    // gamma_a(b)/gamma_{-1}: product of etot[b'] over b' < b
+    union {               // dbp lives from L2 to the start of L3, pre from L4 to L5
+        float dbp[8][64];     // dbeta partial sums of the column parts of the two sides
+        float pre[4][128];    // gamma_a(b)/gamma_{-1}: product of etot[b'] over b' < b
+    };
     union {               // thread j turns its four column-sum partials into suf[.][j]: same addresses, no hazard
         float colp[4][128];   // column-sum partials per lane quadrant
         float suf[4][128];    // gamma_L/gamma_a(b): product of etot[b'] over b' >= b
@@ -336,13 +338,16 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             }
         }
         PROF(g_prof_bwd, 0);
-        // row-private record data of L2 straight from global memory: the Q-side threads, idle through L1, issue the
-        // loads now so that their latency hides behind L1
-        uint4 e4[HK / 8], x4[HK / 8], w4[HK / 8];
-        if (!krole && live) {
+        // L2 and L6 split a token's columns between its two threads: the K-side lane takes the first half of the
+        // columns (x or j < D/2), the Q-side lane the second; `cq0` = this thread's first 16-byte piece (QW columns).
+        constexpr int QW = D / (2 * NP);
+        const int cq0 = ((krole ? 0 : D / 2) + half * QW) / 8;
+        // row-private record data of L2 straight from global memory, issued now so that the latency hides behind L1
+        uint4 e4[QW / 8], x4[QW / 8], w4[QW / 8];
+        if (live) {
 #pragma unroll
-            for (int i = 0; i < HK / 8; ++i) {
-                const uint32_t off = rp_off(t, half * (HK / 8) + i);
+            for (int i = 0; i < QW / 8; ++i) {
+                const uint32_t off = rp_off(t, cq0 + i);
                 e4[i] = ldg128(rc + Rc.E + off);
                 x4[i] = ldg128(rc + Rc.VWX + off);
                 w4[i] = ldg128(rc + Rc.W + off);
@@ -381,52 +386,47 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mma_ph ^= 1u;  // Q-side threads skip this wait
         }
         PROF(g_prof_bwd, 1);
-        // ---- L2: dX = T^T dU -> BM_A rows 64..127
+        // ---- L2: dX = T^T dU: columns x < D/2 -> BM_A rows 0..63 (K-side lanes), x >= D/2 -> rows 64..127 (Q-side lanes)
         PHASE_SYNC();
         if (tid == 0) {
-            mma_k<MNMAJ, MNMAJ>(tmem + BM_A, D, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[0], 64, 0, 0, LCc, false);
+            mma_k<MNMAJ, MNMAJ>(tmem + BM_A + D / 2, D / 2, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[0], 64, D / 2, 0, LCc, false);
+            mma_k<MNMAJ, MNMAJ>(tmem + BM_A, D / 2, sb + Lo.S[1], 64, 64, 0, sb + Lo.S[0], 64, 0, 0, LCc, false);
             umma_commit(&mi.bar_mma);
         }
-        if (!krole) {
-            WAIT_MMA();
-            if (warp_active) {
-                const float bt = live ? mi.beta[t] : 0.f;
-                float dbs = 0.f;
-                __nv_bfloat16* gdv = a.dv + ((tok0 + t) * a.H + h) * D;
-                __nv_bfloat16* gdwx = a.dwx + ((tok0 + t) * a.H + h) * D;
+        WAIT_MMA();
+        if (tid == 0) {  // PT is dead: fetch the block-anchored column operand of L4
+            mbar_expect_tx(&mi.bar_g4a, TB);
+            bulk_g2s(sm + Lo.S[1], rc + Rc.CC, TB, &mi.bar_g4a);
+        }
+        if (warp_active) {
+            const float bt = live ? mi.beta[t] : 0.f;
+            float dbs = 0.f;
+            __nv_bfloat16* gdv = a.dv + ((tok0 + t) * a.H + h) * D;
+            __nv_bfloat16* gdwx = a.dwx + ((tok0 + t) * a.H + h) * D;
+            uint32_t v[QW];
+            if constexpr (QW == 16) tmem_ld16(tmem + BM_A + lane_base + 8 * cq0, v);
+            else tmem_ld32(tmem + BM_A + lane_base + 8 * cq0, v);
+            tmem_wait_ld();
+            if (live) {
 #pragma unroll
-                for (int s = 0; s < HK; s += 32) {
-                    uint32_t v[32];
-                    tmem_ld32(tmem + BM_A + lane_base + half * HK + s, v);
-                    tmem_wait_ld();
-                    if (live) {
+                for (int i = 0; i < QW / 8; ++i) {
+                    const int cc = cq0 + i;
+                    float ee[8], xx[8], ww[8], ndr[8], o1[8], o2[8];
+                    unpack8(e4[i], ee); unpack8(x4[i], xx); unpack8(w4[i], ww);
 #pragma unroll
-                        for (int ch = 0; ch < 4; ++ch) {
-                            const int i = s / 8 + ch, cc = half * (HK / 8) + i;
-                            float ee[8], xx[8], ww[8], ndr[8], o1[8], o2[8];
-                            unpack8(e4[i], ee); unpack8(x4[i], xx); unpack8(w4[i], ww);
-#pragma unroll
-                            for (int e = 0; e < 8; ++e) {
-                                const float dx = __uint_as_float(v[8 * ch + e]);
-                                const float dr = bt * dx;
-                                dbs += dx * ee[e];
-                                ndr[e] = -dr;
-                                o1[e] = dr * ww[e];
-                                o2[e] = dr * xx[e];
-                            }
-                            sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8(ndr));
-                            stg128(gdv + 8 * cc, pack8(o1));
-                            stg128(gdwx + 8 * cc, pack8(o2));
-                        }
+                    for (int e = 0; e < 8; ++e) {
+                        const float dx = __uint_as_float(v[8 * i + e]);
+                        const float dr = bt * dx;
+                        dbs += dx * ee[e];
+                        ndr[e] = -dr;
+                        o1[e] = dr * ww[e];
+                        o2[e] = dr * xx[e];
                     }
+                    sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8(ndr));
+                    stg128(gdv + 8 * cc, pack8(o1));
+                    stg128(gdwx + 8 * cc, pack8(o2));
                 }
-                if (live) mi.dbp[half][t] = dbs;
-            }
-        } else {
-            WAIT_MMA();
-            if (tid == 0) {  // PT is dead: fetch the block-anchored column operand of L4
-                mbar_expect_tx(&mi.bar_g4a, TB);
-                bulk_g2s(sm + Lo.S[1], rc + Rc.CC, TB, &mi.bar_g4a);
+                mi.dbp[(krole ? 0 : NP) + half][t] = dbs;
             }
         }
         PROF(g_prof_bwd, 2);
@@ -446,7 +446,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         {
             float sdb = 0.f;
 #pragma unroll
-            for (int pp = 0; pp < NP; ++pp) sdb += mi.dbp[pp][t];
+            for (int pp = 0; pp < NP; ++pp) sdb += mi.dbp[pp][t] + mi.dbp[NP + pp][t];
             a.dbeta[(tok0 + t) * a.H + h] = __float2bfloat16_rn(sdb);
         }
         WAIT_MMA();
@@ -758,12 +758,18 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             }
         }
         PROF(g_prof_bwd, 6);
-        // ---- L6: d log a_t = dlp_t + carry + sum_{t' > t} XA_t' + sum_{t' >= t} XQ_t' + sum_{t' < t} Z_t'  -> BM_KT rows 0..63
+        // ---- L6: d log a_t = dlp_t + carry + sum_{t' > t} XA_t' + sum_{t' >= t} XQ_t' + sum_{t' < t} Z_t' -> BM_KT:
+        //      key channels j < D/2 in rows 0..63 (K-side lanes), j >= D/2 in rows 64..127 (Q-side lanes: the 0/1 tile
+        //      used as the upper half of the M = 128 operand), so both threads of a token share the epilogue
         PHASE_SYNC();
         if (tid == 0) {
-            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D, sb + Lo.TRI, 64, 0, 0, sb + Lo.S[2], 128, 0, 0, LCc, false);
-            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D, sb + Lo.TRI, 64, 0, 64, sb + Lo.S[2], 128, 0, 64, LCc, true);
-            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D, sb + Lo.TRI, 64, 0, 128, sb + Lo.S[4], 64, 0, 0, LCc, true);
+            const uint32_t tri = sb + Lo.TRI, trh = tri - 8192;
+            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D / 2, tri, 64, 0, 0, sb + Lo.S[2], 128, 0, 0, LCc, false);
+            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D / 2, tri, 64, 0, 64, sb + Lo.S[2], 128, 0, 64, LCc, true);
+            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D / 2, tri, 64, 0, 128, sb + Lo.S[4], 64, 0, 0, LCc, true);
+            mma_k<KMAJ, MNMAJ>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 0, sb + Lo.S[2], 128, D / 2, 0, LCc, false);
+            mma_k<KMAJ, MNMAJ>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 64, sb + Lo.S[2], 128, D / 2, 64, LCc, true);
+            mma_k<KMAJ, MNMAJ>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 128, sb + Lo.S[4], 64, D / 2, 0, LCc, true);
             umma_commit(&mi.bar_mma);
             // K0, Q0 are dead: fetch G^T of the chunk and the raw q rows for L8
             mbar_expect_tx(&mi.bar_g8, tile_bytes(D, 64));
@@ -773,41 +779,10 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mbar_expect_tx(&mi.bar_bg, TB);   // the erase gate b over gamma_t/gamma_a (dead after L5)
             bulk_g2s(sm + Lo.FI, rc + Rc.Bg, TB, &mi.bar_bg);
         }
-        if (krole) {
-            WAIT_MMA();
-            mbar_wait(&mi.bar_bg, ph);
-            if (warp_active) {
-                __nv_bfloat16* gdf = a.df + ((tok0 + t) * a.H + h) * D;
-                __nv_bfloat16* gdbx = a.dbx + ((tok0 + t) * a.H + h) * D;
-#pragma unroll
-                for (int s = 0; s < HK; s += 32) {
-                    uint32_t v[32];
-                    tmem_ld32(tmem + BM_KT + lane_base + half * HK + s, v);
-                    tmem_wait_ld();
-                    if (live) {
-#pragma unroll
-                        for (int ch = 0; ch < 4; ++ch) {
-                            const int i = s / 8 + ch, cc = half * (HK / 8) + i;
-                            float bb[8], dp[8], dla[8], dbp[8];
-                            unpack8(lds128(sm + Lo.FI + rp_off(t, cc)), bb);
-                            unpack8(lds128(sm + Lo.S[0] + tile_chunk_off(64, t, cc)), dp);
-#pragma unroll
-                            for (int e = 0; e < 8; ++e) {
-                                dla[e] = __uint_as_float(v[8 * ch + e]) + dp[e] + mi.extra[8 * cc + e];
-                                dbp[e] = -dla[e] * bb[e];
-                            }
-                            stg128(gdf + 8 * cc, pack8(dla));    // d log a; the epilogue kernel turns it into df
-                            const uint4 w = pack8(dbp);
-                            stg128(gdbx + 8 * cc, w);
-                            sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), w);   // GW rows 0..63 = db_pre
-                        }
-                    }
-                }
-            }
-        } else {
-            // Q side: dw_pre rows (this thread wrote them to dwx in L2) -> GW rows 64..127;  [tt_b|0 ; 0|tt_w] -> S[1]
+        {
+            // dw_pre rows (written to dwx in L2) -> GW rows 64..127, [tt_b|0 ; 0|tt_w] -> S[1]: Q-side threads, loads first
             uint4 d4[HK / 8], t4[4];
-            if (live) {
+            if (!krole && live) {
                 const __nv_bfloat16* gdwx = a.dwx + ((tok0 + t) * a.H + h) * D;
 #pragma unroll
                 for (int i = 0; i < HK / 8; ++i) d4[i] = *reinterpret_cast<const uint4*>(gdwx + 8 * (half * (HK / 8) + i));
@@ -815,10 +790,10 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 for (int i = 0; i < 4; ++i) t4[i] = ldg128(rc + Rc.tt + t * 64 + 16 * i);
             }
             WAIT_MMA();
-            if (live) {
+            if (!krole && live) {
 #pragma unroll
                 for (int i = 0; i < HK / 8; ++i) sts128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, half * (HK / 8) + i), d4[i]);
-                // TT2: row t = [tt_b | 0], row 64+t = [0 | tt_w] over 32 columns; half 0 writes the K-side row
+                // TT2: row t = [tt_b | 0], row 64+t = [0 | tt_w] over 32 columns; part 0 writes the K-side row
                 const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
                 const int rc8 = r >> 3;  // 16-byte chunks per gate half
 #pragma unroll
@@ -826,6 +801,33 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                     const bool is_b = i < rc8, is_w = i >= rc8 && i < 2 * rc8;
                     if (half == 0) sts128(sm + Lo.S[1] + tile_chunk_off(128, t, i), is_b ? t4[i] : z4);
                     else if (half == 1) sts128(sm + Lo.S[1] + tile_chunk_off(128, 64 + t, i), is_w ? t4[i] : z4);
+                }
+            }
+            mbar_wait(&mi.bar_bg, ph);
+            if (warp_active) {
+                __nv_bfloat16* gdf = a.df + ((tok0 + t) * a.H + h) * D;
+                __nv_bfloat16* gdbx = a.dbx + ((tok0 + t) * a.H + h) * D;
+                uint32_t v[QW];
+                if constexpr (QW == 16) tmem_ld16(tmem + BM_KT + lane_base + 8 * cq0, v);
+                else tmem_ld32(tmem + BM_KT + lane_base + 8 * cq0, v);
+                tmem_wait_ld();
+                if (live) {
+#pragma unroll
+                    for (int i = 0; i < QW / 8; ++i) {
+                        const int cc = cq0 + i;
+                        float bb[8], dp[8], dla[8], dbp[8];
+                        unpack8(lds128(sm + Lo.FI + rp_off(t, cc)), bb);
+                        unpack8(lds128(sm + Lo.S[0] + tile_chunk_off(64, t, cc)), dp);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            dla[e] = __uint_as_float(v[8 * i + e]) + dp[e] + mi.extra[8 * cc + e];
+                            dbp[e] = -dla[e] * bb[e];
+                        }
+                        stg128(gdf + 8 * cc, pack8(dla));    // d log a; the epilogue kernel turns it into df
+                        const uint4 w = pack8(dbp);
+                        stg128(gdbx + 8 * cc, w);
+                        sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), w);   // GW rows 0..63 = db_pre
+                    }
                 }
             }
         }
