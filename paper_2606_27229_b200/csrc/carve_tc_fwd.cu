@@ -294,6 +294,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     if (tid == 0) { fence_async_smem(); issue_kq(0); issue_fb(0); issue_wv(0); }
 
     uint32_t mma_ph = 0, tma_ph = 0;
+    // write strength of this thread's token, fetched one chunk ahead (a plain global load: its latency must not sit
+    // on the chunk's serial path)
+    float beta_nx = (krole && half == 0 && live) ? __bfloat162float(a.beta[((size_t)b * a.T + t) * a.H + h]) : 0.f;
     PROF_INIT();
     for (int c = 0; c < nchunks; ++c) {
         const bool fold_now = (c % gate_every) == 0;
@@ -320,7 +323,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             mi.nrm[row][half] = ss;
             if (krole && half == 0) {
                 // clamped away from 0 so that e_t = u_t / beta_t exists (u_t changes by < 1e-30 |e_t|)
-                const float bt = fmaxf(__bfloat162float(a.beta[(tok0 + t) * a.H + h]), 1e-30f);
+                const float bt = fmaxf(beta_nx, 1e-30f);
+                if (c + 1 < nchunks) beta_nx = __bfloat162float(a.beta[(tok0 + LCc + t) * a.H + h]);
                 sBeta[t] = bt;
                 if (rc) reinterpret_cast<float*>(rc + Rc.beta)[t] = bt;
             }
