@@ -231,7 +231,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     const size_t state_tile = tile_bytes(DV, DK);
     const Rec Rc(DK, DV);
     uint8_t* rec_chain = a.rec ? a.rec + (size_t)chain * nchunks * Rc.total : nullptr;
-    uint8_t* ws_chain = rec_chain ? rec_chain + Rc.SB : nullptr;  // state tile of chunk 0
+    const bool s1 = a.scale == 1.f;   // then scale.P and scale.Qbar of the record are the shared-memory tiles themselves
 
     // initial state: fp32 -> TMEM, bf16 -> Sb (and the workspace slot of chunk 0)
     if (row < DV) {
@@ -255,7 +255,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 const uint4 w = pack8(f8);
                 const uint32_t off = tile_chunk_off(DV, row, c0 / 8 + ch);
                 sts128(sm + Lo.Sb + off, w);
-                if (ws_chain) *reinterpret_cast<uint4*>(ws_chain + off) = w;
             }
         }
         tmem_wait_st();
@@ -305,6 +304,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 0);
         // ---- P0: fold G^T = S^T Ucat^T -> TM_X2[0, R2)
         PHASE_SYNC();
+        if (rc && tid == 0) {   // record: state entering the chunk (Sb stays intact until P13)
+            bulk_s2g(rc + Rc.SB, sb + Lo.Sb, (uint32_t)state_tile);
+            bulk_commit();
+        }
         if (fold_now && tid == 0) {
             mma_rt<128, MNMAJ, KMAJ>(tmem + TM_X2, R2, sb + Lo.Sb, DV, 0, sb + Lo.Ucat, R2, 0, DV, false);
             umma_commit(&mi.bar_mma);
@@ -569,8 +572,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                             sts128(sm + Lo.Y1 + off, pack8(o1));      // C_t
                             sts128(sm + Lo.Ktil + off, pack8(o2));    // Ktil_t
                             if (rc) {
-                                *reinterpret_cast<uint4*>(rc + Rc.CC + off) = pack8(o1);
-                                *reinterpret_cast<uint4*>(rc + Rc.KT + off) = pack8(o2);
                                 *reinterpret_cast<uint4*>(rc + Rc.IC + rp_off(t, cc)) = pack8(ic);
                             }
                         }
@@ -580,7 +581,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         for (int e = 0; e < 8; ++e) { qv[e] *= rnq; kv[e] *= rnkn; }
                         if (has_next && bn > blk) {  // first row of its block
                             sts128(ver_row(bn, false, tn, cc), pack8(kv));
-                            if (rc) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = pack8(kv);
                         }
                         if (rc) *reinterpret_cast<uint4*>(rc + Rc.FQ + rp_off(t, cc)) = pack8(Fp);
 #pragma unroll
@@ -590,8 +590,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                                 for (int e = 0; e < 8; ++e) o[e] = qv[e] * Fp[e];
                                 const uint4 wq = pack8(o);
                                 sts128(ver_row(jb, true, t, cc), wq);
-                                if (rc && jb == blk) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, 64 + t, cc)) = wq;
-                                if (rc && jb == 0) {
+                                if (rc && jb == 0 && !s1) {
 #pragma unroll
                                     for (int e = 0; e < 8; ++e) o[e] *= a.scale;
                                     *reinterpret_cast<uint4*>(rc + Rc.Q0 + tile_chunk_off(64, t, cc)) = pack8(o);
@@ -601,9 +600,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                                     for (int e = 0; e < 8; ++e) o[e] = kv[e] * Fp[e];
                                     const uint4 wk = pack8(o);
                                     sts128(ver_row(jb, false, tn, cc), wk);
-                                    if (rc && jb == blk && bn == blk)
-                                        *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = wk;
-                                    if (rc && jb == 0) *reinterpret_cast<uint4*>(rc + Rc.K0 + tile_chunk_off(64, tn, cc)) = wk;
                                 }
                                 if (jb > 0) {
                                     const float4 e0 = *reinterpret_cast<const float4*>(&mi.etot[jb - 1][8 * cc]);
@@ -615,10 +611,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         }
                         if (!has_next) {  // Kbar_0 = k^_0
                             sts128(sm + Lo.KQbar + tile_chunk_off(128, 0, cc), pack8(kv));
-                            if (rc) {
-                                *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, 0, cc)) = pack8(kv);
-                                *reinterpret_cast<uint4*>(rc + Rc.K0 + tile_chunk_off(64, 0, cc)) = pack8(kv);
-                            }
                         }
                     }
                 }
@@ -634,9 +626,34 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             if (nb > 2) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 32, 16, sb + Lo.Y0, 64, 0, sb + Lo.Y1, 64, 32, DK, false);
             if (nb > 3) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 48, 16, sb + Lo.Y2 + tile_bytes(96, DK), 32, 0, sb + Lo.Y1, 64, 48, DK, false);
             mma_rt<128, KMAJ, KMAJ>(tmem + TM_ACC, DV, sb + Lo.KQbar, 128, 0, sb + Lo.Sb, DV, 0, DK, false);
+            if (rc) {
+                // record: operand tiles straight from shared memory (bulk copies, no thread stores).  The sources are
+                // rewritten from P9a on: thread 0 waits for the copies to have read them before the barrier there.
+                constexpr uint32_t TB = tile_bytes(64, DK);
+                bulk_s2g(rc + Rc.KT, sb + Lo.Ktil, TB);
+                bulk_s2g(rc + Rc.CC, sb + Lo.Y1, TB);
+                for (int cb = 0; cb < DK / 64; ++cb) {
+                    bulk_s2g(rc + Rc.K0 + cb * 8192, sb + Lo.KQbar + cb * 16384, 8192);                  // Kbar rows
+                    if (s1) bulk_s2g(rc + Rc.Q0 + cb * 8192, sb + Lo.KQbar + cb * 16384 + 8192, 8192);   // Qbar rows
+                    // rows anchored at their own block: the 16 K-side and 16 Q-side rows of block jb in version jb
+                    const uint32_t vt[4] = {sb + Lo.KQbar, sb + Lo.Y2, sb + Lo.Y0, sb + Lo.Y2 + tile_bytes(96, DK)};
+                    const uint32_t vstride[4] = {128 * 128, 96 * 128, 64 * 128, 32 * 128};   // column-block strides
+                    const uint32_t vq[4] = {64 * 128, 48 * 128, 32 * 128, 16 * 128};         // first Q-side row
+                    for (int jb = 0; jb < nb; ++jb) {
+                        uint8_t* dst = rc + Rc.KQo + cb * 16384 + jb * 2048;
+                        bulk_s2g(dst, vt[jb] + cb * vstride[jb], 2048);
+                        bulk_s2g(dst + 8192, vt[jb] + cb * vstride[jb] + vq[jb], 2048);
+                    }
+                }
+                bulk_commit();
+            }
             umma_commit(&mi.bar_mma);
         }
         WAIT_MMA();
+        if (rc) {   // the version tiles (Y2 and, at d = 128, the TP region behind it) still feed the record's bulk copies
+            if (tid == 0) bulk_wait_read();
+            __syncthreads();
+        }
         PROF(g_prof_fwd, 10);
         // ---- P9a: beta A -> Mm (fp32, only the strictly lower part is ever read), P -> TP rows 64.. (bf16, masked s <= t)
         {
@@ -652,7 +669,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     for (int e = 0; e < 16; ++e) f[e] = (16 * jb + e <= tok) ? __uint_as_float(v[e]) : 0.f;
                     sts128(sm + Lo.TP + tile_chunk_off(128, 64 + tok, 2 * jb), pack8(f));
                     sts128(sm + Lo.TP + tile_chunk_off(128, 64 + tok, 2 * jb + 1), pack8(f + 8));
-                    if (rc) {  // the record keeps scale.P in rows 0..63
+                    if (rc && !s1) {  // the record keeps scale.P in rows 0..63 (scale = 1: bulk copy of the tile)
 #pragma unroll
                         for (int e = 0; e < 16; ++e) f[e] *= a.scale;
                         *reinterpret_cast<uint4*>(rc + Rc.PT + tile_chunk_off(128, tok, 2 * jb)) = pack8(f);
@@ -673,7 +690,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         for (int jb = (t >> 4) + 1; jb < 4; ++jb) {
                             sts128(sm + Lo.TP + tile_chunk_off(128, 64 + t, 2 * jb), z4);
                             sts128(sm + Lo.TP + tile_chunk_off(128, 64 + t, 2 * jb + 1), z4);
-                            if (rc) {
+                            if (rc && !s1) {
                                 *reinterpret_cast<uint4*>(rc + Rc.PT + tile_chunk_off(128, t, 2 * jb)) = z4;
                                 *reinterpret_cast<uint4*>(rc + Rc.PT + tile_chunk_off(128, t, 2 * jb + 1)) = z4;
                             }
@@ -748,7 +765,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         f[e] = s <= tr_ ? Tm[mm_idx(tr_, s)] : 0.f;
                     }
                     sts128(sm + Lo.TP + tile_chunk_off(128, tr_, 2 * qq + k8), pack8(f));
-                    if (rc) *reinterpret_cast<uint4*>(rc + Rc.PT + tile_chunk_off(128, 64 + tr_, 2 * qq + k8)) = pack8(f);
                 }
             }
         }
@@ -758,6 +774,11 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         if (tid == 0) {
             mma_rt<128, KMAJ, MNMAJ>(tmem + TM_X1, DV, sb + Lo.TP, 128, 0, sb + Lo.Y2, 64, 0, LCc, false);
             umma_commit(&mi.bar_mma);
+            if (rc) {   // record [scale.P ; T]: the two row halves of TP swapped (TP is next written in P9 of the next chunk)
+                if (s1) bulk_s2g(rc + Rc.PT, sb + Lo.TP + 8192, 8192);
+                bulk_s2g(rc + Rc.PT + 8192, sb + Lo.TP, 8192);
+                bulk_commit();
+            }
             if (c + 1 < nchunks) issue_kq(c + 1);
         }
         WAIT_MMA();
@@ -777,7 +798,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     const uint32_t off = tile_chunk_off(64, t, cc);
                     sts128(sm + Lo.Us + off, pack8(f));
                     if (rc) {
-                        *reinterpret_cast<uint4*>(rc + Rc.U + off) = pack8(f);
 #pragma unroll
                         for (int e = 0; e < 8; ++e) f[e] *= rbt;  // e_t = u_t / beta_t (Alg. 2 step 7)
                         *reinterpret_cast<uint4*>(rc + Rc.E + rp_off(t, cc)) = pack8(f);
@@ -792,6 +812,11 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             mma_rt<128, KMAJ, MNMAJ>(tmem + TM_ACC, DV, sb + Lo.TP, 128, 0, sb + Lo.Us, 64, 0, LCc, true);
             mma_rt<128, MNMAJ, MNMAJ>(tmem + TM_X2, DK, sb + Lo.Us, 64, 0, sb + Lo.Ktil, 64, 0, LCc, false);
             umma_commit(&mi.bar_mma);
+            if (rc) {   // record U (its buffer is refilled by the next chunk's loads below)
+                bulk_s2g(rc + Rc.U, sb + Lo.Us, tile_bytes(64, DV));
+                bulk_commit();
+                bulk_wait_read();
+            }
         }
         WAIT_MMA();
         if (tid == 0 && c + 1 < nchunks) { fence_async_smem(); issue_fb(c + 1); issue_wv(c + 1); }
@@ -814,8 +839,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         if (q * 32 < DV) {
             const bool last_chunk = c + 1 == nchunks;
-            uint8_t* ws_next = !ws_chain ? nullptr
-                               : last_chunk ? a.sfin + (size_t)chain * state_tile : ws_chain + (size_t)(c + 1) * Rc.total;
 #pragma unroll 1
             for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
                 uint32_t sv[8], wv[8];
@@ -832,7 +855,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 const uint4 w = pack8(f);
                 const uint32_t off = tile_chunk_off(DV, row, cc);
                 sts128(sm + Lo.Sb + off, w);
-                if (ws_next) *reinterpret_cast<uint4*>(ws_next + off) = w;
                 if (last_chunk) {
                     float* dst = a.S_final + ((size_t)chain * DV + row) * DK + 8 * cc;
                     *reinterpret_cast<float4*>(dst) = make_float4(f[0], f[1], f[2], f[3]);
@@ -845,6 +867,11 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 17);
     }
     PHASE_SYNC();
+    if (rec_chain && tid == 0) {   // the final state as the reverse kernel's operand tile; drain every bulk store
+        bulk_s2g(a.sfin + (size_t)chain * state_tile, sb + Lo.Sb, (uint32_t)state_tile);
+        bulk_commit();
+        bulk_wait_all();
+    }
     if (warp == 0) tmem_dealloc(tmem, TM_COLS);
 }
 
