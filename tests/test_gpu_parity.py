@@ -251,3 +251,36 @@ def test_config3_long_context_forward_reduced_heads(oracle):
     cfg = synth.CFG3.with_(H=2)
     x = synth.make_inputs(cfg)
     _check_fwd_bwd(oracle, cfg, x, with_bwd=False)
+
+
+@pytest.mark.parametrize("B,H,T,L,d,r,seed", [(3, 5, 64, 64, 128, 8, 101), (1, 3, 192, 64, 128, 16, 102), (2, 1, 32, 16, 64, 16, 103),
+                                              (1, 7, 384, 128, 128, 16, 104), (5, 2, 96, 32, 64, 8, 105)])
+def test_tensor_path_odd_shapes(oracle, B, H, T, L, d, r, seed):
+    """Single-chunk sequences, odd batch / head counts, every supported r, nonzero S0, A and tau present."""
+    cfg = synth.Config("t", B=B, H=H, T=T, L=L, dk=d, dv=d, r=r, dtype="bf16", wstd=0.1, s0_std=0.05, seed=seed)
+    x = synth.make_inputs(cfg, with_decay_params=True)
+    _check_fwd_bwd(oracle, cfg, x, path=carve.CARVE_PATH_TENSOR)
+
+
+def test_tensor_path_repeated_calls_same_workspace(oracle):
+    """Back-to-back fwd/bwd pairs on one stream reuse the workspace and the outputs: results must not change."""
+    import torch
+    cfg = synth.Config("t", B=2, H=3, T=512, L=64, dk=128, dv=128, r=16, dtype="bf16", wstd=0.1, seed=77)
+    x, ct = synth.make_inputs(cfg), synth.make_cotangents(cfg)
+    p = params_of(cfg, path=carve.CARVE_PATH_TENSOR)
+    O, Sf, h = run_fwd(p, x, need_bwd=True)
+    g0, gd = run_bwd(p, h, ct)
+    xd, ws = h
+    from tests.gpu_util import to_device
+    dO = to_device({"dO": ct["dO"]}, torch.bfloat16)["dO"]
+    dSf = torch.from_numpy(np.ascontiguousarray(ct["dS_final"], dtype=np.float32)).cuda()
+    Od = torch.empty(cfg.B, cfg.T, cfg.H, cfg.dv, dtype=torch.bfloat16, device="cuda")
+    Sfd = torch.empty(cfg.B, cfg.H, cfg.dv, cfg.dk, dtype=torch.float32, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    for _ in range(3):
+        carve.carve_fwd(p, xd, Od, Sfd, ws, st)
+        carve.carve_bwd(p, xd, dO, dSf, gd, ws, st)
+    torch.cuda.synchronize()
+    assert np.array_equal(Od.float().cpu().numpy().astype(np.float64), O)
+    for n in GRADS:
+        assert np.array_equal(gd[n].float().cpu().numpy().astype(np.float64), g0[n]), n
