@@ -1113,7 +1113,7 @@ extern "C" void carve_debug_prof_bwd(unsigned long long* out)
 }
 #endif
 
-bool tc_bwd_supported(const carve_params_t& p) { return tc_fwd_supported(p); }
+bool tc_bwd_supported(const carve_params_t& p) { return tc_fwd_supported(p) && p.dk == p.dv; }
 
 cudaError_t tc_bwd_launch(const Args& a, uint8_t* ws, const TcWsLayout& w, float* dA, float* dtau, float* dUb, float* dUw,
                           float* dVb, float* dVw, cudaStream_t st)

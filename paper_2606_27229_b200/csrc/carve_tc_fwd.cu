@@ -31,6 +31,7 @@ PROF_DECL(g_prof_fwd)
 
 struct TcArgs {
     int B, H, T, L, r;
+    int dvf;        // full d_v of the tensors (= VS x the value channels one CTA owns)
     int l2norm;
     float scale, eps;
     const __nv_bfloat16* beta;
@@ -170,7 +171,14 @@ __device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid, int nthr
 
 // NP = number of column parts a tile row is split into = warpgroups per CTA (threads = 128 NP); every thread
 // serves one TMEM lane (tile row) and DK/NP columns.
-template <int DK, int DV, int NP>
+// VS = value split: a cluster of VS CTAs shares one chain, each owning DV of the d_v = VS*DV value channels.
+// The value columns of R, U, O and S are independent of one another (Thm 11); only the fold
+// G = [Ub;Uw] S sums over them, so the CTAs exchange their partial G through distributed shared memory once per
+// chunk and redo the (cheap) key-axis work redundantly.
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
+template <int DK, int DV, int NP, int VS>
 __global__ void __launch_bounds__(128 * NP, 1)
 carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, const __grid_constant__ CUtensorMap mk,
                     const __grid_constant__ CUtensorMap mv, const __grid_constant__ CUtensorMap mf,
@@ -195,7 +203,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     const bool krole = q < 2;
     const int t = row & 63;          // token of this row
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
-    const int chain = blockIdx.x, b = chain / a.H, h = chain % a.H;
+    const int crank = VS > 1 ? (int)(blockIdx.x % VS) : 0;   // rank inside the cluster = which slice of value channels
+    const int vofs = crank * DV;
+    const int chain = blockIdx.x / VS, b = chain / a.H, h = chain % a.H;
     const int LCc = a.L < LC ? a.L : LC;
     const int nchunks = a.T / LCc, gate_every = a.L / LCc;
     const bool warp_active = (q & 1) * 32 < LCc;  // this warp holds at least one live token row
@@ -211,7 +221,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     if (warp == 0) tmem_alloc(&mi.tmem_base, TM_COLS);
     for (int i = tid; i < R2 * DV; i += NTH) {
         const int ii = i / DV, x = i % DV;
-        const float v = ii < r ? __ldg(a.Ub + (size_t)ii * DV + x) : __ldg(a.Uw + (size_t)(ii - r) * DV + x);
+        const float v = ii < r ? __ldg(a.Ub + (size_t)ii * a.dvf + vofs + x) : __ldg(a.Uw + (size_t)(ii - r) * a.dvf + vofs + x);
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Ucat + tile_off(R2, ii, x)) = __float2bfloat16_rn(v);
     }
     for (int i = tid; i < DM * 64; i += NTH) {
@@ -219,7 +229,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         float v = 0.f;
         // each gate half padded to 16 columns, so that the two up-projections are separate K = 16 slices
         if (c < 16) { if (c < r && n < DK) v = __ldg(a.Vb + (size_t)n * r + c); }
-        else if (c < 32) { if (c - 16 < r && n < DV) v = __ldg(a.Vw + (size_t)n * r + (c - 16)); }
+        else if (c < 32) { if (c - 16 < r && n < DV) v = __ldg(a.Vw + (size_t)(vofs + n) * r + (c - 16)); }
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Vcat + tile_off(DM, n, c)) = __float2bfloat16_rn(v);
     }
     for (int j = tid; j < DK; j += NTH) {
@@ -235,7 +245,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
 
     // initial state: fp32 -> TMEM, bf16 -> Sb (and the workspace slot of chunk 0)
     if (row < DV) {
-        const float* s0 = a.S0 ? a.S0 + ((size_t)chain * DV + row) * DK : nullptr;
+        const float* s0 = a.S0 ? a.S0 + ((size_t)chain * a.dvf + vofs + row) * DK : nullptr;
 #pragma unroll
         for (int s = 0; s < HK; s += 32) {
             const int c0 = half * HK + s;
@@ -286,8 +296,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         mbar_expect_tx(&mi.bar_wv, 2u * LCc * DV * 2u);
         const int tr = b * a.T + c * LCc;
         for (int cb = 0; cb < DV / 64; ++cb) {
-            tma_load_3d(sm + Lo.WX + cb * 64 * 128, &mwx, &mi.bar_wv, cb * 64, h, tr);
-            tma_load_3d(sm + Lo.V + cb * 64 * 128, &mv, &mi.bar_wv, cb * 64, h, tr);
+            tma_load_3d(sm + Lo.WX + cb * 64 * 128, &mwx, &mi.bar_wv, vofs + cb * 64, h, tr);
+            tma_load_3d(sm + Lo.V + cb * 64 * 128, &mv, &mi.bar_wv, vofs + cb * 64, h, tr);
         }
     };
     if (tid == 0) { fence_async_smem(); issue_kq(0); issue_fb(0); issue_wv(0); }
@@ -336,6 +346,28 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             WAIT_MMA();
             PROF(g_prof_fwd, 1);
             // ---- P1: G^T (lanes j) -> bf16 into the spare columns [32, 32+R2) of the Vcat tile
+            if (VS > 1) {
+                // partial G^T of this CTA's value channels -> the peer's Y1 (fp32 [dk][32]); Y1 of the peer is free once it
+                // has passed P8 of its previous chunk (second cluster barrier phase, armed there)
+                if (c > 0) cluster_wait();
+                if (half == 0 && q * 32 < DK) {
+                    uint32_t raddr;
+                    const uint32_t laddr = sb + Lo.Y1 + (uint32_t)row * 128u;
+                    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(raddr) : "r"(laddr), "r"(crank ^ 1));
+                    for (int c0 = 0; c0 < R2; c0 += 16) {
+                        uint32_t v[16];
+                        tmem_ld16(tmem + TM_X2 + lane_base + c0, v);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int e = 0; e < 16; e += 4)
+                            asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(raddr + (c0 + e) * 4), "r"(v[e]),
+                                         "r"(v[e + 1]), "r"(v[e + 2]), "r"(v[e + 3])
+                                         : "memory");
+                    }
+                }
+                cluster_arrive();
+                cluster_wait();
+            }
             if (half == 0 && q * 32 < DK) {
                 for (int c0 = 0; c0 < R2; c0 += 16) {
                     uint32_t v[16];
@@ -344,6 +376,11 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     float f[16];
 #pragma unroll
                     for (int e = 0; e < 16; ++e) f[e] = __uint_as_float(v[e]);
+                    if (VS > 1) {   // + the peer's partial
+                        const float* pr = reinterpret_cast<const float*>(sm + Lo.Y1) + row * 32 + c0;
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) f[e] += pr[e];
+                    }
                     sts128(sm + Lo.Vcat + tile_chunk_off(DM, row, (32 + c0) / 8), pack8(f));
                     sts128(sm + Lo.Vcat + tile_chunk_off(DM, row, (32 + c0) / 8 + 1), pack8(f + 8));
                     if (rc) {
@@ -650,6 +687,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             umma_commit(&mi.bar_mma);
         }
         WAIT_MMA();
+        if (VS > 1) cluster_arrive();   // C (Y1) is consumed: the peer may send the next chunk's partial G
         if (rc) {   // the version tiles (Y2 and, at d = 128, the TP region behind it) still feed the record's bulk copies
             if (tid == 0) bulk_wait_read();
             __syncthreads();
@@ -823,7 +861,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 16);
         // ---- P13: outputs and the state carry
         if (!krole && warp_active) {
-            __nv_bfloat16* dst = a.O + ((tok0 + t) * a.H + h) * DV;
+            __nv_bfloat16* dst = a.O + ((tok0 + t) * a.H + h) * a.dvf + vofs;
 #pragma unroll 1
             for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
                 uint32_t v[8];
@@ -856,7 +894,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 const uint32_t off = tile_chunk_off(DV, row, cc);
                 sts128(sm + Lo.Sb + off, w);
                 if (last_chunk) {
-                    float* dst = a.S_final + ((size_t)chain * DV + row) * DK + 8 * cc;
+                    float* dst = a.S_final + ((size_t)chain * a.dvf + vofs + row) * DK + 8 * cc;
                     *reinterpret_cast<float4*>(dst) = make_float4(f[0], f[1], f[2], f[3]);
                     *reinterpret_cast<float4*>(dst + 4) = make_float4(f[4], f[5], f[6], f[7]);
                 }
@@ -866,6 +904,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         tma_ph ^= 1u;
         PROF(g_prof_fwd, 17);
     }
+    if (VS > 1) cluster_wait();   // pairs with the last arrive; also keeps this CTA's shared memory alive for the peer
     PHASE_SYNC();
     if (rec_chain && tid == 0) {   // the final state as the reverse kernel's operand tile; drain every bulk store
         bulk_s2g(a.sfin + (size_t)chain * state_tile, sb + Lo.Sb, (uint32_t)state_tile);
@@ -921,39 +960,52 @@ extern "C" void carve_debug_prof_fwd(unsigned long long* out)
 
 bool tc_fwd_supported(const carve_params_t& p)
 {
-    return p.dtype == CARVE_BF16 && p.dk == p.dv && (p.dk == 64 || p.dk == 128) && p.r <= 16;
+    if (p.dtype != CARVE_BF16 || p.r > 16) return false;
+    if (p.dk == p.dv && (p.dk == 64 || p.dk == 128)) return true;
+    return p.dk == 128 && p.dv == 256 && p.L <= 64;   // value channels split over a cluster of two CTAs (forward only)
 }
 
 size_t tc_state_tile_bytes(const carve_params_t& p) { return tc::tile_bytes(p.dv, p.dk); }
 size_t tc_record_bytes(const carve_params_t& p) { return tcp::Rec(p.dk, p.dv).total; }
 
-template <int D>
+template <int D, int VS>
 static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, uint8_t* sfin, cudaStream_t st)
 {
     const int LCc = a.L < tcp::LC ? a.L : tcp::LC;
     CUtensorMap mq, mk, mv, mf, mbx, mwx;
     if (!tc_make_token_map(&mq, a.q, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mk, a.k, a.B, a.T, a.H, D, LCc) ||
-        !tc_make_token_map(&mv, a.v, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mf, a.f, a.B, a.T, a.H, D, LCc) ||
-        !tc_make_token_map(&mbx, a.bx, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mwx, a.wx, a.B, a.T, a.H, D, LCc))
+        !tc_make_token_map(&mv, a.v, a.B, a.T, a.H, a.dv, LCc) || !tc_make_token_map(&mf, a.f, a.B, a.T, a.H, D, LCc) ||
+        !tc_make_token_map(&mbx, a.bx, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mwx, a.wx, a.B, a.T, a.H, a.dv, LCc))
         return cudaErrorInvalidValue;
     TcArgs t{};
     t.B = a.B; t.H = a.H; t.T = a.T; t.L = a.L; t.r = a.r; t.l2norm = a.l2norm; t.scale = a.scale; t.eps = a.eps;
+    t.dvf = a.dv;
     t.beta = static_cast<const __nv_bfloat16*>(a.beta);
     t.A = a.A; t.tau = a.tau; t.Ub = a.Ub; t.Uw = a.Uw; t.Vb = a.Vb; t.Vw = a.Vw; t.S0 = a.S0;
     t.O = static_cast<__nv_bfloat16*>(a.O); t.S_final = a.S_final; t.rec = rec; t.sfin = sfin;
     const size_t smem = tcp::Layout(D, D, 2 * a.r).total;
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
-    auto kern = carve_fwd_tc_kernel<D, D, NP>;
+    auto kern = carve_fwd_tc_kernel<D, D, NP, VS>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<a.B * a.H, 128 * NP, smem, st>>>(t, mq, mk, mv, mf, mbx, mwx);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(a.B * a.H * VS));
+    cfg.blockDim = dim3(128 * NP);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = VS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, t, mq, mk, mv, mf, mbx, mwx);
 }
 
 cudaError_t tc_fwd_launch(const Args& a, uint8_t* rec, uint8_t* sfin, cudaStream_t st)
 {
-    if (a.dk == 128) return launch_tc_fwd<128>(a, rec, sfin, st);
-    if (a.dk == 64) return launch_tc_fwd<64>(a, rec, sfin, st);
+    if (a.dk == 128 && a.dv == 256) return launch_tc_fwd<128, 2>(a, rec, sfin, st);   // inference only: two CTAs per chain
+    if (a.dk == 128) return launch_tc_fwd<128, 1>(a, rec, sfin, st);
+    if (a.dk == 64) return launch_tc_fwd<64, 1>(a, rec, sfin, st);
     return cudaErrorInvalidValue;
 }
 

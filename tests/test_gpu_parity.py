@@ -63,11 +63,13 @@ def test_head_dims_bf16(oracle, dk, dv, r):
 
 @pytest.mark.parametrize("dk,dv,r", [(128, 256, 16), (256, 64, 8)])
 def test_large_heads_forward_only(oracle, dk, dv, r):
-    """dk=128, dv=256 (config 3's head shape) and dk=256 are forward-only: bwd must refuse them, not fall back."""
+    """dk=128, dv=256 (config 3's head shape; tensor path, value channels split over a two-CTA cluster) and dk=256
+    (SIMT) are forward-only: bwd must refuse them, not fall back."""
     cfg = synth.Config("t", B=1, H=2, T=128, L=64, dk=dk, dv=dv, r=r, dtype="bf16", s0_std=0.01, seed=5)
     x = synth.make_inputs(cfg)
     _check_fwd_bwd(oracle, cfg, x, with_bwd=False)
     assert carve.carve_workspace_bytes(params_of(cfg), True) == 0
+    assert carve.carve_resolved_path(params_of(cfg), False) == (carve.CARVE_PATH_TENSOR if dv == 256 else carve.CARVE_PATH_SIMT)
 
 
 def test_single_chunk_and_scale(oracle):
