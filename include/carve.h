@@ -61,7 +61,10 @@ typedef enum {
 
 typedef enum { CARVE_F32 = 0, CARVE_BF16 = 1 } carve_dtype_t;
 
-/* Kernel family.  AUTO picks TENSOR for bf16 shapes it supports and SIMT otherwise. */
+/* Kernel family.  AUTO picks TENSOR for the shapes it covers and SIMT otherwise.  TENSOR (tcgen05 + TMA, fp32
+ * state in tensor memory) covers bf16 tokens with r <= 16 and dk == dv in {64,128} (forward and backward, every L),
+ * plus dk = 128, dv = 256 with L <= 64 for inference calls (forward without workspace).  An explicit TENSOR
+ * request outside that set returns CARVE_ERR_SHAPE; carve_resolved_path reports the choice. */
 typedef enum { CARVE_PATH_AUTO = 0, CARVE_PATH_SIMT = 1, CARVE_PATH_TENSOR = 2 } carve_path_t;
 
 typedef struct {
