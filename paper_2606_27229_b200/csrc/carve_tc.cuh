@@ -2,9 +2,9 @@
 // and TMEM maps, the thread <-> tile-row mapping, and small math helpers.
 // walks through the phases; the comments here state what each buffer holds.
 //
-// One CTA of 256 threads owns one (batch, head) chain for the whole sequence.  Every MMA has M = 128:
-// accumulator row r lives in TMEM lane r, warp w reads lanes 32*(w%4).., and the two warpgroups
-// (w/4 = 0, 1) split the columns of a tile in halves.  Rows 0..63 of a stacked tile are the
+// One CTA of 128 NP threads (NP = d/32 warpgroups: 256 threads at d = 64, 512 at d = 128) owns one (batch, head)
+// chain for the whole sequence.  Every MMA has M = 128: accumulator row r lives in TMEM lane r, warp w reads
+// lanes 32*(w%4).., and the NP warpgroups (w/4) split the columns of a tile into parts of 32.  Rows 0..63 of a stacked tile are the
 // "K-role" rows of the chunk's 64 tokens, rows 64..127 the "Q-role" rows of the same tokens, so
 // one instruction computes e.g. [Kbar; Qbar] S^T.
 #pragma once
@@ -65,14 +65,14 @@ struct Layout {  // byte offsets into the 1024-aligned dynamic shared memory
 //   SB   [dv][dk]   state entering the chunk, bf16
 //   KT   [64][dk]   Ktil_t = k^_t gamma_L/gamma_t
 //   PT   [128][64]  rows 0..63 scale.P (masked s <= t), rows 64..127 T = (I + diag(beta) A)^-1
-//   U    [64][dv]   u_t ;   E [64][dv]  e_t = u_t / beta_t  (row-private)
+//   U    [64][dv]   u_t  (e_t = u_t / beta_t is formed from it)
 //   K0,Q0 [64][dk]  Kbar_t = k^_t gamma_{t-1}, scale.Qbar_t = scale.q^_t gamma_t   (chunk-anchored)
 //   KQo  [128][dk]  the same rows anchored at the start of their own 16-token block
 //   CC   [64][dk]   C_s = k^_s gamma_a/gamma_s (a = start of s's 16-token block)
-//   VWX,W [64][dv]  w.v.(1-w) and w;  Bg [64][dk] erase gate b;  FQ,IC [64][dk] gamma_t/gamma_a and its inverse
+//   VWX,W [64][dv]  w.v.(1-w) and w;  Bg [64][dk] erase gate b;  FQ,IC [64][dk] gamma_t/gamma_a and its inverse (row-private, piece-major)
 //   tt   [64][32]   tanh bottleneck (bf16, plain rows);  GT [dk][32] G^T (tile);  etot [4][dk], rn [128], beta [64] fp32
 struct Rec {
-    uint32_t SB, KT, PT, U, K0, Q0, KQo, CC, E, VWX, W, Bg, FQ, IC, tt, GT, etot, rn, beta, total;
+    uint32_t SB, KT, PT, U, K0, Q0, KQo, CC, VWX, W, Bg, FQ, IC, tt, GT, etot, rn, beta, total;
     __host__ __device__ Rec(int dk, int dv)
     {
         uint32_t o = 0;
@@ -85,7 +85,6 @@ struct Rec {
         Q0 = take(tile_bytes(64, dk));
         KQo = take(tile_bytes(128, dk));
         CC = take(tile_bytes(64, dk));
-        E = take(tile_bytes(64, dv));
         VWX = take(tile_bytes(64, dv));
         W = take(tile_bytes(64, dv));
         Bg = take(tile_bytes(64, dk));

@@ -331,12 +331,11 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         constexpr int QW = D / (2 * NP);
         const int cq0 = ((krole ? 0 : D / 2) + half * QW) / 8;
         // row-private record data of L2 straight from global memory, issued now so that the latency hides behind L1
-        uint4 e4[QW / 8], x4[QW / 8], w4[QW / 8];
+        uint4 x4[QW / 8], w4[QW / 8];
         if (live) {
 #pragma unroll
             for (int i = 0; i < QW / 8; ++i) {
                 const uint32_t off = rp_off(t, cq0 + i);
-                e4[i] = ldg128(rc + Rc.E + off);
                 x4[i] = ldg128(rc + Rc.VWX + off);
                 w4[i] = ldg128(rc + Rc.W + off);
             }
@@ -388,6 +387,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         }
         if (warp_active) {
             const float bt = live ? mi.beta[t] : 0.f;
+            const float rbt = live ? __fdividef(1.f, bt) : 0.f;   // e_t = u_t / beta_t (beta is clamped to >= 1e-30 by the forward)
             float dbs = 0.f;
             __nv_bfloat16* gdv = a.dv + ((tok0 + t) * a.H + h) * D;
             __nv_bfloat16* gdwx = a.dwx + ((tok0 + t) * a.H + h) * D;
@@ -400,12 +400,13 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 for (int i = 0; i < QW / 8; ++i) {
                     const int cc = cq0 + i;
                     float ee[8], xx[8], ww[8], ndr[8], o1[8], o2[8];
-                    unpack8(e4[i], ee); unpack8(x4[i], xx); unpack8(w4[i], ww);
+                    unpack8(lds128(sm + Lo.S[4] + tile_chunk_off(64, t, cc)), ee);   // u_t (U tile, still the L3 operand)
+                    unpack8(x4[i], xx); unpack8(w4[i], ww);
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
                         const float dx = __uint_as_float(v[8 * i + e]);
                         const float dr = bt * dx;
-                        dbs += dx * ee[e];
+                        dbs += dx * (ee[e] * rbt);
                         ndr[e] = -dr;
                         o1[e] = dr * ww[e];
                         o2[e] = dr * xx[e];

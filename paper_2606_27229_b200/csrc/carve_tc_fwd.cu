@@ -608,9 +608,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                             const uint32_t off = tile_chunk_off(64, t, cc);
                             sts128(sm + Lo.Y1 + off, pack8(o1));      // C_t
                             sts128(sm + Lo.Ktil + off, pack8(o2));    // Ktil_t
-                            if (rc) {
-                                *reinterpret_cast<uint4*>(rc + Rc.IC + rp_off(t, cc)) = pack8(ic);
-                            }
+                            if (rc) *reinterpret_cast<uint4*>(rc + Rc.IC + rp_off(t, cc)) = pack8(ic);
                         }
                         unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, 64 + t, cc)), qv);
                         unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, krow, cc)), kv);
@@ -823,7 +821,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 14);
         // ---- P11: U -> bf16 rows (over V')
         if (krole && warp_active) {
-            const float rbt = live ? __fdividef(1.f, sBeta[t]) : 0.f;
 #pragma unroll 1
             for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
                 uint32_t v[8];
@@ -835,11 +832,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[e]);
                     const uint32_t off = tile_chunk_off(64, t, cc);
                     sts128(sm + Lo.Us + off, pack8(f));
-                    if (rc) {
-#pragma unroll
-                        for (int e = 0; e < 8; ++e) f[e] *= rbt;  // e_t = u_t / beta_t (Alg. 2 step 7)
-                        *reinterpret_cast<uint4*>(rc + Rc.E + rp_off(t, cc)) = pack8(f);
-                    }
                 }
             }
         }
