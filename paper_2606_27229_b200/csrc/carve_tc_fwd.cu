@@ -770,17 +770,18 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         // ---- P9b: beta R = beta (V' - Kbar S^T) -> Y2 (rows t)
         if (krole && warp_active) {
             const float bt = live ? sBeta[t] : 0.f;
-#pragma unroll 1
-            for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
-                uint32_t v[8];
-                tmem_ld8(tmem + TM_ACC + lane_base + 8 * cc, v);
-                tmem_wait_ld();
-                if (live) {
+            static_assert(HV == 32 && HK == 32, "one 32-column TMEM load per thread and phase");
+            uint32_t v[32];
+            tmem_ld32(tmem + TM_ACC + lane_base + half * HV, v);
+            tmem_wait_ld();
+            if (live) {
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch) {
                     float fv[8];
-                    const uint32_t off = tile_chunk_off(64, t, cc);
+                    const uint32_t off = tile_chunk_off(64, t, half * 4 + ch);
                     unpack8(lds128(sm + Lo.V + off), fv);
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) fv[e] = bt * (fv[e] - __uint_as_float(v[e]));
+                    for (int e = 0; e < 8; ++e) fv[e] = bt * (fv[e] - __uint_as_float(v[8 * ch + e]));
                     sts128(sm + Lo.Y2 + off, pack8(fv));
                 }
             }
@@ -821,17 +822,16 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 14);
         // ---- P11: U -> bf16 rows (over V')
         if (krole && warp_active) {
-#pragma unroll 1
-            for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
-                uint32_t v[8];
-                tmem_ld8(tmem + TM_X1 + lane_base + 8 * cc, v);
-                tmem_wait_ld();
-                if (live) {
+            uint32_t v[32];
+            tmem_ld32(tmem + TM_X1 + lane_base + half * HV, v);
+            tmem_wait_ld();
+            if (live) {
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch) {
                     float f[8];
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[e]);
-                    const uint32_t off = tile_chunk_off(64, t, cc);
-                    sts128(sm + Lo.Us + off, pack8(f));
+                    for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[8 * ch + e]);
+                    sts128(sm + Lo.Us + tile_chunk_off(64, t, half * 4 + ch), pack8(f));
                 }
             }
         }
@@ -854,34 +854,36 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         // ---- P13: outputs and the state carry
         if (!krole && warp_active) {
             __nv_bfloat16* dst = a.O + ((tok0 + t) * a.H + h) * a.dvf + vofs;
-#pragma unroll 1
-            for (int cc = half * (HV / 8); cc < (half + 1) * (HV / 8); ++cc) {
-                uint32_t v[8];
-                tmem_ld8(tmem + TM_ACC + lane_base + 8 * cc, v);
-                tmem_wait_ld();
-                if (live) {
+            uint32_t v[32];
+            tmem_ld32(tmem + TM_ACC + lane_base + half * HV, v);
+            tmem_wait_ld();
+            if (live) {
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch) {
                     float f[8];
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) f[e] = a.scale * __uint_as_float(v[e]);
-                    *reinterpret_cast<uint4*>(dst + 8 * cc) = pack8(f);
+                    for (int e = 0; e < 8; ++e) f[e] = a.scale * __uint_as_float(v[8 * ch + e]);
+                    *reinterpret_cast<uint4*>(dst + 8 * (half * 4 + ch)) = pack8(f);
                 }
             }
         }
         if (q * 32 < DV) {
             const bool last_chunk = c + 1 == nchunks;
-#pragma unroll 1
-            for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
-                uint32_t sv[8], wv[8];
-                tmem_ld8(tmem + TM_S + lane_base + 8 * cc, sv);
-                tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, wv);
-                tmem_wait_ld();
+#pragma unroll
+            for (int s16 = 0; s16 < 2; ++s16) {
+              uint32_t sv16[16], wv16[16];
+              tmem_ld16(tmem + TM_S + lane_base + half * HK + 16 * s16, sv16);
+              tmem_ld16(tmem + TM_X2 + lane_base + half * HK + 16 * s16, wv16);
+              tmem_wait_ld();
+#pragma unroll
+              for (int c2 = 0; c2 < 2; ++c2) {
+                const int cc = half * (HK / 8) + 2 * s16 + c2;
                 float f[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    f[e] = __uint_as_float(sv[e]) * mi.gamL[8 * cc + e] + __uint_as_float(wv[e]);
-                    sv[e] = __float_as_uint(f[e]);
+                    f[e] = __uint_as_float(sv16[8 * c2 + e]) * mi.gamL[8 * cc + e] + __uint_as_float(wv16[8 * c2 + e]);
+                    sv16[8 * c2 + e] = __float_as_uint(f[e]);
                 }
-                tmem_st8(tmem + TM_S + lane_base + 8 * cc, sv);
                 const uint4 w = pack8(f);
                 const uint32_t off = tile_chunk_off(DV, row, cc);
                 sts128(sm + Lo.Sb + off, w);
@@ -890,6 +892,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     *reinterpret_cast<float4*>(dst) = make_float4(f[0], f[1], f[2], f[3]);
                     *reinterpret_cast<float4*>(dst + 4) = make_float4(f[4], f[5], f[6], f[7]);
                 }
+              }
+              tmem_st16(tmem + TM_S + lane_base + half * HK + 16 * s16, sv16);
             }
             tmem_wait_st();
         }
