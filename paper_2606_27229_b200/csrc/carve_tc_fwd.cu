@@ -467,12 +467,15 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         //      half of the part's columns and do the erase side (log a) and the write side (V' = w v) for them.
         if (warp_active) {
             const int cc0 = half * (HK / 8) + (krole ? 0 : HK / 16);
-#pragma unroll 1
-            for (int cc = cc0; cc < cc0 + HK / 16; ++cc) {
-                uint32_t pr[8], pw[8];
-                tmem_ld8(tmem + TM_X1 + lane_base + 8 * cc, pr);
-                tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, pw);
-                tmem_wait_ld();
+            uint32_t pr16[16], pw16[16];
+            tmem_ld16(tmem + TM_X1 + lane_base + 8 * cc0, pr16);
+            tmem_ld16(tmem + TM_X2 + lane_base + 8 * cc0, pw16);
+            tmem_wait_ld();
+#pragma unroll
+            for (int ci = 0; ci < HK / 16; ++ci) {
+                const int cc = cc0 + ci;
+                const uint32_t* pr = pr16 + 8 * ci;
+                const uint32_t* pw = pw16 + 8 * ci;
                 if (live) {
                     const uint32_t off = tile_chunk_off(64, t, cc);
                     {
