@@ -76,7 +76,7 @@ size_t tc_record_bytes(const carve_params_t& p);
 // Workspace of the tensor path (byte offsets): chunk records, final-state tiles, per-chain weight-gradient
 // partials (layout of part_stride_of) and per-chunk dA/dtau partials.
 struct TcWsLayout {
-    size_t rec, sfin, part, partAT, dgs, total_bytes;
+    size_t rec, sfin, part, partAT, dgs, flags, total_bytes;
     int part_stride;
 };
 inline TcWsLayout tc_ws_layout(const carve_params_t& p)
@@ -93,6 +93,7 @@ inline TcWsLayout tc_ws_layout(const carve_params_t& p)
     w.part = take(chains * (size_t)w.part_stride * sizeof(float));
     w.partAT = take(chains * nchunks * 2 * p.dk * sizeof(float));
     w.dgs = take(chains * (size_t)p.dk * 32 * sizeof(float));
+    w.flags = take(chains * sizeof(int));   // chunks finished per chain (reverse kernel -> overlapped epilogue)
     w.total_bytes = off;
     return w;
 }

@@ -48,6 +48,7 @@ struct BwdArgs {
     float* part;
     int part_stride;
     float* dgs;   // [chains][dk][32] dG^T of the later solve chunk of a gate chunk (L = 128)
+    int* flags;   // [chains] number of chunks whose outputs are complete (read by the overlapped epilogue kernel)
 };
 
 // TMEM column map of the reverse kernel.
@@ -298,6 +299,9 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         mbar_expect_tx(&mi.bar_pt, 16384);
         bulk_g2s(sm + Lo.S[1], rec_chain + (size_t)c2 * Rc.total + Rc.PT, 16384, &mi.bar_pt);
     };
+    // The chunk-local epilogue kernel is launched behind this one with programmatic stream serialization: let it start
+    // now on the SMs this grid leaves idle; it follows the per-chain progress flags written below.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     bool first = true, first_glue = true;
     PROF_INIT();
     for (int it = 0, c = nchunks - 1; c >= 0; --c, ++it) {
@@ -940,6 +944,10 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         // ---- L10: the adjoint of the state entering the chunk
         PROF(g_prof_bwd, 11);
         finalize(true, c == 0);
+        if (tid == 0) {   // every output row of this chunk was stored before the barrier inside finalize: publish it
+            __threadfence();
+            asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.flags + chain), "r"(nchunks - c) : "memory");
+        }
         PROF(g_prof_bwd, 12);
         first = false;
     }
@@ -974,13 +982,24 @@ __global__ void __launch_bounds__(256)
 carve_bwd_tc_epilogue_kernel(const __nv_bfloat16* __restrict__ gq, const __nv_bfloat16* __restrict__ gk,
                              const __nv_bfloat16* __restrict__ gf, const float* __restrict__ A,
                              const float* __restrict__ tau, __nv_bfloat16* dq, __nv_bfloat16* dk, __nv_bfloat16* df,
-                             float* __restrict__ partAT, int T, int H, int LCc, int l2norm, float eps)
+                             float* __restrict__ partAT, int T, int H, int LCc, int l2norm, float eps, const int* flags,
+                             int chains)
 {
     constexpr int V = D / 32;   // channels per lane
     __shared__ float red[8][2][D];
     const int nchunks = T / LCc;
-    const int chain = blockIdx.x / nchunks, c = blockIdx.x % nchunks, b = chain / H, h = chain % H;
+    // blocks in the order the reverse kernel finishes chunks (last chunk of every chain first): this grid may already
+    // run, on idle SMs, while the reverse kernel works; a block waits for "its" chunk through the chain's progress flag
+    const int c = nchunks - 1 - (int)(blockIdx.x / chains), chain = blockIdx.x % chains, b = chain / H, h = chain % H;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        int done;
+        do {
+            asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(done) : "l"(flags + chain) : "memory");
+            if (done < nchunks - c) __nanosleep(256);
+        } while (done < nchunks - c);
+    }
+    __syncthreads();
     float eA[V], ta[V], accA[V], accT[V];
 #pragma unroll
     for (int e = 0; e < V; ++e) {
@@ -1051,7 +1070,7 @@ carve_bwd_tc_epilogue_kernel(const __nv_bfloat16* __restrict__ gq, const __nv_bf
         float s = 0.f;
 #pragma unroll
         for (int w = 0; w < 8; ++w) s += red[w][i / D][i % D];
-        partAT[(size_t)blockIdx.x * 2 * D + i] = s;
+        partAT[((size_t)chain * nchunks + c) * 2 * D + i] = s;
     }
 }
 
@@ -1084,19 +1103,34 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
     t.dbeta = static_cast<__nv_bfloat16*>(a.dbeta); t.dS0 = a.dS0;
     t.part = reinterpret_cast<float*>(ws + w.part); t.part_stride = w.part_stride;
     t.dgs = reinterpret_cast<float*>(ws + w.dgs);
+    t.flags = reinterpret_cast<int*>(ws + w.flags);
     const size_t smem = BLayout(D).total;
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
     auto kern = carve_bwd_tc_kernel<D, NP>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int chains = a.B * a.H, nchunks = a.T / LCc;
+    if ((e = cudaMemsetAsync(t.flags, 0, (size_t)chains * sizeof(int), st)) != cudaSuccess) return e;
     kern<<<chains, 128 * NP, smem, st>>>(t, mdO, mk, mq);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     float* partAT = reinterpret_cast<float*>(ws + w.partAT);
-    carve_bwd_tc_epilogue_kernel<D><<<chains * nchunks, 256, 0, st>>>(
-        static_cast<const __nv_bfloat16*>(a.q), static_cast<const __nv_bfloat16*>(a.k),
-        static_cast<const __nv_bfloat16*>(a.f), a.A, a.tau, t.dq, t.dk, t.df, partAT, a.T, a.H, LCc, a.l2norm, a.eps);
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    {
+        // programmatic stream serialization: the epilogue grid may be scheduled while the reverse kernel is still running
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3((unsigned)(chains * nchunks));
+        cfg.blockDim = dim3(256);
+        cfg.dynamicSmemBytes = 0;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, carve_bwd_tc_epilogue_kernel<D>, static_cast<const __nv_bfloat16*>(a.q),
+                               static_cast<const __nv_bfloat16*>(a.k), static_cast<const __nv_bfloat16*>(a.f), a.A, a.tau, t.dq,
+                               t.dk, t.df, partAT, a.T, a.H, LCc, a.l2norm, a.eps, (const int*)t.flags, chains);
+        if (e != cudaSuccess) return e;
+    }
     const int nW = 2 * a.r * D + 2 * D * a.r;
     carve_reduce_at_kernel<<<chains, 2 * D, 0, st>>>(partAT, t.part, nchunks, w.part_stride, nW, D);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
