@@ -175,8 +175,7 @@ __device__ __forceinline__ void warp_colsum(float (&v)[N], int lane)
 // NP = column parts per tile row = warpgroups per CTA (threads = 128 NP): 32 columns per thread.
 template <int D, int NP>
 __global__ void __launch_bounds__(128 * NP, 1)
-carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, const __grid_constant__ CUtensorMap mk,
-                    const __grid_constant__ CUtensorMap mq)
+carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, const __grid_constant__ CUtensorMap mq)
 {
     constexpr int NTH = 128 * NP;
     constexpr int HK = D / NP;                     // columns per warpgroup ("half" = part index 0..NP-1)
@@ -210,7 +209,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         mbar_init(&mi.bar_g4a, 1); mbar_init(&mi.bar_g4b, 1); mbar_init(&mi.bar_g5, 1); mbar_init(&mi.bar_g8, 1);
         mbar_init(&mi.bar_fi, 1); mbar_init(&mi.bar_bg, 1); mbar_init(&mi.bar_pt, 1);
         mbar_fence_init();
-        tma_prefetch_desc(&mdO); tma_prefetch_desc(&mk); tma_prefetch_desc(&mq);
+        tma_prefetch_desc(&mdO); tma_prefetch_desc(&mq);
     }
     if (warp == 0) tmem_alloc(&mi.tmem_base, TM_COLS);
     for (int i = tid; i < 32 * D; i += NTH) {
@@ -1089,9 +1088,8 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
                           float* dVb, float* dVw, cudaStream_t st)
 {
     const int LCc = a.L < tcp::LC ? a.L : tcp::LC;
-    CUtensorMap mdO, mk, mq;
-    if (!tc_make_token_map(&mdO, a.dO, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mk, a.k, a.B, a.T, a.H, D, LCc) ||
-        !tc_make_token_map(&mq, a.q, a.B, a.T, a.H, D, LCc))
+    CUtensorMap mdO, mq;
+    if (!tc_make_token_map(&mdO, a.dO, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mq, a.q, a.B, a.T, a.H, D, LCc))
         return cudaErrorInvalidValue;
     BwdArgs t{};
     t.B = a.B; t.H = a.H; t.T = a.T; t.L = a.L; t.r = a.r; t.l2norm = a.l2norm; t.scale = a.scale; t.eps = a.eps;
@@ -1111,7 +1109,7 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
     if (e != cudaSuccess) return e;
     const int chains = a.B * a.H, nchunks = a.T / LCc;
     if ((e = cudaMemsetAsync(t.flags, 0, (size_t)chains * sizeof(int), st)) != cudaSuccess) return e;
-    kern<<<chains, 128 * NP, smem, st>>>(t, mdO, mk, mq);
+    kern<<<chains, 128 * NP, smem, st>>>(t, mdO, mq);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     float* partAT = reinterpret_cast<float*>(ws + w.partAT);
     {

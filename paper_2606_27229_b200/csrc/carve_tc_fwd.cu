@@ -619,6 +619,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         for (int e = 0; e < 8; ++e) { qv[e] *= rnq; kv[e] *= rnkn; }
                         if (has_next && bn > blk) {  // first row of its block
                             sts128(ver_row(bn, false, tn, cc), pack8(kv));
+                            if (rc && (bn & 1)) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = pack8(kv);
                         }
                         if (rc) *reinterpret_cast<uint4*>(rc + Rc.FQ + rp_off(t, cc)) = pack8(Fp);
 #pragma unroll
@@ -628,6 +629,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                                 for (int e = 0; e < 8; ++e) o[e] = qv[e] * Fp[e];
                                 const uint4 wq = pack8(o);
                                 sts128(ver_row(jb, true, t, cc), wq);
+                                if (rc && jb == blk && (blk & 1)) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, 64 + t, cc)) = wq;
                                 if (rc && jb == 0 && !s1) {
 #pragma unroll
                                     for (int e = 0; e < 8; ++e) o[e] *= a.scale;
@@ -638,6 +640,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                                     for (int e = 0; e < 8; ++e) o[e] = kv[e] * Fp[e];
                                     const uint4 wk = pack8(o);
                                     sts128(ver_row(jb, false, tn, cc), wk);
+                                    if (rc && jb == blk && bn == blk && (blk & 1))
+                                        *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = wk;
                                 }
                                 if (jb > 0) {
                                     const float4 e0 = *reinterpret_cast<const float4*>(&mi.etot[jb - 1][8 * cc]);
@@ -664,35 +668,30 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             if (nb > 2) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 32, 16, sb + Lo.Y0, 64, 0, sb + Lo.Y1, 64, 32, DK, false);
             if (nb > 3) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 48, 16, sb + Lo.Y2 + tile_bytes(96, DK), 32, 0, sb + Lo.Y1, 64, 48, DK, false);
             mma_rt<128, KMAJ, KMAJ>(tmem + TM_ACC, DV, sb + Lo.KQbar, 128, 0, sb + Lo.Sb, DV, 0, DK, false);
+            umma_commit(&mi.bar_mma);
             if (rc) {
-                // record: operand tiles straight from shared memory (bulk copies, no thread stores).  The sources are
-                // rewritten from P9a on: thread 0 waits for the copies to have read them before the barrier there.
+                // record: operand tiles straight from shared memory (bulk copies).  Only sources that stay intact until
+                // the wait in P12 are used: Ktil, C, version 0 (Kbar/Qbar) and version 2 (Y0).  The rows of the odd
+                // 16-token blocks (versions 1 and 3 live in Y2/TP, rewritten in P9) were stored by their threads in P7b.
                 constexpr uint32_t TB = tile_bytes(64, DK);
                 bulk_s2g(rc + Rc.KT, sb + Lo.Ktil, TB);
                 bulk_s2g(rc + Rc.CC, sb + Lo.Y1, TB);
                 for (int cb = 0; cb < DK / 64; ++cb) {
                     bulk_s2g(rc + Rc.K0 + cb * 8192, sb + Lo.KQbar + cb * 16384, 8192);                  // Kbar rows
                     if (s1) bulk_s2g(rc + Rc.Q0 + cb * 8192, sb + Lo.KQbar + cb * 16384 + 8192, 8192);   // Qbar rows
-                    // rows anchored at their own block: the 16 K-side and 16 Q-side rows of block jb in version jb
-                    const uint32_t vt[4] = {sb + Lo.KQbar, sb + Lo.Y2, sb + Lo.Y0, sb + Lo.Y2 + tile_bytes(96, DK)};
-                    const uint32_t vstride[4] = {128 * 128, 96 * 128, 64 * 128, 32 * 128};   // column-block strides
-                    const uint32_t vq[4] = {64 * 128, 48 * 128, 32 * 128, 16 * 128};         // first Q-side row
-                    for (int jb = 0; jb < nb; ++jb) {
-                        uint8_t* dst = rc + Rc.KQo + cb * 16384 + jb * 2048;
-                        bulk_s2g(dst, vt[jb] + cb * vstride[jb], 2048);
-                        bulk_s2g(dst + 8192, vt[jb] + cb * vstride[jb] + vq[jb], 2048);
+                    uint8_t* dst = rc + Rc.KQo + cb * 16384;
+                    bulk_s2g(dst, sb + Lo.KQbar + cb * 16384, 2048);                 // block 0, K side (version 0)
+                    bulk_s2g(dst + 8192, sb + Lo.KQbar + cb * 16384 + 8192, 2048);   // block 0, Q side
+                    if (nb > 2) {
+                        bulk_s2g(dst + 4096, sb + Lo.Y0 + cb * 8192, 2048);                  // block 2, K side (version 2)
+                        bulk_s2g(dst + 8192 + 4096, sb + Lo.Y0 + cb * 8192 + 4096, 2048);    // block 2, Q side
                     }
                 }
                 bulk_commit();
             }
-            umma_commit(&mi.bar_mma);
         }
         WAIT_MMA();
         if (VS > 1) cluster_arrive();   // C (Y1) is consumed: the peer may send the next chunk's partial G
-        if (rc) {   // the version tiles (Y2 and, at d = 128, the TP region behind it) still feed the record's bulk copies
-            if (tid == 0) bulk_wait_read();
-            __syncthreads();
-        }
         PROF(g_prof_fwd, 10);
         // ---- P9a: beta A -> Mm (fp32, only the strictly lower part is ever read), P -> TP rows 64.. (bf16, masked s <= t)
         {
