@@ -101,28 +101,55 @@ __device__ __forceinline__ void warp_store(float* Q, int qr, int qc, const float
 }
 
 // Tm <- (I + Mm)^-1 for the leading n x n block (n in {16,32,64}); Mm strictly lower (only that part is read).
-// Blocked forward substitution (Alg. 2 step 7): 16x16 diagonal blocks by substitution, then
+// Blocked forward substitution (Alg. 2 step 7): 8x8 diagonal blocks by substitution, 16x16 blocks by fp32 FMA, then
 // T_ij = -T_ii (M_ij T_jj) one level at a time, the block products on tensor cores (tf32 mma.sync).
 __device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid, int nthreads)
 {
     const int warp = tid >> 5, lane = tid & 31;
+    // step 1a: 8x8 diagonal sub-blocks by forward substitution (thread = sub-block, column), zero above the diagonal
     if (tid < n) {
-        const int blk = tid >> 4, c = tid & 15, o = 16 * blk;
-        float x[16];
+        const int c = tid & 7, o = 8 * (tid >> 3);
+        float x[8];
 #pragma unroll
-        for (int tt = 0; tt < 16; ++tt) {
+        for (int tt = 0; tt < 8; ++tt) {
             float acc = 0.f;
 #pragma unroll
             for (int s = 0; s < tt; ++s) acc += Mm[mm_idx(o + tt, o + s)] * x[s];
             x[tt] = (tt == c) ? 1.f : (tt < c ? 0.f : -acc);
             Tm[mm_idx(o + tt, o + c)] = x[tt];
         }
+    } else if (tid < 2 * n) {
+        // the upper-right 8x8 block of every 16-block is zero
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int idx = 4 * (tid - n) + e, blk = idx >> 6, rr = (idx >> 3) & 7, cc = idx & 7;
+            Tm[mm_idx(16 * blk + rr, 16 * blk + 8 + cc)] = 0.f;
+        }
     } else if (n >= 64) {
         // blocks (0,1) and (2,3) of T are zero; the level-64 products read them
-        for (int i = tid - 64; i < 512; i += nthreads - 64) {
+        for (int i = tid - 2 * n; i < 512; i += nthreads - 2 * n) {
             const int blk = i >> 8, rr = (i >> 4) & 15, cc = i & 15;
             Tm[mm_idx(32 * blk + rr, 32 * blk + 16 + cc)] = 0.f;
         }
+    }
+    __syncthreads();
+    // step 1b: lower-left 8x8 block of every 16-block, T21 = -T22 (M21 T11), one element per thread (fp32 FMA)
+    {
+        const bool act = tid < 4 * n;
+        const int o = 16 * (tid >> 6), i = (tid >> 3) & 7, j = tid & 7;
+        float xv = 0.f, yv = 0.f;
+        if (act) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) xv += Mm[mm_idx(o + 8 + i, o + k)] * Tm[mm_idx(o + k, o + j)];
+            Tm[mm_idx(o + 8 + i, o + j)] = xv;   // X = M21 T11 (these entries are read only below)
+        }
+        __syncthreads();
+        if (act) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) yv += Tm[mm_idx(o + 8 + i, o + 8 + k)] * Tm[mm_idx(o + 8 + k, o + j)];
+        }
+        __syncthreads();
+        if (act) Tm[mm_idx(o + 8 + i, o + j)] = -yv;
     }
     __syncthreads();
     if (n >= 32) {
