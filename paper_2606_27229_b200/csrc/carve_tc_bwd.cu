@@ -832,6 +832,14 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mma_k<MNMAJ, MNMAJ>(tmem + BM_WG, 32, sb + Lo.S[2], 128, 0, 64, sb + Lo.S[1], 128, 0, 64, LCc, true);
             umma_commit(&mi.bar_mma);
         }
+        if (c > 0 && live) {   // next chunk's row-private L2 inputs -> L2 cache, so that the loads at its top are short
+            const uint8_t* rn_ = rc - Rc.total;
+#pragma unroll
+            for (int i = 0; i < QW / 8; ++i) {
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(rn_ + Rc.VWX + rp_off(t, cq0 + i)));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(rn_ + Rc.W + rp_off(t, cq0 + i)));
+            }
+        }
         WAIT_MMA();
         if (half == 0 && warp_active) {
             // dz = ZZ (1 - tt^2): K side owns the erase half (cols 0..r), Q side the write half (cols r..2r)
