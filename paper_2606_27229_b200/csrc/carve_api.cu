@@ -148,13 +148,12 @@ carve_status_t carve_fwd(const carve_params_t* p, const void* q, const void* k, 
     a.A = A; a.tau = tau; a.Ub = Ub; a.Uw = Uw; a.Vb = Vb; a.Vw = Vw; a.S0 = S0;
     a.O = O; a.S_final = S_final;
     if (path == CARVE_PATH_TENSOR) {
-        uint8_t *rec = nullptr, *sfin = nullptr;
+        uint8_t* rec = nullptr;
         if (workspace) {
             const TcWsLayout w = tc_ws_layout(*p);
             rec = static_cast<uint8_t*>(workspace) + w.rec;
-            sfin = static_cast<uint8_t*>(workspace) + w.sfin;
         }
-        return tc_fwd_launch(a, rec, sfin, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess ? CARVE_OK : CARVE_ERR_CUDA;
+        return tc_fwd_launch(a, rec, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess ? CARVE_OK : CARVE_ERR_CUDA;
     }
     fill_ws(a, *p, workspace);
     return simt_fwd_launch(a, p->dtype, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess ? CARVE_OK

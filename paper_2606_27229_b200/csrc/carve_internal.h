@@ -73,10 +73,10 @@ bool tc_bwd_supported(const carve_params_t& p);
 size_t tc_state_tile_bytes(const carve_params_t& p);
 size_t tc_record_bytes(const carve_params_t& p);
 
-// Workspace of the tensor path (byte offsets): chunk records, final-state tiles, per-chain weight-gradient
+// Workspace of the tensor path (byte offsets): chunk records, per-chain weight-gradient
 // partials (layout of part_stride_of) and per-chunk dA/dtau partials.
 struct TcWsLayout {
-    size_t rec, sfin, part, partAT, dgs, flags, total_bytes;
+    size_t rec, part, partAT, dgs, flags, total_bytes;
     int part_stride;
 };
 inline TcWsLayout tc_ws_layout(const carve_params_t& p)
@@ -88,7 +88,6 @@ inline TcWsLayout tc_ws_layout(const carve_params_t& p)
     size_t off = 0;
     auto take = [&](size_t n) { size_t o = off; off += (n + 1023) & ~(size_t)1023; return o; };
     w.rec = take(chains * nchunks * tc_record_bytes(p));
-    w.sfin = take(chains * tc_state_tile_bytes(p));
     w.part_stride = part_stride_of(p.dk, p.dv, p.r);
     w.part = take(chains * (size_t)w.part_stride * sizeof(float));
     w.partAT = take(chains * nchunks * 2 * p.dk * sizeof(float));
@@ -99,7 +98,7 @@ inline TcWsLayout tc_ws_layout(const carve_params_t& p)
 }
 
 // rec / sfin: workspace views (nullptr for an inference forward).
-cudaError_t tc_fwd_launch(const Args& a, uint8_t* rec, uint8_t* sfin, cudaStream_t st);
+cudaError_t tc_fwd_launch(const Args& a, uint8_t* rec, cudaStream_t st);
 cudaError_t tc_bwd_launch(const Args& a, uint8_t* ws, const TcWsLayout& w, float* dA, float* dtau, float* dUb,
                           float* dUw, float* dVb, float* dVw, cudaStream_t st);
 

@@ -40,7 +40,6 @@ struct BwdArgs {
     int l2norm;
     float scale, eps;
     const uint8_t* rec;
-    const uint8_t* sfin;
     const float* dS_final;
     const float *Ub, *Uw, *Vb, *Vw;
     __nv_bfloat16 *dq, *dk, *dv, *df, *dbx, *dwx, *dbeta;
@@ -1101,7 +1100,7 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
         return cudaErrorInvalidValue;
     BwdArgs t{};
     t.B = a.B; t.H = a.H; t.T = a.T; t.L = a.L; t.r = a.r; t.l2norm = a.l2norm; t.scale = a.scale; t.eps = a.eps;
-    t.rec = ws + w.rec; t.sfin = ws + w.sfin; t.dS_final = a.dS_final;
+    t.rec = ws + w.rec; t.dS_final = a.dS_final;
     t.Ub = a.Ub; t.Uw = a.Uw; t.Vb = a.Vb; t.Vw = a.Vw;
     t.dq = static_cast<__nv_bfloat16*>(a.dq); t.dk = static_cast<__nv_bfloat16*>(a.dk_);
     t.dv = static_cast<__nv_bfloat16*>(a.dv_); t.df = static_cast<__nv_bfloat16*>(a.df);

@@ -39,7 +39,6 @@ struct TcArgs {
     __nv_bfloat16* O;
     float* S_final;
     uint8_t* rec;   // [chains][T/LC] chunk records (carve_tc.cuh Rec) for the reverse kernel, or nullptr
-    uint8_t* sfin;  // [chains] bf16 row tile of the final state (the reverse kernel's first "next state")
 };
 
 // Runtime-shaped product from two row tiles (see tc_common.cuh umma_tiles_rt); M fixed at compile time.
@@ -931,11 +930,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     }
     if (VS > 1) cluster_wait();   // pairs with the last arrive; also keeps this CTA's shared memory alive for the peer
     PHASE_SYNC();
-    if (rec_chain && tid == 0) {   // the final state as the reverse kernel's operand tile; drain every bulk store
-        bulk_s2g(a.sfin + (size_t)chain * state_tile, sb + Lo.Sb, (uint32_t)state_tile);
-        bulk_commit();
-        bulk_wait_all();
-    }
+    if (rec_chain && tid == 0) bulk_wait_all();   // drain the record's bulk stores
     if (warp == 0) tmem_dealloc(tmem, TM_COLS);
 }
 
@@ -994,7 +989,7 @@ size_t tc_state_tile_bytes(const carve_params_t& p) { return tc::tile_bytes(p.dv
 size_t tc_record_bytes(const carve_params_t& p) { return tcp::Rec(p.dk, p.dv).total; }
 
 template <int D, int VS>
-static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, uint8_t* sfin, cudaStream_t st)
+static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
 {
     const int LCc = a.L < tcp::LC ? a.L : tcp::LC;
     CUtensorMap mq, mk, mv, mf, mbx, mwx;
@@ -1007,7 +1002,7 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, uint8_t* sfin, cud
     t.dvf = a.dv;
     t.beta = static_cast<const __nv_bfloat16*>(a.beta);
     t.A = a.A; t.tau = a.tau; t.Ub = a.Ub; t.Uw = a.Uw; t.Vb = a.Vb; t.Vw = a.Vw; t.S0 = a.S0;
-    t.O = static_cast<__nv_bfloat16*>(a.O); t.S_final = a.S_final; t.rec = rec; t.sfin = sfin;
+    t.O = static_cast<__nv_bfloat16*>(a.O); t.S_final = a.S_final; t.rec = rec;
     const size_t smem = tcp::Layout(D, D, 2 * a.r).total;
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
     auto kern = carve_fwd_tc_kernel<D, D, NP, VS>;
@@ -1026,11 +1021,11 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, uint8_t* sfin, cud
     return cudaLaunchKernelEx(&cfg, kern, t, mq, mk, mv, mf, mbx, mwx);
 }
 
-cudaError_t tc_fwd_launch(const Args& a, uint8_t* rec, uint8_t* sfin, cudaStream_t st)
+cudaError_t tc_fwd_launch(const Args& a, uint8_t* rec, cudaStream_t st)
 {
-    if (a.dk == 128 && a.dv == 256) return launch_tc_fwd<128, 2>(a, rec, sfin, st);   // inference only: two CTAs per chain
-    if (a.dk == 128) return launch_tc_fwd<128, 1>(a, rec, sfin, st);
-    if (a.dk == 64) return launch_tc_fwd<64, 1>(a, rec, sfin, st);
+    if (a.dk == 128 && a.dv == 256) return launch_tc_fwd<128, 2>(a, rec, st);   // inference only: two CTAs per chain
+    if (a.dk == 128) return launch_tc_fwd<128, 1>(a, rec, st);
+    if (a.dk == 64) return launch_tc_fwd<64, 1>(a, rec, st);
     return cudaErrorInvalidValue;
 }
 
