@@ -494,6 +494,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mbar_expect_tx(&mi.bar_fi, 2 * TB);
             bulk_g2s(sm + Lo.FI, rc + Rc.FQ, TB, &mi.bar_fi);
             bulk_g2s(sm + Lo.FI + TB, rc + Rc.IC, TB, &mi.bar_fi);
+            // the erase gate b follows into the same buffer at L6: have it in L2 by then
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rc + Rc.Bg), "r"(TB) : "memory");
         }
         if (tid < D) {
             float sx = 0.f;
@@ -838,6 +840,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(rn_ + Rc.VWX + rp_off(t, cq0 + i)));
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(rn_ + Rc.W + rp_off(t, cq0 + i)));
             }
+            if (!krole && half < 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(rn_ + Rc.tt + t * 64));
         }
         WAIT_MMA();
         if (half == 0 && warp_active) {
