@@ -125,8 +125,12 @@ size_t carve_host_arena_bytes(const carve_params_t *p, int with_bwd);
 /*
  * One forward (+ backward when with_bwd != 0) with HOST tensors: copies the inputs to the device
  * arena, runs carve_fwd (and carve_bwd with the host cotangents dO, dS_final), copies O, S_final
- * and the gradients back, all enqueued on `cuda_stream`.  Host buffers should be pinned for the
- * copies to be asynchronous.  Pointer meanings and NULL rules are those of carve_fwd / carve_bwd;
+ * and the gradients back.  The batch is cut into up to 8 slices (the largest divisor of B that is <= 8), each
+ * run on a short-lived stream of its own forked from and joined back into `cuda_stream`, so that copy-in,
+ * kernels and copy-out of different slices overlap; work enqueued on `cuda_stream` before the call precedes
+ * it, work enqueued after the call follows it.  The shared-weight gradients are the sums of the slices'
+ * (fixed order: deterministic, but rounded differently from one carve_bwd over the whole batch).  Host
+ * buffers should be pinned for the copies to be asynchronous.  Pointer meanings and NULL rules are those of carve_fwd / carve_bwd;
  * when with_bwd == 0 the cotangent and gradient pointers are ignored.
  */
 carve_status_t carve_fwd_bwd_host(const carve_params_t *p, int with_bwd, const void *q, const void *k,

@@ -82,6 +82,17 @@ size_t elt(const carve_params_t* p) { return p->dtype == CARVE_BF16 ? 2 : 4; }
 
 using namespace carve;
 
+// out[i] = sum over slices s (ascending) of in[s * stride + i]   (carve_fwd_bwd_host: shared-weight gradients)
+static __global__ void carve_sum_slices_kernel(float* __restrict__ out, const float* __restrict__ in, int n, int ns,
+                                               size_t stride)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float acc = 0.f;
+    for (int s = 0; s < ns; ++s) acc += in[s * stride + i];
+    out[i] = acc;
+}
+
 extern "C" {
 
 const char* carve_version(void) { return "carve-b200 0.1 (sm_100a)"; }
@@ -160,12 +171,15 @@ carve_status_t carve_fwd(const carve_params_t* p, const void* q, const void* k, 
                                                                                               : CARVE_ERR_CUDA;
 }
 
-carve_status_t carve_bwd(const carve_params_t* p, const void* q, const void* k, const void* v, const void* f,
-                         const void* bx, const void* wx, const void* beta, const float* A, const float* tau,
-                         const float* Ub, const float* Uw, const float* Vb, const float* Vw, const float* S0,
-                         const void* dO, const float* dS_final, void* dq, void* dk, void* dv, void* df, void* dbx,
-                         void* dwx, void* dbeta, float* dA, float* dtau, float* dUb, float* dUw, float* dVb,
-                         float* dVw, float* dS0, void* workspace, size_t workspace_bytes, void* cuda_stream)
+// carve_bwd; `epilogue_after`: the tensor path launches its chunk-local epilogue as a plain dependent kernel
+// instead of overlapping it with the reverse kernel (see Args::epilogue_after).
+static carve_status_t bwd_impl(const carve_params_t* p, const void* q, const void* k, const void* v, const void* f,
+                               const void* bx, const void* wx, const void* beta, const float* A, const float* tau,
+                               const float* Ub, const float* Uw, const float* Vb, const float* Vw, const float* S0,
+                               const void* dO, const float* dS_final, void* dq, void* dk, void* dv, void* df, void* dbx,
+                               void* dwx, void* dbeta, float* dA, float* dtau, float* dUb, float* dUw, float* dVb,
+                               float* dVw, float* dS0, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                               bool epilogue_after)
 {
     carve_status_t s = check_params(p, true);
     if (s != CARVE_OK) return s;
@@ -191,6 +205,7 @@ carve_status_t carve_bwd(const carve_params_t* p, const void* q, const void* k, 
     a.A = A; a.tau = tau; a.Ub = Ub; a.Uw = Uw; a.Vb = Vb; a.Vw = Vw; a.S0 = S0;
     a.dO = dO; a.dS_final = dS_final;
     a.dq = dq; a.dk_ = dk; a.dv_ = dv; a.df = df; a.dbx = dbx; a.dwx = dwx; a.dbeta = dbeta; a.dS0 = dS0;
+    a.epilogue_after = epilogue_after;
     if (path == CARVE_PATH_TENSOR)
         return tc_bwd_launch(a, static_cast<uint8_t*>(workspace), tc_ws_layout(*p), dA, dtau, dUb, dUw, dVb, dVw,
                              static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess
@@ -203,10 +218,26 @@ carve_status_t carve_bwd(const carve_params_t* p, const void* q, const void* k, 
                : CARVE_ERR_CUDA;
 }
 
+carve_status_t carve_bwd(const carve_params_t* p, const void* q, const void* k, const void* v, const void* f,
+                         const void* bx, const void* wx, const void* beta, const float* A, const float* tau,
+                         const float* Ub, const float* Uw, const float* Vb, const float* Vw, const float* S0,
+                         const void* dO, const float* dS_final, void* dq, void* dk, void* dv, void* df, void* dbx,
+                         void* dwx, void* dbeta, float* dA, float* dtau, float* dUb, float* dUw, float* dVb,
+                         float* dVw, float* dS0, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    return bwd_impl(p, q, k, v, f, bx, wx, beta, A, tau, Ub, Uw, Vb, Vw, S0, dO, dS_final, dq, dk, dv, df, dbx, dwx, dbeta,
+                    dA, dtau, dUb, dUw, dVb, dVw, dS0, workspace, workspace_bytes, cuda_stream, false);
+}
+
 // ---- host-buffer entry point ---------------------------------------------------------------------
+// The batch is cut into up to 8 slices (chains are independent; [B,T,H,d] makes a batch slice one
+// contiguous slab of every token tensor).  Each slice runs copy-in -> carve_fwd -> carve_bwd -> copy-out on a
+// stream of its own, so the host->device copies of slice i+1, the kernels of slice i and the device->host
+// copies of slice i-1 overlap (PCIe is full duplex; the chains of all slices together still fill the SMs).
+// The weight gradients of the slices are summed in a fixed order by one small kernel.
 namespace {
 struct HostPlan {
-    size_t tok_k, tok_v, tok_1, st, w_u, w_vb, w_vw, w_a;  // byte sizes
+    size_t tok_k, tok_v, tok_1, st, w_u, w_vb, w_vw, w_a;  // byte sizes (token tensors and states: per slice)
 };
 HostPlan plan_of(const carve_params_t* p)
 {
@@ -223,23 +254,35 @@ HostPlan plan_of(const carve_params_t* p)
     return h;
 }
 size_t up256(size_t n) { return (n + 255) & ~(size_t)255; }
+int host_slices(const carve_params_t* p)
+{
+    int n = 1;
+    for (int d = 2; d <= 8; ++d)
+        if (p->B % d == 0) n = d;
+    return n;
+}
+size_t wgrad_floats(const carve_params_t* p) { return (size_t)2 * p->H * p->dk + 2 * p->r * p->dv + p->dk * p->r + p->dv * p->r; }
 }  // namespace
 
 size_t carve_host_arena_bytes(const carve_params_t* p, int with_bwd)
 {
     if (check_params(p, with_bwd != 0) != CARVE_OK) return 0;
-    const HostPlan h = plan_of(p);
-    size_t n = 0;
-    n += 4 * up256(h.tok_k) + 3 * up256(h.tok_v) + up256(h.tok_1);              // q,k,f,bx ; v,wx,O ; beta
-    n += 2 * up256(h.w_a) + 2 * up256(h.w_u) + up256(h.w_vb) + up256(h.w_vw);   // A,tau,Ub,Uw,Vb,Vw
-    n += 2 * up256(h.st);                                                        // S0, S_final
+    const int ns = host_slices(p);
+    carve_params_t ps = *p;
+    ps.B = p->B / ns;
+    const HostPlan h = plan_of(&ps);
+    size_t n = 0, per = 0;
+    n += 2 * up256(h.w_a) + 2 * up256(h.w_u) + up256(h.w_vb) + up256(h.w_vw);  // A,tau,Ub,Uw,Vb,Vw
+    per += 4 * up256(h.tok_k) + 3 * up256(h.tok_v) + up256(h.tok_1);           // q,k,f,bx ; v,wx,O ; beta
+    per += 2 * up256(h.st);                                                     // S0, S_final
     if (with_bwd) {
-        n += up256(h.tok_v) + up256(h.st);                                       // dO, dS_final
-        n += 4 * up256(h.tok_k) + 2 * up256(h.tok_v) + up256(h.tok_1);          // dq,dk,df,dbx ; dv,dwx ; dbeta
-        n += 2 * up256(h.w_a) + 2 * up256(h.w_u) + up256(h.w_vb) + up256(h.w_vw) + up256(h.st);
-        n += up256(carve_workspace_bytes(p, 1));
+        per += up256(h.tok_v) + up256(h.st);                                    // dO, dS_final
+        per += 4 * up256(h.tok_k) + 2 * up256(h.tok_v) + up256(h.tok_1);       // dq,dk,df,dbx ; dv,dwx ; dbeta
+        per += up256(h.st) + up256(wgrad_floats(p) * 4);                        // dS0, weight gradients of the slice
+        per += up256(carve_workspace_bytes(&ps, 1));
+        n += up256(wgrad_floats(p) * 4);                                        // summed weight gradients
     }
-    return n;
+    return n + per * ns;
 }
 
 carve_status_t carve_fwd_bwd_host(const carve_params_t* p, int with_bwd, const void* q, const void* k,
@@ -258,59 +301,127 @@ carve_status_t carve_fwd_bwd_host(const carve_params_t* p, int with_bwd, const v
     if (!q || !k || !v || !f || !bx || !wx || !beta || !Ub || !Uw || !Vb || !Vw || !O || !S_final) return CARVE_ERR_NULL;
     if (with_bwd && (!dO || !dq || !dk || !dv || !df || !dbx || !dwx || !dbeta || !dUb || !dUw || !dVb || !dVw || !dS0))
         return CARVE_ERR_NULL;
+    if (resolve_path(p, with_bwd != 0) < 0) return CARVE_ERR_SHAPE;
+    if ((s = check_arch()) != CARVE_OK) return s;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const HostPlan h = plan_of(p);
+    const int ns = host_slices(p);
+    carve_params_t ps = *p;
+    ps.B = p->B / ns;
+    const HostPlan h = plan_of(&ps);
     char* cur = static_cast<char*>(device_arena);
     bool ok = true;
-    auto up = [&](const void* src, size_t bytes) -> void* {  // host -> device copy into the arena
+    auto slot = [&](size_t bytes) -> void* { void* d = cur; cur += up256(bytes); return d; };
+    auto up = [&](const void* src, size_t bytes, cudaStream_t on) -> void* {  // host -> device copy into the arena
         if (!src) return nullptr;
-        void* d = cur;
-        cur += up256(bytes);
-        ok = ok && cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
+        void* d = slot(bytes);
+        ok = ok && cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, on) == cudaSuccess;
         return d;
     };
-    auto slot = [&](size_t bytes) -> void* { void* d = cur; cur += up256(bytes); return d; };
-
-    void *d_q = up(q, h.tok_k), *d_k = up(k, h.tok_k), *d_v = up(v, h.tok_v), *d_f = up(f, h.tok_k),
-         *d_bx = up(bx, h.tok_k), *d_wx = up(wx, h.tok_v), *d_beta = up(beta, h.tok_1);
-    float *d_A = (float*)up(A, h.w_a), *d_tau = (float*)up(tau, h.w_a), *d_Ub = (float*)up(Ub, h.w_u),
-          *d_Uw = (float*)up(Uw, h.w_u), *d_Vb = (float*)up(Vb, h.w_vb), *d_Vw = (float*)up(Vw, h.w_vw),
-          *d_S0 = (float*)up(S0, h.st);
-    void* d_O = slot(h.tok_v);
-    float* d_Sf = (float*)slot(h.st);
-    void* d_ws = nullptr;
-    size_t ws_bytes = 0;
-    if (with_bwd) {
-        ws_bytes = carve_workspace_bytes(p, 1);
-        d_ws = slot(ws_bytes);
-    }
-    if (!ok) return CARVE_ERR_CUDA;
-    s = carve_fwd(p, d_q, d_k, d_v, d_f, d_bx, d_wx, d_beta, d_A, d_tau, d_Ub, d_Uw, d_Vb, d_Vw, d_S0, d_O, d_Sf,
-                  d_ws, ws_bytes, cuda_stream);
-    if (s != CARVE_OK) return s;
-    auto down = [&](void* dst, const void* src, size_t bytes) {
-        if (dst) ok = ok && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+    auto down = [&](void* dst, const void* src, size_t bytes, cudaStream_t on) {
+        if (dst) ok = ok && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, on) == cudaSuccess;
     };
-    down(O, d_O, h.tok_v);
-    down(S_final, d_Sf, h.st);
-    if (with_bwd) {
-        void* d_dO = up(dO, h.tok_v);
-        float* d_dSf = (float*)up(dS_final, h.st);
-        void *d_dq = slot(h.tok_k), *d_dk = slot(h.tok_k), *d_df = slot(h.tok_k), *d_dbx = slot(h.tok_k),
-             *d_dv = slot(h.tok_v), *d_dwx = slot(h.tok_v), *d_dbeta = slot(h.tok_1);
-        float *d_dA = dA ? (float*)slot(h.w_a) : nullptr, *d_dtau = dtau ? (float*)slot(h.w_a) : nullptr;
-        float *d_dUb = (float*)slot(h.w_u), *d_dUw = (float*)slot(h.w_u), *d_dVb = (float*)slot(h.w_vb),
-              *d_dVw = (float*)slot(h.w_vw), *d_dS0 = (float*)slot(h.st);
-        if (!ok) return CARVE_ERR_CUDA;
-        s = carve_bwd(p, d_q, d_k, d_v, d_f, d_bx, d_wx, d_beta, d_A, d_tau, d_Ub, d_Uw, d_Vb, d_Vw, d_S0, d_dO,
-                      d_dSf, d_dq, d_dk, d_dv, d_df, d_dbx, d_dwx, d_dbeta, d_dA, d_dtau, d_dUb, d_dUw, d_dVb,
-                      d_dVw, d_dS0, d_ws, ws_bytes, cuda_stream);
-        if (s != CARVE_OK) return s;
-        down(dq, d_dq, h.tok_k); down(dk, d_dk, h.tok_k); down(df, d_df, h.tok_k); down(dbx, d_dbx, h.tok_k);
-        down(dv, d_dv, h.tok_v); down(dwx, d_dwx, h.tok_v); down(dbeta, d_dbeta, h.tok_1);
-        down(dA, d_dA, h.w_a); down(dtau, d_dtau, h.w_a); down(dUb, d_dUb, h.w_u); down(dUw, d_dUw, h.w_u);
-        down(dVb, d_dVb, h.w_vb); down(dVw, d_dVw, h.w_vw); down(dS0, d_dS0, h.st);
+    auto at = [](const void* base, size_t off) -> const char* { return base ? static_cast<const char*>(base) + off : nullptr; };
+    auto atw = [](void* base, size_t off) -> char* { return base ? static_cast<char*>(base) + off : nullptr; };
+
+    // shared weights, on the caller's stream, before the slices fork from it
+    float *d_A = (float*)up(A, h.w_a, st), *d_tau = (float*)up(tau, h.w_a, st), *d_Ub = (float*)up(Ub, h.w_u, st),
+          *d_Uw = (float*)up(Uw, h.w_u, st), *d_Vb = (float*)up(Vb, h.w_vb, st), *d_Vw = (float*)up(Vw, h.w_vw, st);
+    const size_t nwg = wgrad_floats(p);
+    float* d_wsum = with_bwd ? (float*)slot(nwg * 4) : nullptr;
+    float* d_wpart = nullptr;  // first slice's weight-gradient block; the others follow at a fixed byte stride
+    size_t wpart_stride = 0;
+
+    cudaStream_t side[8] = {};
+    cudaEvent_t fork = nullptr, join[8] = {}, arrived[8] = {};  // arrived[i]: slice i's host -> device copies done
+    ok = ok && cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaEventRecord(fork, st) == cudaSuccess;
+    for (int i = 0; i < ns && ok; ++i) {
+        if (ns > 1) {
+            ok = ok && cudaStreamCreateWithFlags(&side[i], cudaStreamNonBlocking) == cudaSuccess;
+            ok = ok && cudaEventCreateWithFlags(&join[i], cudaEventDisableTiming) == cudaSuccess;
+            ok = ok && cudaEventCreateWithFlags(&arrived[i], cudaEventDisableTiming) == cudaSuccess;
+            ok = ok && cudaStreamWaitEvent(side[i], fork, 0) == cudaSuccess;
+        } else {
+            side[i] = st;
+        }
     }
+    carve_status_t rs = CARVE_OK;
+    for (int i = 0; i < ns && ok && rs == CARVE_OK; ++i) {
+        cudaStream_t ss = side[i];
+        // copies of different streams may run on different copy engines and share the link: keep the slices'
+        // uploads in order, so that slice i is complete (and its kernels start) after (i+1)/ns of the transfer
+        if (ns > 1 && i > 0) ok = ok && cudaStreamWaitEvent(ss, arrived[i - 1], 0) == cudaSuccess;
+        const size_t okk = (size_t)i * h.tok_k, ov = (size_t)i * h.tok_v, o1 = (size_t)i * h.tok_1, os = (size_t)i * h.st;
+        void *d_q = up(at(q, okk), h.tok_k, ss), *d_k = up(at(k, okk), h.tok_k, ss), *d_v = up(at(v, ov), h.tok_v, ss),
+             *d_f = up(at(f, okk), h.tok_k, ss), *d_bx = up(at(bx, okk), h.tok_k, ss), *d_wx = up(at(wx, ov), h.tok_v, ss),
+             *d_beta = up(at(beta, o1), h.tok_1, ss);
+        float* d_S0 = (float*)up(at(S0, os), h.st, ss);
+        // the cotangents go up with the inputs: queued behind the forward they would hold the copy engine's queue
+        void* d_dO = with_bwd ? up(at(dO, ov), h.tok_v, ss) : nullptr;
+        float* d_dSf = with_bwd ? (float*)up(at(dS_final, os), h.st, ss) : nullptr;
+        if (ns > 1) ok = ok && cudaEventRecord(arrived[i], ss) == cudaSuccess;
+        void* d_O = slot(h.tok_v);
+        float* d_Sf = (float*)slot(h.st);
+        void* d_ws = nullptr;
+        size_t ws_bytes = 0;
+        if (with_bwd) {
+            ws_bytes = carve_workspace_bytes(&ps, 1);
+            d_ws = slot(ws_bytes);
+        }
+        if (!ok) break;
+        rs = carve_fwd(&ps, d_q, d_k, d_v, d_f, d_bx, d_wx, d_beta, d_A, d_tau, d_Ub, d_Uw, d_Vb, d_Vw, d_S0, d_O, d_Sf,
+                       d_ws, ws_bytes, ss);
+        if (rs != CARVE_OK) break;
+        if (with_bwd) {
+            void *d_dq = slot(h.tok_k), *d_dk = slot(h.tok_k), *d_df = slot(h.tok_k), *d_dbx = slot(h.tok_k),
+                 *d_dv = slot(h.tok_v), *d_dwx = slot(h.tok_v), *d_dbeta = slot(h.tok_1);
+            float* d_dS0 = (float*)slot(h.st);
+            float* wp = (float*)slot(nwg * 4);
+            float *d_dA = wp, *d_dtau = d_dA + (size_t)p->H * p->dk, *d_dUb = d_dtau + (size_t)p->H * p->dk,
+                  *d_dUw = d_dUb + (size_t)p->r * p->dv, *d_dVb = d_dUw + (size_t)p->r * p->dv,
+                  *d_dVw = d_dVb + (size_t)p->dk * p->r;
+            if (!ok) break;
+            rs = bwd_impl(&ps, d_q, d_k, d_v, d_f, d_bx, d_wx, d_beta, d_A, d_tau, d_Ub, d_Uw, d_Vb, d_Vw, d_S0, d_dO,
+                          d_dSf, d_dq, d_dk, d_dv, d_df, d_dbx, d_dwx, d_dbeta, d_dA, d_dtau, d_dUb, d_dUw, d_dVb,
+                          d_dVw, d_dS0, d_ws, ws_bytes, ss, ns > 1);
+            if (rs != CARVE_OK) break;
+            down(atw(dq, okk), d_dq, h.tok_k, ss); down(atw(dk, okk), d_dk, h.tok_k, ss);
+            down(atw(df, okk), d_df, h.tok_k, ss); down(atw(dbx, okk), d_dbx, h.tok_k, ss);
+            down(atw(dv, ov), d_dv, h.tok_v, ss); down(atw(dwx, ov), d_dwx, h.tok_v, ss);
+            down(atw(dbeta, o1), d_dbeta, h.tok_1, ss); down(atw(dS0, os), d_dS0, h.st, ss);
+            if (i == 0) d_wpart = wp;
+            if (i == 1) wpart_stride = (size_t)((char*)wp - (char*)d_wpart) / 4;
+        }
+        // after the backward: a download between the two calls would make carve_bwd wait for the copy engine's queue
+        down(atw(O, ov), d_O, h.tok_v, ss);
+        down(atw(S_final, os), d_Sf, h.st, ss);
+    }
+    // join: the caller's stream continues after every slice has finished
+    for (int i = 0; i < ns; ++i) {
+        if (ns > 1 && side[i] && join[i]) {
+            ok = cudaEventRecord(join[i], side[i]) == cudaSuccess && ok;
+            ok = cudaStreamWaitEvent(st, join[i], 0) == cudaSuccess && ok;
+        }
+    }
+    if (with_bwd && ok && rs == CARVE_OK) {
+        carve_sum_slices_kernel<<<(unsigned)((nwg + 255) / 256), 256, 0, st>>>(d_wsum, d_wpart, (int)nwg, ns, wpart_stride);
+        ok = ok && cudaGetLastError() == cudaSuccess;
+        const float* w = d_wsum;
+        down(dA, w, h.w_a, st); w += (size_t)p->H * p->dk;
+        down(dtau, w, h.w_a, st); w += (size_t)p->H * p->dk;
+        down(dUb, w, h.w_u, st); w += (size_t)p->r * p->dv;
+        down(dUw, w, h.w_u, st); w += (size_t)p->r * p->dv;
+        down(dVb, w, h.w_vb, st); w += (size_t)p->dk * p->r;
+        down(dVw, w, h.w_vw, st);
+    }
+    // streams and events are released by the runtime once the work enqueued on them has completed
+    for (int i = 0; i < ns; ++i) {
+        if (ns > 1 && side[i]) cudaStreamDestroy(side[i]);
+        if (join[i]) cudaEventDestroy(join[i]);
+        if (arrived[i]) cudaEventDestroy(arrived[i]);
+    }
+    if (fork) cudaEventDestroy(fork);
+    if (rs != CARVE_OK) return rs;
     return ok ? CARVE_OK : CARVE_ERR_CUDA;
 }
 

@@ -13,6 +13,10 @@ namespace carve {
 struct Args {
     int B, H, T, L, dk, dv, r;
     int l2norm;
+    // tensor path, backward: launch the chunk-local epilogue as a plain dependent kernel.  The overlapped form
+    // (an early grid that polls per-chain progress flags) fills every idle SM, which starves the chains of other
+    // calls running beside this one (the batch slices of carve_fwd_bwd_host).
+    bool epilogue_after = false;
     float scale, eps;
     // forward inputs
     const void *q, *k, *v, *f, *bx, *wx, *beta;

@@ -1133,7 +1133,7 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
         attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = attr;
-        cfg.numAttrs = 1;
+        cfg.numAttrs = a.epilogue_after ? 0 : 1;
         e = cudaLaunchKernelEx(&cfg, carve_bwd_tc_epilogue_kernel<D>, static_cast<const __nv_bfloat16*>(a.q),
                                static_cast<const __nv_bfloat16*>(a.k), static_cast<const __nv_bfloat16*>(a.f), a.A, a.tau, t.dq,
                                t.dk, t.df, partAT, a.T, a.H, LCc, a.l2norm, a.eps, (const int*)t.flags, chains);

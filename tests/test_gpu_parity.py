@@ -133,9 +133,12 @@ def test_determinism_and_zero_content_grads(oracle):
         assert np.all(outs[0][2][n] == 0.0), n
 
 
-def test_host_entry_point_matches_device_entry_point(oracle):
+@pytest.mark.parametrize("B", [1, 4, 6])
+def test_host_entry_point_matches_device_entry_point(oracle, B):
+    """carve_fwd_bwd_host cuts the batch into slices on streams of its own: per-chain results are those of the
+    device entry points bit for bit; the shared-weight gradients are the slices' sums (another rounding order)."""
     import torch
-    cfg = synth.Config("t", B=1, H=2, T=128, L=64, dk=64, dv=64, r=8, dtype="bf16", wstd=0.1, seed=21)
+    cfg = synth.Config("t", B=B, H=2, T=128, L=64, dk=64, dv=64, r=8, dtype="bf16", wstd=0.1, seed=21)
     x = synth.make_inputs(cfg)
     ct = synth.make_cotangents(cfg)
     p = params_of(cfg)
@@ -154,7 +157,11 @@ def test_host_entry_point_matches_device_entry_point(oracle):
     assert np.array_equal(Oh.float().numpy().astype(np.float64), O)
     assert np.array_equal(Sfh.numpy().astype(np.float64), Sf)
     for n in GRADS:
-        assert np.array_equal(gh[n].float().numpy().astype(np.float64), g[n]), n
+        got = gh[n].float().numpy().astype(np.float64)
+        if B > 1 and n in ("dA", "dtau", "dUb", "dUw", "dVb", "dVw"):
+            assert relerr(got, g[n]) < 1e-5, n
+        else:
+            assert np.array_equal(got, g[n]), n
 
 
 # ---- both kernel families against the oracle on the same bf16 case --------------------------------
