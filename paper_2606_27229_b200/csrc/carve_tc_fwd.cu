@@ -102,7 +102,7 @@ __device__ __forceinline__ void warp_store(float* Q, int qr, int qc, const float
 // Tm <- (I + Mm)^-1 for the leading n x n block (n in {16,32,64}); Mm strictly lower (only that part is read).
 // Blocked forward substitution (Alg. 2 step 7): 8x8 diagonal blocks by substitution, 16x16 blocks by fp32 FMA, then
 // T_ij = -T_ii (M_ij T_jj) one level at a time, the block products on tensor cores (tf32 mma.sync).
-__device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid, int nthreads)
+__device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid, int nthreads, uint8_t* tp)
 {
     const int warp = tid >> 5, lane = tid & 31;
     // step 1a: 8x8 diagonal sub-blocks by forward substitution (thread = sub-block, column), zero above the diagonal
@@ -151,6 +151,27 @@ __device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid, int nthr
         if (act) Tm[mm_idx(o + 8 + i, o + j)] = -yv;
     }
     __syncthreads();
+    // n = 64: the bf16 tile `tp` (rows 0..63 of a 128-row tile, zero above the diagonal) is written as the blocks become
+    // final, by the warps the tensor-core levels leave idle; the last level writes it from its accumulators.
+    const bool fused = n == 64 && nthreads > 128;
+    auto put8 = [&](int r, int ch, bool zero) {   // 8 columns [8 ch, 8 ch + 8) of row r
+        float f[8];
+        if (zero) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) f[e] = 0.f;
+        } else {
+            *reinterpret_cast<float4*>(f) = *reinterpret_cast<const float4*>(&Tm[mm_idx(r, 8 * ch)]);
+            *reinterpret_cast<float4*>(f + 4) = *reinterpret_cast<const float4*>(&Tm[mm_idx(r, 8 * ch + 4)]);
+        }
+        sts128(tp + tile_chunk_off(128, r, ch), pack8(f));
+    };
+    if (fused && warp >= 4) {
+        // each row's diagonal 16-block (final after step 1) and the zeros to its right
+        for (int it = tid - 128; it < 64 * 8; it += nthreads - 128) {
+            const int r = it >> 3, ch = it & 7, d0 = 2 * (r >> 4);
+            if (ch >= d0) put8(r, ch, ch >= d0 + 2);
+        }
+    }
     if (n >= 32) {
         // level 32: blocks (1,0) and (3,2); warp = (pair, 8-column tile)
         const int npair = n / 32;
@@ -174,10 +195,41 @@ __device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid, int nthr
             warp_store<2>(Tm, 32, 8 * warp, d, 1.f, lane);
             __syncwarp();
             warp_prod<2, 4>(d, Tm, 32, 32, Tm, 32, 8 * warp, lane);
-            __syncwarp();
-            warp_store<2>(Tm, 32, 8 * warp, d, -1.f, lane);
+            if (fused) {
+                const int g = lane >> 2, l4 = lane & 3;
+#pragma unroll
+                for (int m = 0; m < 2; ++m) {
+                    const int r0 = 32 + 16 * m + g;
+                    *reinterpret_cast<uint32_t*>(tp + tile_chunk_off(128, r0, warp) + 4 * l4) = pack_bf16(-d[m][0], -d[m][1]);
+                    *reinterpret_cast<uint32_t*>(tp + tile_chunk_off(128, r0 + 8, warp) + 4 * l4) = pack_bf16(-d[m][2], -d[m][3]);
+                }
+            } else {
+                __syncwarp();
+                warp_store<2>(Tm, 32, 8 * warp, d, -1.f, lane);
+            }
+        } else if (fused) {
+            // the level-32 blocks (rows 16..31 x cols 0..15, rows 48..63 x cols 32..47) are final
+            for (int it = tid - 128; it < 64; it += nthreads - 128) {
+                const int hi = it >> 5, r = 16 + 32 * hi + ((it >> 1) & 15), ch = 4 * hi + (it & 1);
+                put8(r, ch, false);
+            }
         }
+    }
+    if (!fused) {
         __syncthreads();
+        const int tr_ = tid >> 2, qq = tid & 3;  // row, 16-column quarter
+        if (tr_ < n) {
+#pragma unroll
+            for (int k8 = 0; k8 < 2; ++k8) {
+                float f[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const int s_ = 16 * qq + 8 * k8 + e;
+                    f[e] = s_ <= tr_ ? Tm[mm_idx(tr_, s_)] : 0.f;
+                }
+                sts128(tp + tile_chunk_off(128, tr_, 2 * qq + k8), pack8(f));
+            }
+        }
     }
 }
 
@@ -817,22 +869,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         __syncthreads();
         PROF(g_prof_fwd, 12);
         // ---- P9c: T = (I + beta A)^-1 -> TP rows 0..63 (bf16, zero above the diagonal)
-        tri_inverse(Mm, Tm, LCc, tid, NTH);
-        {
-            const int tr_ = tid >> 2, qq = tid & 3;  // row, 16-column quarter
-            if (tr_ < LCc) {
-#pragma unroll
-                for (int k8 = 0; k8 < 2; ++k8) {
-                    float f[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        const int s = 16 * qq + 8 * k8 + e;
-                        f[e] = s <= tr_ ? Tm[mm_idx(tr_, s)] : 0.f;
-                    }
-                    sts128(sm + Lo.TP + tile_chunk_off(128, tr_, 2 * qq + k8), pack8(f));
-                }
-            }
-        }
+        tri_inverse(Mm, Tm, LCc, tid, NTH, sm + Lo.TP);
         PROF(g_prof_fwd, 13);
         // ---- P10: U = T (beta R) -> TM_X1
         PHASE_SYNC();
