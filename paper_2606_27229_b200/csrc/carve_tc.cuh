@@ -127,6 +127,10 @@ __device__ __forceinline__ float tanh_fast(float x)
     return y;
 }
 
+// sigmoid through one tanh.approx (one transcendental op instead of exp + reciprocal; |error| < 3e-4, below the bf16
+// rounding of the values it feeds)
+__device__ __forceinline__ float sigmoid_tanh(float x) { return fmaf(0.5f, tanh_fast(0.5f * x), 0.5f); }
+
 __device__ __forceinline__ uint4 lds128(const uint8_t* p) { return *reinterpret_cast<const uint4*>(p); }
 __device__ __forceinline__ void sts128(uint8_t* p, uint4 v) { *reinterpret_cast<uint4*>(p) = v; }
 __device__ __forceinline__ void unpack8(uint4 w, float (&f)[8])

@@ -563,10 +563,15 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
 #pragma unroll
                         for (int e = 0; e < 8; ++e) {
                             const int j = 8 * cc + e;
+                            // sigmoid and softplus of the same argument share exp(-|pre|): 3 transcendental ops, not 4
                             const float pre = fb[e] + __uint_as_float(pr[e]);
-                            bg[e] = sigmoid_fast(pre);
+                            const float ex = __expf(-fabsf(pre)), s1p = 1.f + ex;
+                            if (rc) {
+                                const float rs = __fdividef(1.f, s1p);
+                                bg[e] = pre >= 0.f ? rs : ex * rs;
+                            }
                             const float g = -mi.eA[j] * softplus_fast(ff[e] + mi.tau[j]);
-                            const float la = g - softplus_fast(pre);
+                            const float la = g - (fmaxf(pre, 0.f) + __logf(s1p));
                             const float h16 = __bfloat162float(__float2bfloat16_rn(la));
                             hi[e] = h16;
                             lo[e] = la - h16;
@@ -581,7 +586,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                         unpack8(lds128(sm + Lo.V + off), fv);
 #pragma unroll
                         for (int e = 0; e < 8; ++e) {
-                            fw[e] = sigmoid_fast(fw[e] + __uint_as_float(pw[e]));
+                            fw[e] = sigmoid_tanh(fw[e] + __uint_as_float(pw[e]));
                             fv[e] *= fw[e];
                         }
                         sts128(sm + Lo.V + off, pack8(fv));
