@@ -265,6 +265,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     static_assert(DK == DV, "the shared-memory map assumes dk == dv");
     constexpr int DM = DK > DV ? DK : DV;
     constexpr int NTH = 128 * NP;
+    // issues (and waits for) the record's bulk copies: lane 0 of a Q-side warp of the last column part, which has
+    // little or nothing to do in the phases that follow the copies (P9a/P9b/P11), unlike the MMA-issuing thread 0
+    constexpr int REC_TID = NTH - 64;
     constexpr int HK = DK / NP, HV = DV / NP;  // columns per warpgroup ("half" = part index 0..NP-1)
     extern __shared__ uint8_t smem_raw[];
     uint8_t* sm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -392,7 +395,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 0);
         // ---- P0: fold G^T = S^T Ucat^T -> TM_X2[0, R2)
         PHASE_SYNC();
-        if (rc && tid == 0) {   // record: state entering the chunk (Sb stays intact until P13)
+        if (rc && tid == REC_TID) {   // record: state entering the chunk (Sb stays intact until P13)
             bulk_s2g(rc + Rc.SB, sb + Lo.Sb, (uint32_t)state_tile);
             bulk_commit();
         }
@@ -741,6 +744,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
+        if (rc && tid == REC_TID) bulk_wait_read();   // the previous chunk's [P;T] copy has left TP (rewritten in P9)
         PROF(g_prof_fwd, 9);
         // ---- P8: A|P blocks (one 16-column block per anchoring) and the state products
         PHASE_SYNC();
@@ -752,9 +756,12 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             if (nb > 3) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 48, 16, sb + Lo.Y2 + tile_bytes(96, DK), 32, 0, sb + Lo.Y1, 64, 48, DK, false);
             mma_rt<128, KMAJ, KMAJ>(tmem + TM_ACC, DV, sb + Lo.KQbar, 128, 0, sb + Lo.Sb, DV, 0, DK, false);
             umma_commit(&mi.bar_mma);
-            if (rc) {
+        }
+        {
+            const int nb = LCc >> 4;
+            if (rc && tid == REC_TID) {
                 // record: operand tiles straight from shared memory (bulk copies).  Only sources that stay intact until
-                // the wait in P12 are used: Ktil, C, version 0 (Kbar/Qbar) and version 2 (Y0).  The rows of the odd
+                // the wait in P11 are used: Ktil, C, version 0 (Kbar/Qbar) and version 2 (Y0).  The rows of the odd
                 // 16-token blocks (versions 1 and 3 live in Y2/TP, rewritten in P9) were stored by their threads in P7b.
                 constexpr uint32_t TB = tile_bytes(64, DK);
                 bulk_s2g(rc + Rc.KT, sb + Lo.Ktil, TB);
@@ -881,12 +888,12 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         if (tid == 0) {
             mma_rt<128, KMAJ, MNMAJ>(tmem + TM_X1, DV, sb + Lo.TP, 128, 0, sb + Lo.Y2, 64, 0, LCc, false);
             umma_commit(&mi.bar_mma);
-            if (rc) {   // record [scale.P ; T]: the two row halves of TP swapped (TP is next written in P9 of the next chunk)
-                if (s1) bulk_s2g(rc + Rc.PT, sb + Lo.TP + 8192, 8192);
-                bulk_s2g(rc + Rc.PT + 8192, sb + Lo.TP, 8192);
-                bulk_commit();
-            }
             if (c + 1 < nchunks) issue_kq(c + 1);
+        }
+        if (rc && tid == REC_TID) {   // record [scale.P ; T]: the two row halves of TP swapped (TP is next written in P9 of the next chunk)
+            if (s1) bulk_s2g(rc + Rc.PT, sb + Lo.TP + 8192, 8192);
+            bulk_s2g(rc + Rc.PT + 8192, sb + Lo.TP, 8192);
+            bulk_commit();
         }
         WAIT_MMA();
         PROF(g_prof_fwd, 14);
@@ -905,6 +912,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
+        // the record copies issued so far have left their buffers: the next chunk's loads (below) and P13 may overwrite them
+        if (rc && tid == REC_TID) bulk_wait_read();
         PROF(g_prof_fwd, 15);
         // ---- P12: O += P U;  W = U^T Ktil -> TM_X2
         PHASE_SYNC();
@@ -972,7 +981,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     }
     if (VS > 1) cluster_wait();   // pairs with the last arrive; also keeps this CTA's shared memory alive for the peer
     PHASE_SYNC();
-    if (rec_chain && tid == 0) bulk_wait_all();   // drain the record's bulk stores
+    if (rec_chain && (tid == 0 || tid == REC_TID)) bulk_wait_all();   // drain the record's bulk stores
     if (warp == 0) tmem_dealloc(tmem, TM_COLS);
 }
 
