@@ -617,15 +617,15 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         if (!krole && warp_active) {
             const int blk = t >> 4;
             const bool last = live && (t & 15) == 15;
-#pragma unroll 1
-            for (int cc = half * (HK / 8); cc < (half + 1) * (HK / 8); ++cc) {
-                uint32_t v[8];
-                tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, v);
-                tmem_wait_ld();
-                if (last) {
+            uint32_t v[32];
+            tmem_ld32(tmem + TM_X2 + lane_base + half * HK, v);
+            tmem_wait_ld();
+            if (last) {
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) mi.etot[blk][8 * cc + e] = __expf(__uint_as_float(v[e]));
-                }
+                for (int e4 = 0; e4 < 8; ++e4)
+                    *reinterpret_cast<float4*>(&mi.etot[blk][half * HK + 4 * e4]) =
+                        make_float4(__expf(__uint_as_float(v[4 * e4])), __expf(__uint_as_float(v[4 * e4 + 1])),
+                                    __expf(__uint_as_float(v[4 * e4 + 2])), __expf(__uint_as_float(v[4 * e4 + 3])));
             }
         }
         __syncthreads();
