@@ -113,6 +113,7 @@ struct Misc {
     float nrm[128][4];          // partial sums of squares: rows 0..63 k, 64..127 q; [column part]
     float beta[64];             // write strength of the chunk's tokens
     uint64_t bar_mma, bar_kq, bar_fb, bar_wv;
+    uint64_t bar_acc;           // the state products of P8 (waited for after the A|P blocks have been consumed)
     uint32_t tmem_base;
 };
 

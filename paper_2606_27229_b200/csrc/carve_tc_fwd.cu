@@ -294,7 +294,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
 
     // ---- one-time setup --------------------------------------------------------------------------
     if (tid == 0) {
-        mbar_init(&mi.bar_mma, 1); mbar_init(&mi.bar_kq, 1); mbar_init(&mi.bar_fb, 1); mbar_init(&mi.bar_wv, 1);
+        mbar_init(&mi.bar_mma, 1); mbar_init(&mi.bar_acc, 1); mbar_init(&mi.bar_kq, 1); mbar_init(&mi.bar_fb, 1); mbar_init(&mi.bar_wv, 1);
         mbar_fence_init();
         tma_prefetch_desc(&mq); tma_prefetch_desc(&mk); tma_prefetch_desc(&mv);
         tma_prefetch_desc(&mf); tma_prefetch_desc(&mbx); tma_prefetch_desc(&mwx);
@@ -383,7 +383,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     };
     if (tid == 0) { fence_async_smem(); issue_kq(0); issue_fb(0); issue_wv(0); }
 
-    uint32_t mma_ph = 0, tma_ph = 0;
+    uint32_t mma_ph = 0, tma_ph = 0, acc_ph = 0;
     // write strength of this thread's token, fetched one chunk ahead (a plain global load: its latency must not sit
     // on the chunk's serial path)
     float beta_nx = (krole && half == 0 && live) ? __bfloat162float(a.beta[((size_t)b * a.T + t) * a.H + h]) : 0.f;
@@ -754,8 +754,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             if (nb > 1) mma_rt<128, KMAJ, KMAJ>(tmem + TM_X2 + 16, 16, sb + Lo.Y2, 96, 0, sb + Lo.Y1, 64, 16, DK, false);
             if (nb > 2) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 32, 16, sb + Lo.Y0, 64, 0, sb + Lo.Y1, 64, 32, DK, false);
             if (nb > 3) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 48, 16, sb + Lo.Y2 + tile_bytes(96, DK), 32, 0, sb + Lo.Y1, 64, 48, DK, false);
+            umma_commit(&mi.bar_mma);   // the A|P blocks: P9a starts on them while the state products still run
             mma_rt<128, KMAJ, KMAJ>(tmem + TM_ACC, DV, sb + Lo.KQbar, 128, 0, sb + Lo.Sb, DV, 0, DK, false);
-            umma_commit(&mi.bar_mma);
+            umma_commit(&mi.bar_acc);
         }
         {
             const int nb = LCc >> 4;
@@ -860,6 +861,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         PROF(g_prof_fwd, 11);
         // ---- P9b: beta R = beta (V' - Kbar S^T) -> Y2 (rows t)
+        mbar_wait(&mi.bar_acc, acc_ph);
+        acc_ph ^= 1u;
+        tc_fence_after();
         if (krole && warp_active) {
             const float bt = live ? sBeta[t] : 0.f;
             static_assert(HV == 32 && HK == 32, "one 32-column TMEM load per thread and phase");
