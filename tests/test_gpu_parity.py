@@ -208,20 +208,13 @@ def test_tensor_path_determinism(oracle):
 
 
 # ---- BASELINE.json config 1 at full size, in the launch configuration bench.py times ------------------
-def test_config1_full_size_sampled_chains(oracle):
-    """The whole 1.3B-like workload runs on the GPU (128 chains x 64 chunks); the oracle recomputes sampled
-    (batch, head) chains one by one -- chains are independent (Alg. 2 l.318) -- for every per-token output, S_final
-    and dS0.  The shared-weight gradients sum over all chains, so they are checked on the sampled chains run as
-    their own B'=3, H'=1 problem at full T."""
-    cfg = synth.CFG1
+def _check_full_size_sampled_chains(oracle, cfg, chains):
     x, ct = synth.make_inputs(cfg), synth.make_cotangents(cfg)
     p = params_of(cfg)
     assert carve.carve_resolved_path(p, True) == carve.CARVE_PATH_TENSOR
     O, Sf, h = run_fwd(p, x, need_bwd=True)
     g, _ = run_bwd(p, h, ct)
-    chains = [(0, 0), (3, 7), (7, 15)]
     tol = TOL["bf16"]
-    xs_all, cts_all = None, None
     for b, hh in chains:
         xs = synth.slice_chains(x, [(b, hh)])
         cts = synth.slice_chains(ct, [(b, hh)])
@@ -238,6 +231,21 @@ def test_config1_full_size_sampled_chains(oracle):
     cts = synth.slice_chains(ct, chains)
     sub = cfg.with_(B=len(chains), H=1)
     _check_fwd_bwd(oracle, sub, xs, ct=cts)
+
+
+def test_config1_full_size_sampled_chains(oracle):
+    """The whole 1.3B-like workload runs on the GPU (128 chains x 64 chunks); the oracle recomputes sampled
+    (batch, head) chains one by one -- chains are independent (Alg. 2 l.318) -- for every per-token output, S_final
+    and dS0.  The shared-weight gradients sum over all chains, so they are checked on the sampled chains run as
+    their own B'=3, H'=1 problem at full T."""
+    _check_full_size_sampled_chains(oracle, synth.CFG1, [(0, 0), (3, 7), (7, 15)])
+
+
+def test_config4_full_size_sampled_chains(oracle):
+    """Config 4 at full size: 2048 chains, i.e. many more chains than SMs (several waves of the per-chain grid),
+    with its stress structure (beta = 1 on 10 % of tokens, no decay on 10 % of key dims).  Same sampling as config 1;
+    the sampled chains include the first and the last one and one from the middle waves."""
+    _check_full_size_sampled_chains(oracle, synth.CFG4, [(0, 0), (29, 13), (63, 31)])
 
 
 @pytest.mark.parametrize("L", [16, 32, 64, 128])
