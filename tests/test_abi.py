@@ -56,6 +56,10 @@ def test_argument_errors_before_any_launch(lib):
     assert lib.carve_fwd(ctypes.byref(cp), *nul, None, 0, None) == 1            # CARVE_ERR_NULL
     bad = _p(T=100).c()
     assert lib.carve_fwd(ctypes.byref(bad), *nul, None, 0, None) == 2           # CARVE_ERR_SHAPE
+    for empty in (dict(T=0), dict(B=0), dict(H=0)):                             # empty inputs: refused, never launched
+        e = _p(**empty).c()
+        assert lib.carve_fwd(ctypes.byref(e), *nul, None, 0, None) == 2, empty
+        assert carve.carve_workspace_bytes(_p(**empty), True) == 0, empty
     buf = (ctypes.c_char * 4096)()
     base = (ctypes.addressof(buf) + 255) & ~255
     ptrs = [ctypes.c_void_p(base)] * 16
