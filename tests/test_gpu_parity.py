@@ -248,6 +248,13 @@ def test_config4_full_size_sampled_chains(oracle):
     _check_full_size_sampled_chains(oracle, synth.CFG4, [(0, 0), (29, 13), (63, 31)])
 
 
+@pytest.mark.parametrize("L", [16, 128])
+def test_config2_full_size_sampled_chains(oracle, L):
+    """Config 2 at full size (64 chains, T = 8192, active content gates) at the two ends of the chunk-length sweep:
+    L = 16 (512 fold reads per chain) and L = 128 (a gate chunk spans two solve chunks)."""
+    _check_full_size_sampled_chains(oracle, synth.CFG2[L], [(0, 0), (2, 9), (3, 15)])
+
+
 @pytest.mark.parametrize("L", [16, 32, 64, 128])
 def test_config2_chunk_sweep_reduced_batch(oracle, L):
     """Config 2 (chunk-length sweep, gate projections ~N(0,0.1^2)) at full T = 8192 with B*H reduced to 2 chains."""
