@@ -277,6 +277,22 @@ def test_config3_long_context_forward_reduced_heads(oracle):
     _check_fwd_bwd(oracle, cfg, x, with_bwd=False)
 
 
+def test_config3_full_size_sampled_chains(oracle):
+    """Config 3 at full size (16 chains x 1024 chunks, d_v = 256 split over a two-CTA cluster, random S0, forward
+    only): the whole workload runs on the GPU, the oracle recomputes the first and the last chain."""
+    cfg = synth.CFG3
+    x = synth.make_inputs(cfg)
+    p = params_of(cfg)
+    O, Sf, _ = run_fwd(p, x, need_bwd=False)
+    assert np.isfinite(O).all() and np.isfinite(Sf).all()
+    tol = TOL["bf16"]
+    s = oracle_shape(oracle, cfg, B=1, H=1)
+    for b, hh in [(0, 0), (0, 15)]:
+        O_ref, S_ref = oracle.fwd(s, synth.slice_chains(x, [(b, hh)]))
+        assert relerr(O[b:b + 1, :, hh:hh + 1], O_ref) <= tol["O"], (b, hh)
+        assert relerr(Sf[b:b + 1, hh:hh + 1], S_ref) <= tol["S"], (b, hh)
+
+
 @pytest.mark.parametrize("B,H,T,L,d,r,seed", [(3, 5, 64, 64, 128, 8, 101), (1, 3, 192, 64, 128, 16, 102), (2, 1, 32, 16, 64, 16, 103),
                                               (1, 7, 384, 128, 128, 16, 104), (5, 2, 96, 32, 64, 8, 105)])
 def test_tensor_path_odd_shapes(oracle, B, H, T, L, d, r, seed):
