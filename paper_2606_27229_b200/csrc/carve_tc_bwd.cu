@@ -181,7 +181,10 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     constexpr uint32_t TB = tile_bytes(64, D);     // one [64][D] tile
     constexpr uint32_t SBb = tile_bytes(D, D);     // one state tile
     extern __shared__ uint8_t smem_raw[];
-    uint8_t* sm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    // 1024-byte alignment by an offset from the __shared__ array (not by integer rounding of a generic pointer), so
+    // that the compiler still knows these are shared-memory addresses: LDS/STS with 32-bit address arithmetic
+    // instead of generic LD/ST with 64-bit arithmetic.
+    uint8_t* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     const BLayout Lo(D);
     BMisc& mi = *reinterpret_cast<BMisc*>(sm + Lo.misc);
     const uint32_t sb = smem_u32(sm);
@@ -1151,7 +1154,7 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
 extern "C" void carve_debug_prof_bwd(unsigned long long* out)
 {
     cudaMemcpyFromSymbol(out, g_prof_bwd, sizeof(g_prof_bwd));
-    unsigned long long z[40] = {};
+    unsigned long long z[80] = {};
     cudaMemcpyToSymbol(g_prof_bwd, z, sizeof(z));
 }
 #endif

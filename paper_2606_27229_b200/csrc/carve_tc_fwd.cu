@@ -42,11 +42,11 @@ struct TcArgs {
 };
 
 // Runtime-shaped product from two row tiles (see tc_common.cuh umma_tiles_rt); M fixed at compile time.
-template <int M, int AMAJ, int BMAJ>
+template <int M, int AMAJ, int BMAJ, int KMAX = 128>
 __device__ __forceinline__ void mma_rt(uint32_t d_tmem, int N, uint32_t a_saddr, int a_rows, int a_o0, uint32_t b_saddr,
                                        int b_rows, int b_o0, int K, bool accumulate)
 {
-    umma_tiles_rt<AMAJ, BMAJ>(d_tmem, M, N, a_saddr, a_rows, a_o0, 0, b_saddr, b_rows, b_o0, 0, K, accumulate);
+    umma_prod<AMAJ, BMAJ, KMAX>(d_tmem, M, N, a_saddr, a_rows, a_o0, 0, b_saddr, b_rows, b_o0, 0, K, accumulate);
 }
 
 // fp32 scratch matrices of the triangular inverse: [64][64], columns XOR-swizzled by the row.
@@ -60,52 +60,22 @@ __device__ __forceinline__ void mma_tf32(float (&d)[4], const uint32_t (&a)[4], 
         : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
 }
 
-// One warp: D[16*MT x 8] = sum over k < 8*KS of P[pr + .][pc + k] * Q[qr + k][qc + .]  (fp32 swizzled matrices).
-template <int MT, int KS>
-__device__ __forceinline__ void warp_prod(float (&d)[MT][4], const float* P, int pr, int pc, const float* Q, int qr, int qc,
-                                          int lane)
+__device__ __forceinline__ void ldsm_x4_trans(uint32_t (&r)[4], uint32_t saddr)
 {
-    const int g = lane >> 2, l4 = lane & 3;
-#pragma unroll
-    for (int m = 0; m < MT; ++m)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) d[m][e] = 0.f;
-#pragma unroll
-    for (int ks = 0; ks < KS; ++ks) {
-        uint32_t bfr[2];
-        bfr[0] = __float_as_uint(Q[mm_idx(qr + 8 * ks + l4, qc + g)]);
-        bfr[1] = __float_as_uint(Q[mm_idx(qr + 8 * ks + l4 + 4, qc + g)]);
-#pragma unroll
-        for (int m = 0; m < MT; ++m) {
-            uint32_t afr[4];
-            afr[0] = __float_as_uint(P[mm_idx(pr + 16 * m + g, pc + 8 * ks + l4)]);
-            afr[1] = __float_as_uint(P[mm_idx(pr + 16 * m + g + 8, pc + 8 * ks + l4)]);
-            afr[2] = __float_as_uint(P[mm_idx(pr + 16 * m + g, pc + 8 * ks + l4 + 4)]);
-            afr[3] = __float_as_uint(P[mm_idx(pr + 16 * m + g + 8, pc + 8 * ks + l4 + 4)]);
-            mma_tf32(d[m], afr, bfr);
-        }
-    }
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                 : "r"(saddr));
 }
-template <int MT>
-__device__ __forceinline__ void warp_store(float* Q, int qr, int qc, const float (&d)[MT][4], float sign, int lane)
+__device__ __forceinline__ void stsm_x4_trans(uint32_t saddr, const uint32_t (&r)[4])
 {
-    const int g = lane >> 2, l4 = lane & 3;
-#pragma unroll
-    for (int m = 0; m < MT; ++m) {
-        Q[mm_idx(qr + 16 * m + g, qc + 2 * l4)] = sign * d[m][0];
-        Q[mm_idx(qr + 16 * m + g, qc + 2 * l4 + 1)] = sign * d[m][1];
-        Q[mm_idx(qr + 16 * m + g + 8, qc + 2 * l4)] = sign * d[m][2];
-        Q[mm_idx(qr + 16 * m + g + 8, qc + 2 * l4 + 1)] = sign * d[m][3];
-    }
+    asm volatile("stmatrix.sync.aligned.m8n8.x4.trans.shared.b16 [%0], {%1,%2,%3,%4};" ::"r"(saddr), "r"(r[0]), "r"(r[1]),
+                 "r"(r[2]), "r"(r[3])
+                 : "memory");
 }
 
-// Tm <- (I + Mm)^-1 for the leading n x n block (n in {16,32,64}); Mm strictly lower (only that part is read).
-// Blocked forward substitution (Alg. 2 step 7): 8x8 diagonal blocks by substitution, 16x16 blocks by fp32 FMA, then
-// T_ij = -T_ii (M_ij T_jj) one level at a time, the block products on tensor cores (tf32 mma.sync).
-__device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid, int nthreads, uint8_t* tp)
+// 8x8 diagonal blocks of (I + Mm)^-1 -> Tm by forward substitution (thread = (block, column)); Mm strictly lower.
+__device__ __forceinline__ void diag8_inverse(const float* Mm, float* Tm, int n, int tid)
 {
-    const int warp = tid >> 5, lane = tid & 31;
-    // step 1a: 8x8 diagonal sub-blocks by forward substitution (thread = sub-block, column), zero above the diagonal
     if (tid < n) {
         const int c = tid & 7, o = 8 * (tid >> 3);
         float x[8];
@@ -117,117 +87,73 @@ __device__ void tri_inverse(const float* Mm, float* Tm, int n, int tid, int nthr
             x[tt] = (tt == c) ? 1.f : (tt < c ? 0.f : -acc);
             Tm[mm_idx(o + tt, o + c)] = x[tt];
         }
-    } else if (tid < 2 * n) {
-        // the upper-right 8x8 block of every 16-block is zero
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const int idx = 4 * (tid - n) + e, blk = idx >> 6, rr = (idx >> 3) & 7, cc = idx & 7;
-            Tm[mm_idx(16 * blk + rr, 16 * blk + 8 + cc)] = 0.f;
-        }
-    } else if (n >= 64) {
-        // blocks (0,1) and (2,3) of T are zero; the level-64 products read them
-        for (int i = tid - 2 * n; i < 512; i += nthreads - 2 * n) {
-            const int blk = i >> 8, rr = (i >> 4) & 15, cc = i & 15;
-            Tm[mm_idx(32 * blk + rr, 32 * blk + 16 + cc)] = 0.f;
-        }
     }
-    __syncthreads();
-    // step 1b: lower-left 8x8 block of every 16-block, T21 = -T22 (M21 T11), one element per thread (fp32 FMA)
-    {
-        const bool act = tid < 4 * n;
-        const int o = 16 * (tid >> 6), i = (tid >> 3) & 7, j = tid & 7;
-        float xv = 0.f, yv = 0.f;
-        if (act) {
+}
+
+// WY solve, Alg. 2 step 7: X (I + Mm)^T = RHS for X = U^T (value channels x tokens) and, on four
+// more warps, for X = T^T with RHS = I (the inverse itself, which the chunk record keeps for the backward).  Blocked
+// forward substitution over 8-token blocks, entirely in registers on tf32 mma.sync (m16n8k8): a warp owns 16 rows of X
+// (value channels, or columns of T) and walks the token blocks i = 0.. in order,
+//     X_i = (RHS_i - sum_{j<i} X_j N_ij^T) T_ii^T,      N = Mm (= diag(beta) A), T_ii = 8x8 diagonal inverses (Tm).
+// The accumulator fragment of X_j (row g: tokens 2 l4, 2 l4 + 1) is reused as the A operand of the later products with
+// the contraction index permuted (slot l4 <- token 2 l4, slot l4 + 4 <- token 2 l4 + 1); the B operand N_ij^T is then
+// the fp32 pair Mm[8i + g][8j + 2 l4 .. + 1].  No shared-memory round trip and no barrier between dependent products:
+// one product is ~30 cycles of latency against ~1 K for a tcgen05 round trip, which is why this 64 x 64 solve is not
+// on the tcgen05 pipe.  RHS = beta R comes from the bf16 row tile `rhs` ([64][DVC], ldmatrix.trans); U goes back as a
+// bf16 row tile (stmatrix.trans) over V', T into rows 0..63 of the 128-row tile `tp`.
+template <int DVC>
+__device__ __forceinline__ void wy_solve(const float* Mm, const float* Tm, int n, int warp, int lane, uint32_t rhs_saddr,
+                                         uint32_t us_saddr, uint32_t tp_saddr)
+{
+    constexpr int NUW = DVC / 16;   // warps solving for U
+    const bool is_u = warp < NUW;
+    const int m0 = is_u ? 16 * warp : 16 * (warp - NUW);
+    if (!is_u && (warp >= NUW + 4 || m0 >= n)) return;
+    const int g = lane >> 2, l4 = lane & 3, nblk = n >> 3;
+    const int mat = lane >> 3, lr = lane & 7;   // ldmatrix / stmatrix: this lane addresses row lr of matrix `mat`
+    float x[8][4];
+    uint32_t init[4][4];
+    if (is_u) {
 #pragma unroll
-            for (int k = 0; k < 8; ++k) xv += Mm[mm_idx(o + 8 + i, o + k)] * Tm[mm_idx(o + k, o + j)];
-            Tm[mm_idx(o + 8 + i, o + j)] = xv;   // X = M21 T11 (these entries are read only below)
-        }
-        __syncthreads();
-        if (act) {
-#pragma unroll
-            for (int k = 0; k < 8; ++k) yv += Tm[mm_idx(o + 8 + i, o + 8 + k)] * Tm[mm_idx(o + 8 + k, o + j)];
-        }
-        __syncthreads();
-        if (act) Tm[mm_idx(o + 8 + i, o + j)] = -yv;
+        for (int ip = 0; ip < 4; ++ip)
+            if (2 * ip < nblk) ldsm_x4_trans(init[ip], rhs_saddr + tile_chunk_off(64, 8 * (2 * ip + (mat >> 1)) + lr, m0 / 8 + (mat & 1)));
     }
-    __syncthreads();
-    // n = 64: the bf16 tile `tp` (rows 0..63 of a 128-row tile, zero above the diagonal) is written as the blocks become
-    // final, by the warps the tensor-core levels leave idle; the last level writes it from its accumulators.
-    const bool fused = n == 64 && nthreads > 128;
-    auto put8 = [&](int r, int ch, bool zero) {   // 8 columns [8 ch, 8 ch + 8) of row r
-        float f[8];
-        if (zero) {
 #pragma unroll
-            for (int e = 0; e < 8; ++e) f[e] = 0.f;
-        } else {
-            *reinterpret_cast<float4*>(f) = *reinterpret_cast<const float4*>(&Tm[mm_idx(r, 8 * ch)]);
-            *reinterpret_cast<float4*>(f + 4) = *reinterpret_cast<const float4*>(&Tm[mm_idx(r, 8 * ch + 4)]);
-        }
-        sts128(tp + tile_chunk_off(128, r, ch), pack8(f));
-    };
-    if (fused && warp >= 4) {
-        // each row's diagonal 16-block (final after step 1) and the zeros to its right
-        for (int it = tid - 128; it < 64 * 8; it += nthreads - 128) {
-            const int r = it >> 3, ch = it & 7, d0 = 2 * (r >> 4);
-            if (ch >= d0) put8(r, ch, ch >= d0 + 2);
-        }
-    }
-    if (n >= 32) {
-        // level 32: blocks (1,0) and (3,2); warp = (pair, 8-column tile)
-        const int npair = n / 32;
-        if (warp < 2 * npair) {
-            const int pair = warp >> 1, nt = warp & 1, i0 = 32 * pair + 16, j0 = 32 * pair;
-            float d[1][4];
-            warp_prod<1, 2>(d, Mm, i0, j0, Tm, j0, j0 + 8 * nt, lane);   // X = M_ij T_jj
-            warp_store<1>(Tm, i0, j0 + 8 * nt, d, 1.f, lane);
-            __syncwarp();
-            warp_prod<1, 2>(d, Tm, i0, i0, Tm, i0, j0 + 8 * nt, lane);   // T_ii X
-            __syncwarp();
-            warp_store<1>(Tm, i0, j0 + 8 * nt, d, -1.f, lane);
-        }
-        __syncthreads();
-    }
-    if (n >= 64) {
-        // level 64: rows 32..63 x cols 0..31; warp = 8-column tile
-        if (warp < 4) {
-            float d[2][4];
-            warp_prod<2, 4>(d, Mm, 32, 0, Tm, 0, 8 * warp, lane);
-            warp_store<2>(Tm, 32, 8 * warp, d, 1.f, lane);
-            __syncwarp();
-            warp_prod<2, 4>(d, Tm, 32, 32, Tm, 32, 8 * warp, lane);
-            if (fused) {
-                const int g = lane >> 2, l4 = lane & 3;
-#pragma unroll
-                for (int m = 0; m < 2; ++m) {
-                    const int r0 = 32 + 16 * m + g;
-                    *reinterpret_cast<uint32_t*>(tp + tile_chunk_off(128, r0, warp) + 4 * l4) = pack_bf16(-d[m][0], -d[m][1]);
-                    *reinterpret_cast<uint32_t*>(tp + tile_chunk_off(128, r0 + 8, warp) + 4 * l4) = pack_bf16(-d[m][2], -d[m][3]);
-                }
+    for (int i = 0; i < 8; ++i) {
+        if (i < nblk) {
+            float y[4];
+            if (is_u) {
+                const uint32_t w0 = init[i >> 1][2 * (i & 1)], w1 = init[i >> 1][2 * (i & 1) + 1];
+                y[0] = bf16_lo(w0); y[1] = bf16_hi(w0); y[2] = bf16_lo(w1); y[3] = bf16_hi(w1);
             } else {
-                __syncwarp();
-                warp_store<2>(Tm, 32, 8 * warp, d, -1.f, lane);
+                const int t0 = 8 * i + 2 * l4;
+                y[0] = (m0 + g == t0) ? 1.f : 0.f; y[1] = (m0 + g == t0 + 1) ? 1.f : 0.f;
+                y[2] = (m0 + g + 8 == t0) ? 1.f : 0.f; y[3] = (m0 + g + 8 == t0 + 1) ? 1.f : 0.f;
             }
-        } else if (fused) {
-            // the level-32 blocks (rows 16..31 x cols 0..15, rows 48..63 x cols 32..47) are final
-            for (int it = tid - 128; it < 64; it += nthreads - 128) {
-                const int hi = it >> 5, r = 16 + 32 * hi + ((it >> 1) & 15), ch = 4 * hi + (it & 1);
-                put8(r, ch, false);
-            }
-        }
-    }
-    if (!fused) {
-        __syncthreads();
-        const int tr_ = tid >> 2, qq = tid & 3;  // row, 16-column quarter
-        if (tr_ < n) {
+            float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};   // two chains: even / odd j
 #pragma unroll
-            for (int k8 = 0; k8 < 2; ++k8) {
-                float f[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int s_ = 16 * qq + 8 * k8 + e;
-                    f[e] = s_ <= tr_ ? Tm[mm_idx(tr_, s_)] : 0.f;
+            for (int j = 0; j < 8; ++j) {
+                if (j < i) {
+                    const float2 nb = *reinterpret_cast<const float2*>(&Mm[mm_idx(8 * i + g, 8 * j + 2 * l4)]);
+                    const uint32_t af[4] = {__float_as_uint(x[j][0]), __float_as_uint(x[j][2]), __float_as_uint(x[j][1]),
+                                            __float_as_uint(x[j][3])};
+                    const uint32_t bf[2] = {__float_as_uint(nb.x), __float_as_uint(nb.y)};
+                    if (j & 1) mma_tf32(s1, af, bf); else mma_tf32(s0, af, bf);
                 }
-                sts128(tp + tile_chunk_off(128, tr_, 2 * qq + k8), pack8(f));
+            }
+#pragma unroll
+            for (int e = 0; e < 4; ++e) y[e] -= s0[e] + s1[e];
+            const float2 tb = *reinterpret_cast<const float2*>(&Tm[mm_idx(8 * i + g, 8 * i + 2 * l4)]);
+            const uint32_t af[4] = {__float_as_uint(y[0]), __float_as_uint(y[2]), __float_as_uint(y[1]), __float_as_uint(y[3])};
+            const uint32_t bf[2] = {__float_as_uint(tb.x), __float_as_uint(tb.y)};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) x[i][e] = 0.f;
+            mma_tf32(x[i], af, bf);
+            if (i & 1) {   // blocks i-1, i complete: four 8x8 bf16 matrices (block, channel half), rows = tokens
+                const uint32_t w[4] = {pack_bf16(x[i - 1][0], x[i - 1][1]), pack_bf16(x[i - 1][2], x[i - 1][3]),
+                                       pack_bf16(x[i][0], x[i][1]), pack_bf16(x[i][2], x[i][3])};
+                const int tok = 8 * (i - 1 + (mat >> 1)) + lr, ch = m0 / 8 + (mat & 1);
+                stsm_x4_trans(is_u ? us_saddr + tile_chunk_off(64, tok, ch) : tp_saddr + tile_chunk_off(128, tok, ch), w);
             }
         }
     }
@@ -270,7 +196,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     constexpr int REC_TID = NTH - 64;
     constexpr int HK = DK / NP, HV = DV / NP;  // columns per warpgroup ("half" = part index 0..NP-1)
     extern __shared__ uint8_t smem_raw[];
-    uint8_t* sm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    // 1024-byte alignment by an offset from the __shared__ array (not by integer rounding of a generic pointer), so
+    // that the compiler still knows these are shared-memory addresses: LDS/STS with 32-bit address arithmetic
+    // instead of generic LD/ST with 64-bit arithmetic.
+    uint8_t* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     const int r = a.r, R2 = 2 * r;
     const Layout Lo(DK, DV, R2);
     Misc& mi = *reinterpret_cast<Misc*>(sm + Lo.misc);
@@ -395,13 +324,17 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 0);
         // ---- P0: fold G^T = S^T Ucat^T -> TM_X2[0, R2)
         PHASE_SYNC();
+        PROF(g_prof_fwd, 20);
         if (rc && tid == REC_TID) {   // record: state entering the chunk (Sb stays intact until P13)
             bulk_s2g(rc + Rc.SB, sb + Lo.Sb, (uint32_t)state_tile);
             bulk_commit();
         }
-        if (fold_now && tid == 0) {
-            mma_rt<128, MNMAJ, KMAJ>(tmem + TM_X2, R2, sb + Lo.Sb, DV, 0, sb + Lo.Ucat, R2, 0, DV, false);
-            umma_commit(&mi.bar_mma);
+        if (fold_now && warp == 0) {
+            if (elect_one()) {
+                mma_rt<128, MNMAJ, KMAJ, DV>(tmem + TM_X2, R2, sb + Lo.Sb, DV, 0, sb + Lo.Ucat, R2, 0, DV, false);
+                umma_commit(&mi.bar_mma);
+            }
+            __syncwarp();
         }
         // meanwhile: raw k, q have landed -> partial sums of squares; beta
         mbar_wait(&mi.bar_kq, tma_ph);
@@ -423,6 +356,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 if (rc) reinterpret_cast<float*>(rc + Rc.beta)[t] = bt;
             }
         }
+        PROF(g_prof_fwd, 21);
         if (fold_now) {
             WAIT_MMA();
             PROF(g_prof_fwd, 1);
@@ -479,9 +413,12 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 2);
         // ---- P2: Z = [k;q] G^T -> TM_X2[32, 32+R2)
         PHASE_SYNC();
-        if (tid == 0) {
-            mma_rt<128, KMAJ, MNMAJ>(tmem + TM_X2 + 32, R2, sb + Lo.KQraw, 128, 0, sb + Lo.Vcat, DM, 32, DK, false);
-            umma_commit(&mi.bar_mma);
+        if (warp == 0) {
+            if (elect_one()) {
+                mma_rt<128, KMAJ, MNMAJ, DK>(tmem + TM_X2 + 32, R2, sb + Lo.KQraw, 128, 0, sb + Lo.Vcat, DM, 32, DK, false);
+                umma_commit(&mi.bar_mma);
+            }
+            __syncwarp();
         }
         WAIT_MMA();
         PROF(g_prof_fwd, 3);
@@ -535,10 +472,13 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 4);
         // ---- P4: b_proj = [tt_b;tt_b] Vb^T -> TM_X1, w_proj = [tt_w;tt_w] Vw^T -> TM_X2 (both row halves get both)
         PHASE_SYNC();
-        if (tid == 0) {
-            umma_tiles_rt<KMAJ, KMAJ>(tmem + TM_X1, 128, DK, sb + Lo.Y1, 128, 0, 0, sb + Lo.Vcat, DM, 0, 0, 16, false);
-            umma_tiles_rt<KMAJ, KMAJ>(tmem + TM_X2, 128, DV, sb + Lo.Y1, 128, 0, 16, sb + Lo.Vcat, DM, 0, 16, 16, false);
-            umma_commit(&mi.bar_mma);
+        if (warp == 0) {
+            if (elect_one()) {
+                umma_prod<KMAJ, KMAJ, 16>(tmem + TM_X1, 128, DK, sb + Lo.Y1, 128, 0, 0, sb + Lo.Vcat, DM, 0, 0, 16, false);
+                umma_prod<KMAJ, KMAJ, 16>(tmem + TM_X2, 128, DV, sb + Lo.Y1, 128, 0, 16, sb + Lo.Vcat, DM, 0, 16, 16, false);
+                umma_commit(&mi.bar_mma);
+            }
+            __syncwarp();
         }
         mbar_wait(&mi.bar_fb, tma_ph);
         mbar_wait(&mi.bar_wv, tma_ph);
@@ -606,10 +546,14 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 6);
         // ---- P6: block-local prefix sums -> TM_X2[0, DK): rows 0..63 a_b - lg_t, rows 64..127 lg_t - a_b
         PHASE_SYNC();
-        if (tid == 0) {
-            mma_rt<128, KMAJ, MNMAJ>(tmem + TM_X2, DK, sb + Lo.Y2, 128, 0, sb + Lo.Y0, 64, 0, LCc, false);
-            mma_rt<128, KMAJ, MNMAJ>(tmem + TM_X2, DK, sb + Lo.Y2, 128, 0, sb + Lo.Y1, 64, 0, LCc, true);
-            umma_commit(&mi.bar_mma);
+        PROF(g_prof_fwd, 25);
+        if (warp == 0) {
+            if (elect_one()) {
+                mma_rt<128, KMAJ, MNMAJ, LC>(tmem + TM_X2, DK, sb + Lo.Y2, 128, 0, sb + Lo.Y0, 64, 0, LCc, false);
+                mma_rt<128, KMAJ, MNMAJ, LC>(tmem + TM_X2, DK, sb + Lo.Y2, 128, 0, sb + Lo.Y1, 64, 0, LCc, true);
+                umma_commit(&mi.bar_mma);
+            }
+            __syncwarp();
         }
         WAIT_MMA();
         PROF(g_prof_fwd, 7);
@@ -748,16 +692,21 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 9);
         // ---- P8: A|P blocks (one 16-column block per anchoring) and the state products
         PHASE_SYNC();
-        if (tid == 0) {
-            const int nb = LCc >> 4;
-            mma_rt<128, KMAJ, KMAJ>(tmem + TM_X2, 16, sb + Lo.KQbar, 128, 0, sb + Lo.Y1, 64, 0, DK, false);
-            if (nb > 1) mma_rt<128, KMAJ, KMAJ>(tmem + TM_X2 + 16, 16, sb + Lo.Y2, 96, 0, sb + Lo.Y1, 64, 16, DK, false);
-            if (nb > 2) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 32, 16, sb + Lo.Y0, 64, 0, sb + Lo.Y1, 64, 32, DK, false);
-            if (nb > 3) mma_rt<64, KMAJ, KMAJ>(tmem + TM_X2 + 48, 16, sb + Lo.Y2 + tile_bytes(96, DK), 32, 0, sb + Lo.Y1, 64, 48, DK, false);
-            umma_commit(&mi.bar_mma);   // the A|P blocks: P9a starts on them while the state products still run
-            mma_rt<128, KMAJ, KMAJ>(tmem + TM_ACC, DV, sb + Lo.KQbar, 128, 0, sb + Lo.Sb, DV, 0, DK, false);
-            umma_commit(&mi.bar_acc);
+        PROF(g_prof_fwd, 18);
+        if (warp == 0) {
+            if (elect_one()) {
+                const int nb = LCc >> 4;
+                mma_rt<128, KMAJ, KMAJ, DK>(tmem + TM_X2, 16, sb + Lo.KQbar, 128, 0, sb + Lo.Y1, 64, 0, DK, false);
+                if (nb > 1) mma_rt<128, KMAJ, KMAJ, DK>(tmem + TM_X2 + 16, 16, sb + Lo.Y2, 96, 0, sb + Lo.Y1, 64, 16, DK, false);
+                if (nb > 2) mma_rt<64, KMAJ, KMAJ, DK>(tmem + TM_X2 + 32, 16, sb + Lo.Y0, 64, 0, sb + Lo.Y1, 64, 32, DK, false);
+                if (nb > 3) mma_rt<64, KMAJ, KMAJ, DK>(tmem + TM_X2 + 48, 16, sb + Lo.Y2 + tile_bytes(96, DK), 32, 0, sb + Lo.Y1, 64, 48, DK, false);
+                umma_commit(&mi.bar_mma);   // the A|P blocks: P9a starts on them while the state products still run
+                mma_rt<128, KMAJ, KMAJ, DK>(tmem + TM_ACC, DV, sb + Lo.KQbar, 128, 0, sb + Lo.Sb, DV, 0, DK, false);
+                umma_commit(&mi.bar_acc);
+            }
+            __syncwarp();
         }
+        PROF(g_prof_fwd, 19);
         {
             const int nb = LCc >> 4;
             if (rc && tid == REC_TID) {
@@ -884,55 +833,35 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         __syncthreads();
         PROF(g_prof_fwd, 12);
-        // ---- P9c: T = (I + beta A)^-1 -> TP rows 0..63 (bf16, zero above the diagonal)
-        tri_inverse(Mm, Tm, LCc, tid, NTH, sm + Lo.TP);
-        PROF(g_prof_fwd, 13);
-        // ---- P10: U = T (beta R) -> TM_X1
-        PHASE_SYNC();
-        if (tid == 0) {
-            mma_rt<128, KMAJ, MNMAJ>(tmem + TM_X1, DV, sb + Lo.TP, 128, 0, sb + Lo.Y2, 64, 0, LCc, false);
-            umma_commit(&mi.bar_mma);
-            if (c + 1 < nchunks) issue_kq(c + 1);
-        }
-        if (rc && tid == REC_TID) {   // record [scale.P ; T]: the two row halves of TP swapped (TP is next written in P9 of the next chunk)
-            if (s1) bulk_s2g(rc + Rc.PT, sb + Lo.TP + 8192, 8192);
-            bulk_s2g(rc + Rc.PT + 8192, sb + Lo.TP, 8192);
-            bulk_commit();
-        }
-        WAIT_MMA();
-        PROF(g_prof_fwd, 14);
-        // ---- P11: U -> bf16 rows (over V')
-        if (krole && warp_active) {
-            uint32_t v[32];
-            tmem_ld32(tmem + TM_X1 + lane_base + half * HV, v);
-            tmem_wait_ld();
-            if (live) {
-#pragma unroll
-                for (int ch = 0; ch < 4; ++ch) {
-                    float f[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) f[e] = __uint_as_float(v[8 * ch + e]);
-                    sts128(sm + Lo.Us + tile_chunk_off(64, t, half * 4 + ch), pack8(f));
-                }
-            }
-        }
-        // the record copies issued so far have left their buffers: the next chunk's loads (below) and P13 may overwrite them
+        // ---- P9c: WY solve U = (I + beta A)^-1 (beta R) in registers (tf32 mma.sync) -> bf16 rows over V'; T -> TP rows 0..63
+        diag8_inverse(Mm, Tm, LCc, tid);
+        __syncthreads();
+        wy_solve<DV>(Mm, Tm, LCc, warp, lane, sb + Lo.Y2, sb + Lo.Us, sb + Lo.TP);
+        // the record copies issued so far have left their buffers: the next chunk's loads (P13) may overwrite them
         if (rc && tid == REC_TID) bulk_wait_read();
-        PROF(g_prof_fwd, 15);
+        PROF(g_prof_fwd, 13);
         // ---- P12: O += P U;  W = U^T Ktil -> TM_X2
         PHASE_SYNC();
-        if (tid == 0) {
-            mma_rt<128, KMAJ, MNMAJ>(tmem + TM_ACC, DV, sb + Lo.TP, 128, 0, sb + Lo.Us, 64, 0, LCc, true);
-            mma_rt<128, MNMAJ, MNMAJ>(tmem + TM_X2, DK, sb + Lo.Us, 64, 0, sb + Lo.Ktil, 64, 0, LCc, false);
-            umma_commit(&mi.bar_mma);
-            if (rc) {   // record U (its buffer is refilled by the next chunk's loads below)
-                bulk_s2g(rc + Rc.U, sb + Lo.Us, tile_bytes(64, DV));
-                bulk_commit();
-                bulk_wait_read();
+        PROF(g_prof_fwd, 22);
+        if (warp == 0) {
+            if (elect_one()) {
+                mma_rt<128, KMAJ, MNMAJ, LC>(tmem + TM_ACC, DV, sb + Lo.TP, 128, 0, sb + Lo.Us, 64, 0, LCc, true);
+                mma_rt<128, MNMAJ, MNMAJ, LC>(tmem + TM_X2, DK, sb + Lo.Us, 64, 0, sb + Lo.Ktil, 64, 0, LCc, false);
+                umma_commit(&mi.bar_mma);
+                if (c + 1 < nchunks) issue_kq(c + 1);   // the inverse scratch (over the raw k|q tile at d = 128) is consumed
             }
+            __syncwarp();
         }
+        if (rc && tid == REC_TID) {
+            // record [scale.P ; T] (the two row halves of TP swapped; TP is next written in P9 of the next chunk) and U
+            // (its buffer is refilled by the next chunk's loads, issued by this thread at the end of P13)
+            if (s1) bulk_s2g(rc + Rc.PT, sb + Lo.TP + 8192, 8192);
+            bulk_s2g(rc + Rc.PT + 8192, sb + Lo.TP, 8192);
+            bulk_s2g(rc + Rc.U, sb + Lo.Us, tile_bytes(64, DV));
+            bulk_commit();
+        }
+        PROF(g_prof_fwd, 23);
         WAIT_MMA();
-        if (tid == 0 && c + 1 < nchunks) { fence_async_smem(); issue_fb(c + 1); issue_wv(c + 1); }
         PROF(g_prof_fwd, 16);
         // ---- P13: outputs and the state carry
         if (!krole && warp_active) {
@@ -979,6 +908,11 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
               tmem_st16(tmem + TM_S + lane_base + half * HK + 16 * s16, sv16);
             }
             tmem_wait_st();
+        }
+        if (tid == REC_TID && c + 1 < nchunks) {   // U has left its buffer: the next chunk's gate and value tiles
+            if (rc) bulk_wait_read();
+            fence_async_smem();
+            issue_fb(c + 1); issue_wv(c + 1);
         }
         tma_ph ^= 1u;
         PROF(g_prof_fwd, 17);
@@ -1028,7 +962,7 @@ bool tc_make_token_map(CUtensorMap* map, const void* base, int B, int T, int H, 
 extern "C" void carve_debug_prof_fwd(unsigned long long* out)
 {
     cudaMemcpyFromSymbol(out, g_prof_fwd, sizeof(g_prof_fwd));
-    unsigned long long z[40] = {};
+    unsigned long long z[80] = {};
     cudaMemcpyToSymbol(g_prof_fwd, z, sizeof(z));
 }
 #endif

@@ -16,14 +16,14 @@
 #include <stdint.h>
 
 // Optional per-phase cycle counters (build with -DCARVE_PROFILE; block 0: thread 0 = the MMA-issuing, K-side
-// thread in slots 0.., thread 64 = a Q-side thread in slots 20..).
+// thread in slots 0.., thread 64 = a Q-side thread in slots 40..).
 #ifdef CARVE_PROFILE
-#define PROF_DECL(name) static __device__ unsigned long long name[40];
+#define PROF_DECL(name) static __device__ unsigned long long name[80];
 #define PROF_INIT() long long prof_t_ = clock64();
 #define PROF(name, i)                                                              \
     if (blockIdx.x == 0 && (threadIdx.x == 0 || threadIdx.x == 64)) {              \
         const long long prof_n_ = clock64();                                       \
-        name[(threadIdx.x ? 20 : 0) + i] += (unsigned long long)(prof_n_ - prof_t_); \
+        name[(threadIdx.x ? 40 : 0) + i] += (unsigned long long)(prof_n_ - prof_t_); \
         prof_t_ = prof_n_;                                                         \
     }
 #else
@@ -258,6 +258,33 @@ __device__ __forceinline__ void umma_tiles_rt(uint32_t d_tmem, int M, int N, uin
     uint64_t bd = BMAJ == KMAJ ? desc_kmajor(b_saddr, b_rows, b_o0, b_k0) : desc_mnmajor(b_saddr, b_rows, b_o0, b_k0);
     for (int k = 0; k < K; k += 16) {
         umma(d_tmem, ad, bd, idesc, (accumulate || k > 0) ? 1u : 0u);
+        ad = desc_next<AMAJ>(ad, a_rows, a_k0 + k);
+        bd = desc_next<BMAJ>(bd, b_rows, b_k0 + k);
+    }
+}
+
+// One lane of a converged warp (the same one every time): the thread that issues tcgen05.mma / commit / TMA.
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t el;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(el));
+    return el != 0;
+}
+
+// As umma_tiles_rt, fully unrolled over K <= KMAX (slices beyond the run-time K are predicated off): issued from a
+// warp-uniform branch by the elected lane this costs ~20 cycles per instruction instead of ~90 for the rolled loop
+// inside a divergent `if (tid == 0)` (measured; the compiler wraps every tcgen05.mma of a divergent region in an
+// ELECT / R2UR.BROADCAST loop and keeps the descriptor arithmetic on the slow uniform datapath).
+template <int AMAJ, int BMAJ, int KMAX>
+__device__ __forceinline__ void umma_prod(uint32_t d_tmem, int M, int N, uint32_t a_saddr, int a_rows, int a_o0, int a_k0,
+                                          uint32_t b_saddr, int b_rows, int b_o0, int b_k0, int K, bool accumulate)
+{
+    const uint32_t idesc = umma_idesc(M, N, AMAJ, BMAJ);
+    uint64_t ad = AMAJ == KMAJ ? desc_kmajor(a_saddr, a_rows, a_o0, a_k0) : desc_mnmajor(a_saddr, a_rows, a_o0, a_k0);
+    uint64_t bd = BMAJ == KMAJ ? desc_kmajor(b_saddr, b_rows, b_o0, b_k0) : desc_mnmajor(b_saddr, b_rows, b_o0, b_k0);
+#pragma unroll
+    for (int k = 0; k < KMAX; k += 16) {
+        if (k < K) umma(d_tmem, ad, bd, idesc, (accumulate || k > 0) ? 1u : 0u);
         ad = desc_next<AMAJ>(ad, a_rows, a_k0 + k);
         bd = desc_next<BMAJ>(bd, b_rows, b_k0 + k);
     }

@@ -126,6 +126,23 @@ def make_inputs(cfg: Config, zero_content: bool = False, with_decay_params: bool
     return x
 
 
+def scale_qk_rows(x: dict, cfg: Config, lo: float = 0.5, hi: float = 2.0, tiny_rows: int = 0, seed: int = 11) -> dict:
+    """Un-normalise q and k: multiply every token row by its own factor ~ U(lo, hi), so that the operator's
+    L2-norm step (and the 1/|x| factor of its backward) has real work to do.  `tiny_rows` rows of each tensor
+    get a norm of ~1e-3 = sqrt(eps) instead, where the eps inside the square root matters.  Re-rounds to bf16."""
+    rng = np.random.Generator(np.random.PCG64([cfg.seed, seed]))
+    out = dict(x)
+    for name in ("q", "k"):
+        a = np.array(x[name], dtype=np.float32, copy=True)
+        sc = rng.uniform(lo, hi, size=a.shape[:-1] + (1,)).astype(np.float32)
+        if tiny_rows:
+            flat = sc.reshape(-1)
+            flat[rng.choice(flat.size, size=min(tiny_rows, flat.size), replace=False)] = np.float32(1e-3)
+        a *= sc
+        out[name] = bf16_round(a) if cfg.dtype == "bf16" else a
+    return out
+
+
 def make_cotangents(cfg: Config) -> dict:
     """dO ~ N(0,1) in the token dtype and dS_final ~ N(0, 0.01^2) fp32 (drawn after the inputs)."""
     rng = np.random.Generator(np.random.PCG64([cfg.seed, 1]))

@@ -45,6 +45,15 @@ def test_config0_fp32(oracle, zero_content, l2norm):
     _check_fwd_bwd(oracle, cfg, x)
 
 
+@pytest.mark.parametrize("l2norm", [1, 0])
+def test_config0_fp32_unnormalised_qk(oracle, l2norm):
+    """Config 0 with every q, k row rescaled by U(0.5, 2): row a0 (Fig. 2 l.437, Alg. 3 step 3 l.399) on the fp32 path,
+    forward (rsqrt scale) and backward (dq = (dq^ - q^<q^,dq^>)/|q|), with and without the in-kernel normalisation."""
+    cfg = synth.CFG0.with_(qk_l2norm=l2norm, wstd=0.1)
+    x = synth.scale_qk_rows(synth.make_inputs(cfg), cfg)
+    _check_fwd_bwd(oracle, cfg, x)
+
+
 # ---- small cases spanning several sub-chunks, every chunk length, ragged structure -------------
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 @pytest.mark.parametrize("L", [16, 32, 64, 128])
@@ -170,9 +179,26 @@ def test_host_entry_point_matches_device_entry_point(oracle, B):
 def test_kernel_families_bf16(oracle, path, dk, r, L):
     """Several chunks, several 16-token anchor blocks, nonzero S0, active content gates, A and tau present."""
     cfg = synth.Config("t", B=2, H=2, T=256, L=L, dk=dk, dv=dk, r=r, dtype="bf16", wstd=0.1, s0_std=0.05, seed=dk + L)
-    x = synth.make_inputs(cfg, with_decay_params=True)
+    x = synth.scale_qk_rows(synth.make_inputs(cfg, with_decay_params=True), cfg)   # un-normalised q, k (row a0)
     p = params_of(cfg, path=path)
     assert carve.carve_resolved_path(p, True) == path
+    _check_fwd_bwd(oracle, cfg, x, path=path)
+
+
+@pytest.mark.parametrize("path", [carve.CARVE_PATH_SIMT, carve.CARVE_PATH_TENSOR])
+@pytest.mark.parametrize("sigma", [0.3, 3.0])
+@pytest.mark.parametrize("l2norm", [1, 0])
+def test_unnormalised_qk_both_paths(oracle, path, sigma, l2norm):
+    """q, k rows of norm ~ sigma.U(0.5,2) (and, with the normalisation on, four rows of norm ~ sqrt(eps), where the eps
+    inside the square root decides the result): pins the rsqrt(|x|^2 + eps) scale and the 1/|x| factor of its backward
+    on both kernel families.  With qk_l2norm = 0 the same rows go in as given (a smaller range, so that the un-normalised
+    coupling matrix stays well conditioned)."""
+    cfg = synth.Config("t", B=2, H=2, T=128, L=64, dk=64, dv=64, r=8, dtype="bf16", wstd=0.1, s0_std=0.05,
+                       qk_l2norm=l2norm, seed=int(10 * sigma) + l2norm)
+    if l2norm:
+        x = synth.scale_qk_rows(synth.make_inputs(cfg), cfg, 0.5 * sigma, 2.0 * sigma, tiny_rows=4)
+    else:
+        x = synth.scale_qk_rows(synth.make_inputs(cfg), cfg, 0.6, 1.2)
     _check_fwd_bwd(oracle, cfg, x, path=path)
 
 
@@ -207,54 +233,7 @@ def test_tensor_path_determinism(oracle):
         assert np.array_equal(outs[0][2][n], outs[1][2][n]), n
 
 
-# ---- BASELINE.json config 1 at full size, in the launch configuration bench.py times ------------------
-def _check_full_size_sampled_chains(oracle, cfg, chains):
-    x, ct = synth.make_inputs(cfg), synth.make_cotangents(cfg)
-    p = params_of(cfg)
-    assert carve.carve_resolved_path(p, True) == carve.CARVE_PATH_TENSOR
-    O, Sf, h = run_fwd(p, x, need_bwd=True)
-    g, _ = run_bwd(p, h, ct)
-    tol = TOL["bf16"]
-    for b, hh in chains:
-        xs = synth.slice_chains(x, [(b, hh)])
-        cts = synth.slice_chains(ct, [(b, hh)])
-        s = oracle_shape(oracle, cfg, B=1, H=1)
-        O_ref, S_ref = oracle.fwd(s, xs)
-        g_ref = oracle.bwd(s, xs, cts["dO"], cts["dS_final"])
-        assert relerr(O[b:b + 1, :, hh:hh + 1], O_ref) <= tol["O"]
-        assert relerr(Sf[b:b + 1, hh:hh + 1], S_ref) <= tol["S"]
-        for n in ("dq", "dk", "dv", "df", "dbx", "dwx"):
-            assert relerr(g[n][b:b + 1, :, hh:hh + 1], g_ref[n]) <= tol["g"], (n, b, hh)
-        assert relerr(g["dbeta"][b:b + 1, :, hh:hh + 1], g_ref["dbeta"]) <= tol["g"]
-        assert relerr(g["dS0"][b:b + 1, hh:hh + 1], g_ref["dS0"]) <= tol["g"]
-    xs = synth.slice_chains(x, chains)
-    cts = synth.slice_chains(ct, chains)
-    sub = cfg.with_(B=len(chains), H=1)
-    _check_fwd_bwd(oracle, sub, xs, ct=cts)
-
-
-def test_config1_full_size_sampled_chains(oracle):
-    """The whole 1.3B-like workload runs on the GPU (128 chains x 64 chunks); the oracle recomputes sampled
-    (batch, head) chains one by one -- chains are independent (Alg. 2 l.318) -- for every per-token output, S_final
-    and dS0.  The shared-weight gradients sum over all chains, so they are checked on the sampled chains run as
-    their own B'=3, H'=1 problem at full T."""
-    _check_full_size_sampled_chains(oracle, synth.CFG1, [(0, 0), (3, 7), (7, 15)])
-
-
-def test_config4_full_size_sampled_chains(oracle):
-    """Config 4 at full size: 2048 chains, i.e. many more chains than SMs (several waves of the per-chain grid),
-    with its stress structure (beta = 1 on 10 % of tokens, no decay on 10 % of key dims).  Same sampling as config 1;
-    the sampled chains include the first and the last one and one from the middle waves."""
-    _check_full_size_sampled_chains(oracle, synth.CFG4, [(0, 0), (29, 13), (63, 31)])
-
-
-@pytest.mark.parametrize("L", [16, 128])
-def test_config2_full_size_sampled_chains(oracle, L):
-    """Config 2 at full size (64 chains, T = 8192, active content gates) at the two ends of the chunk-length sweep:
-    L = 16 (512 fold reads per chain) and L = 128 (a gate chunk spans two solve chunks)."""
-    _check_full_size_sampled_chains(oracle, synth.CFG2[L], [(0, 0), (2, 9), (3, 15)])
-
-
+# ---- BASELINE.json configs at full size, every tensor of every chain: tests/test_gpu_fullsize.py ------------------
 @pytest.mark.parametrize("L", [16, 32, 64, 128])
 def test_config2_chunk_sweep_reduced_batch(oracle, L):
     """Config 2 (chunk-length sweep, gate projections ~N(0,0.1^2)) at full T = 8192 with B*H reduced to 2 chains."""
@@ -277,28 +256,12 @@ def test_config3_long_context_forward_reduced_heads(oracle):
     _check_fwd_bwd(oracle, cfg, x, with_bwd=False)
 
 
-def test_config3_full_size_sampled_chains(oracle):
-    """Config 3 at full size (16 chains x 1024 chunks, d_v = 256 split over a two-CTA cluster, random S0, forward
-    only): the whole workload runs on the GPU, the oracle recomputes the first and the last chain."""
-    cfg = synth.CFG3
-    x = synth.make_inputs(cfg)
-    p = params_of(cfg)
-    O, Sf, _ = run_fwd(p, x, need_bwd=False)
-    assert np.isfinite(O).all() and np.isfinite(Sf).all()
-    tol = TOL["bf16"]
-    s = oracle_shape(oracle, cfg, B=1, H=1)
-    for b, hh in [(0, 0), (0, 15)]:
-        O_ref, S_ref = oracle.fwd(s, synth.slice_chains(x, [(b, hh)]))
-        assert relerr(O[b:b + 1, :, hh:hh + 1], O_ref) <= tol["O"], (b, hh)
-        assert relerr(Sf[b:b + 1, hh:hh + 1], S_ref) <= tol["S"], (b, hh)
-
-
 @pytest.mark.parametrize("B,H,T,L,d,r,seed", [(3, 5, 64, 64, 128, 8, 101), (1, 3, 192, 64, 128, 16, 102), (2, 1, 32, 16, 64, 16, 103),
                                               (1, 7, 384, 128, 128, 16, 104), (5, 2, 96, 32, 64, 8, 105)])
 def test_tensor_path_odd_shapes(oracle, B, H, T, L, d, r, seed):
     """Single-chunk sequences, odd batch / head counts, every supported r, nonzero S0, A and tau present."""
     cfg = synth.Config("t", B=B, H=H, T=T, L=L, dk=d, dv=d, r=r, dtype="bf16", wstd=0.1, s0_std=0.05, seed=seed)
-    x = synth.make_inputs(cfg, with_decay_params=True)
+    x = synth.scale_qk_rows(synth.make_inputs(cfg, with_decay_params=True), cfg)   # un-normalised q, k (row a0)
     _check_fwd_bwd(oracle, cfg, x, path=carve.CARVE_PATH_TENSOR)
 
 
