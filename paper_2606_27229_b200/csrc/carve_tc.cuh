@@ -119,8 +119,30 @@ struct Misc {
 
 static_assert(sizeof(Misc) <= 8192, "misc area too small");
 
-__device__ __forceinline__ float softplus_fast(float x) { return fmaxf(x, 0.f) + __logf(1.f + __expf(-fabsf(x))); }
-__device__ __forceinline__ float sigmoid_fast(float x) { return __fdividef(1.f, 1.f + __expf(-x)); }
+// Bare MUFU transcendentals (flush-to-zero forms: no denormal range fix-up code around them; every use below either
+// has a result whose flush to 0 is the correct limit or an argument >= 1).
+__device__ __forceinline__ float ex2_ftz(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float lg2_ftz(float x)
+{
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_ftz(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+constexpr float kLog2e = 1.4426950408889634f, kLn2 = 0.6931471805599453f;
+__device__ __forceinline__ float exp_fast(float x) { return ex2_ftz(x * kLog2e); }
+__device__ __forceinline__ float softplus_fast(float x) { return fmaf(kLn2, lg2_ftz(1.f + ex2_ftz(-fabsf(x) * kLog2e)), fmaxf(x, 0.f)); }
+__device__ __forceinline__ float sigmoid_fast(float x) { return rcp_ftz(1.f + ex2_ftz(-x * kLog2e)); }
 __device__ __forceinline__ float tanh_fast(float x)
 {
     float y;

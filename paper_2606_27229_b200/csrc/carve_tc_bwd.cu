@@ -127,12 +127,15 @@ __device__ __forceinline__ uint4 ldg128(const uint8_t* p) { return __ldg(reinter
 __device__ __forceinline__ void stg128(void* p, uint4 v) { *reinterpret_cast<uint4*>(p) = v; }
 
 // Product over K (multiple of 16) from two row tiles, with explicit K offsets (tc_common.cuh umma_tiles_rt), M = 128.
-template <int AMAJ, int BMAJ>
+template <int AMAJ, int BMAJ, int KMAX>
 __device__ __forceinline__ void mma_k(uint32_t d_tmem, int N, uint32_t a_saddr, int a_rows, int a_o0, int a_k0,
                                       uint32_t b_saddr, int b_rows, int b_o0, int b_k0, int K, bool accumulate)
 {
-    umma_tiles_rt<AMAJ, BMAJ>(d_tmem, 128, N, a_saddr, a_rows, a_o0, a_k0, b_saddr, b_rows, b_o0, b_k0, K, accumulate);
+    umma_prod<AMAJ, BMAJ, KMAX>(d_tmem, 128, N, a_saddr, a_rows, a_o0, a_k0, b_saddr, b_rows, b_o0, b_k0, K, accumulate);
 }
+// The MMA / bulk-copy issuing thread: the elected lane of warp 0, inside a warp-uniform branch (tc_common.cuh umma_prod).
+#define LEADER_BEGIN if (warp == 0) { if (elect_one()) {
+#define LEADER_END } __syncwarp(); }
 
 // Column sums over the 32 lanes of a warp by a halving butterfly: on return lane l holds in v[0..N/32)
 // the sums of columns (N/32) l + i.
@@ -346,15 +349,15 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             }
         }
         // ---- L1: dU = Ktil dS'^T + (scale P)^T dO -> BM_A rows 0..63;  dKtil = U dS' -> BM_KT rows 0..63
-        if (tid == 0) {
+        LEADER_BEGIN
             mbar_wait(&mi.bar_g1, ph);
             mbar_wait(&mi.bar_pt, ph);
             tc_fence_after();
-            mma_k<KMAJ, KMAJ>(tmem + BM_A, D, sb + Lo.S[0], 64, 0, 0, sb + Lo.DSB, D, 0, 0, D, false);
-            mma_k<MNMAJ, MNMAJ>(tmem + BM_A, D, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[2], 128, 0, 64, LCc, true);
-            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D, sb + Lo.S[4], 64, 0, 0, sb + Lo.DSB, D, 0, 0, D, false);
+            mma_k<KMAJ, KMAJ, D>(tmem + BM_A, D, sb + Lo.S[0], 64, 0, 0, sb + Lo.DSB, D, 0, 0, D, false);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_A, D, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[2], 128, 0, 64, LCc, true);
+            mma_k<KMAJ, MNMAJ, D>(tmem + BM_KT, D, sb + Lo.S[4], 64, 0, 0, sb + Lo.DSB, D, 0, 0, D, false);
             umma_commit(&mi.bar_mma);
-        }
+        LEADER_END
         if (krole) {
             WAIT_MMA();
             if (warp_active) {
@@ -380,11 +383,11 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROF(g_prof_bwd, 1);
         // ---- L2: dX = T^T dU: columns x < D/2 -> BM_A rows 0..63 (K-side lanes), x >= D/2 -> rows 64..127 (Q-side lanes)
         PHASE_SYNC();
-        if (tid == 0) {
-            mma_k<MNMAJ, MNMAJ>(tmem + BM_A + D / 2, D / 2, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[0], 64, D / 2, 0, LCc, false);
-            mma_k<MNMAJ, MNMAJ>(tmem + BM_A, D / 2, sb + Lo.S[1], 64, 64, 0, sb + Lo.S[0], 64, 0, 0, LCc, false);
+        LEADER_BEGIN
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_A + D / 2, D / 2, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[0], 64, D / 2, 0, LCc, false);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_A, D / 2, sb + Lo.S[1], 64, 64, 0, sb + Lo.S[0], 64, 0, 0, LCc, false);
             umma_commit(&mi.bar_mma);
-        }
+        LEADER_END
         WAIT_MMA();
         if (tid == 0) {  // PT is dead: fetch the block-anchored column operand of L4
             mbar_expect_tx(&mi.bar_g4a, TB);
@@ -426,16 +429,16 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROF(g_prof_bwd, 2);
         // ---- L3: [dA;dP] raw, SP = [-dR;dO] S, dS += [-dR;dO]^T [Kbar; scale Qbar]
         PHASE_SYNC();
-        if (tid == 0) {
+        LEADER_BEGIN
             mbar_wait(&mi.bar_sb, ph);
             mbar_wait(&mi.bar_g3, ph);
             tc_fence_after();
-            mma_k<KMAJ, KMAJ>(tmem + BM_DAP, 64, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[4], 64, 0, 0, D, false);
-            mma_k<KMAJ, MNMAJ>(tmem + BM_A, D, sb + Lo.S[2], 128, 0, 0, sb + Lo.SBq, D, 0, 0, D, false);
-            mma_k<MNMAJ, MNMAJ>(tmem + BM_DS, D, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[5], 64, 0, 0, LCc, true);
-            mma_k<MNMAJ, MNMAJ>(tmem + BM_DS, D, sb + Lo.S[2], 128, 0, 64, sb + Lo.S[6], 64, 0, 0, LCc, true);
+            mma_k<KMAJ, KMAJ, D>(tmem + BM_DAP, 64, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[4], 64, 0, 0, D, false);
+            mma_k<KMAJ, MNMAJ, D>(tmem + BM_A, D, sb + Lo.S[2], 128, 0, 0, sb + Lo.SBq, D, 0, 0, D, false);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_DS, D, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[5], 64, 0, 0, LCc, true);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_DS, D, sb + Lo.S[2], 128, 0, 64, sb + Lo.S[6], 64, 0, 0, LCc, true);
             umma_commit(&mi.bar_mma);
-        }
+        LEADER_END
         if (!krole && half == 0 && live)
         {
             float sdb = 0.f;
@@ -758,14 +761,14 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         //      key channels j < D/2 in rows 0..63 (K-side lanes), j >= D/2 in rows 64..127 (Q-side lanes: the 0/1 tile
         //      used as the upper half of the M = 128 operand), so both threads of a token share the epilogue
         PHASE_SYNC();
-        if (tid == 0) {
+        LEADER_BEGIN
             const uint32_t tri = sb + Lo.TRI, trh = tri - 8192;
-            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D / 2, tri, 64, 0, 0, sb + Lo.S[2], 128, 0, 0, LCc, false);
-            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D / 2, tri, 64, 0, 64, sb + Lo.S[2], 128, 0, 64, LCc, true);
-            mma_k<KMAJ, MNMAJ>(tmem + BM_KT, D / 2, tri, 64, 0, 128, sb + Lo.S[4], 64, 0, 0, LCc, true);
-            mma_k<KMAJ, MNMAJ>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 0, sb + Lo.S[2], 128, D / 2, 0, LCc, false);
-            mma_k<KMAJ, MNMAJ>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 64, sb + Lo.S[2], 128, D / 2, 64, LCc, true);
-            mma_k<KMAJ, MNMAJ>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 128, sb + Lo.S[4], 64, D / 2, 0, LCc, true);
+            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT, D / 2, tri, 64, 0, 0, sb + Lo.S[2], 128, 0, 0, LCc, false);
+            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT, D / 2, tri, 64, 0, 64, sb + Lo.S[2], 128, 0, 64, LCc, true);
+            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT, D / 2, tri, 64, 0, 128, sb + Lo.S[4], 64, 0, 0, LCc, true);
+            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 0, sb + Lo.S[2], 128, D / 2, 0, LCc, false);
+            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 64, sb + Lo.S[2], 128, D / 2, 64, LCc, true);
+            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 128, sb + Lo.S[4], 64, D / 2, 0, LCc, true);
             umma_commit(&mi.bar_mma);
             // K0, Q0 are dead: fetch G^T of the chunk and the raw q rows for L8
             mbar_expect_tx(&mi.bar_g8, tile_bytes(D, 64));
@@ -774,7 +777,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             for (int cb = 0; cb < D / 64; ++cb) tma_load_3d(sm + Lo.S[6] + cb * 8192, &mq, &mi.bar_g5, cb * 64, h, trow);
             mbar_expect_tx(&mi.bar_bg, TB);   // the erase gate b over gamma_t/gamma_a (dead after L5)
             bulk_g2s(sm + Lo.FI, rc + Rc.Bg, TB, &mi.bar_bg);
-        }
+        LEADER_END
         {
             // dw_pre rows (written to dwx in L2) -> GW rows 64..127, [tt_b|0 ; 0|tt_w] -> S[1]: Q-side threads, loads first
             uint4 d4[HK / 8], t4[4];
@@ -830,12 +833,12 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROF(g_prof_bwd, 7);
         // ---- L7: ZZ = [db_pre; dw_pre] [Vb | Vw] -> BM_DAP;  dVb | dVw += [db_pre; dw_pre]^T TT2 -> BM_WG
         PHASE_SYNC();
-        if (tid == 0) {
-            mma_k<KMAJ, KMAJ>(tmem + BM_DAP, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.VcT, 32, 0, 0, D, false);
-            mma_k<MNMAJ, MNMAJ>(tmem + BM_WG, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[1], 128, 0, 0, LCc, !first);
-            mma_k<MNMAJ, MNMAJ>(tmem + BM_WG, 32, sb + Lo.S[2], 128, 0, 64, sb + Lo.S[1], 128, 0, 64, LCc, true);
+        LEADER_BEGIN
+            mma_k<KMAJ, KMAJ, D>(tmem + BM_DAP, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.VcT, 32, 0, 0, D, false);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_WG, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[1], 128, 0, 0, LCc, !first);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_WG, 32, sb + Lo.S[2], 128, 0, 64, sb + Lo.S[1], 128, 0, 64, LCc, true);
             umma_commit(&mi.bar_mma);
-        }
+        LEADER_END
         if (c > 0 && live) {   // next chunk's row-private L2 inputs -> L2 cache, so that the loads at its top are short
             const uint8_t* rn_ = rc - Rc.total;
 #pragma unroll
@@ -877,14 +880,14 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROF(g_prof_bwd, 8);
         // ---- L8: dq^ += dz G -> BM_A rows 64..127;  dG^T = q^T (dz/|q|) -> BM_DAP + 32
         PHASE_SYNC();
-        if (tid == 0) {
+        LEADER_BEGIN
             mbar_wait(&mi.bar_g8, ph);
             mbar_wait(&mi.bar_g5, ph);
             tc_fence_after();
-            mma_k<KMAJ, KMAJ>(tmem + BM_A, D, sb + Lo.S[0], 128, 0, 0, sb + Lo.S[5], D, 0, 0, R2, true);
-            mma_k<MNMAJ, MNMAJ>(tmem + BM_DAP + 32, 32, sb + Lo.S[6], 64, 0, 0, sb + Lo.S[4], 64, 0, 0, LCc, false);
+            mma_k<KMAJ, KMAJ, 32>(tmem + BM_A, D, sb + Lo.S[0], 128, 0, 0, sb + Lo.S[5], D, 0, 0, R2, true);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_DAP + 32, 32, sb + Lo.S[6], 64, 0, 0, sb + Lo.S[4], 64, 0, 0, LCc, false);
             umma_commit(&mi.bar_mma);
-        }
+        LEADER_END
         WAIT_MMA();
         if (tid == 0 && c > 0) issue_l1(c - 1);   // DZ, DZQ, GW, G^T, q are dead
         if (!krole && warp_active) {
@@ -939,11 +942,11 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         // ---- L9: fold glue: dS += [Ub;Uw]^T dG;  d[Ub;Uw]^T += S dG^T -> BM_WU
         if (gate_start) {
             PHASE_SYNC();
-            if (tid == 0) {
-                mma_k<MNMAJ, KMAJ>(tmem + BM_DS, D, sb + Lo.Ucat, 32, 0, 0, sb + Lo.S[1], D, 0, 0, R2, true);
-                mma_k<KMAJ, MNMAJ>(tmem + BM_WU, 32, sb + Lo.SBq, D, 0, 0, sb + Lo.S[1], D, 0, 0, D, !first_glue);
+            LEADER_BEGIN
+                mma_k<MNMAJ, KMAJ, 32>(tmem + BM_DS, D, sb + Lo.Ucat, 32, 0, 0, sb + Lo.S[1], D, 0, 0, R2, true);
+                mma_k<KMAJ, MNMAJ, D>(tmem + BM_WU, 32, sb + Lo.SBq, D, 0, 0, sb + Lo.S[1], D, 0, 0, D, !first_glue);
                 umma_commit(&mi.bar_mma);
-            }
+            LEADER_END
             WAIT_MMA();
             first_glue = false;
         }
@@ -964,6 +967,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         first = false;
     }
 
+    PROF_FLUSH(g_prof_bwd)
     // ---- per-chain partial weight gradients: [dUb|dUw][dVb][dVw] (dA, dtau come from the epilogue kernel)
     if (half == 0 && srow) {
         float* part = a.part + (size_t)chain * a.part_stride;

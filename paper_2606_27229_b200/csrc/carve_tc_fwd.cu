@@ -242,6 +242,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         else if (c < 32) { if (c - 16 < r && n < DV) v = __ldg(a.Vw + (size_t)(vofs + n) * r + (c - 16)); }
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Vcat + tile_off(DM, n, c)) = __float2bfloat16_rn(v);
     }
+    for (int j = tid; j < 4 * 128; j += NTH) mi.etot[j >> 7][j & 127] = 1.f;
     for (int j = tid; j < DK; j += NTH) {
         mi.eA[j] = a.A ? __expf(__ldg(a.A + h * DK + j)) : 1.f;
         mi.tau[j] = a.tau ? __ldg(a.tau + h * DK + j) : 0.f;
@@ -337,7 +338,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             __syncwarp();
         }
         // meanwhile: raw k, q have landed -> partial sums of squares; beta
+        PROF(g_prof_fwd, 27);
         mbar_wait(&mi.bar_kq, tma_ph);
+        PROF(g_prof_fwd, 28);
         if (live) {
             float ss = 0.f;
 #pragma unroll
@@ -422,7 +425,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         WAIT_MMA();
         PROF(g_prof_fwd, 3);
-        // ---- P3: tt = tanh(Z rnorm_q) -> [0 tt_w; tt_b 0];  block-triangular +-1 matrix
+        // ---- P3: tt = tanh(Z rnorm_q) -> [tt_b pad 16 | tt_w pad 16] (both row halves)
         if (!krole && half == 0 && warp_active) {
             const float rnq = a.l2norm ? rsqrtf(sumsq(row) + a.eps) : 1.f;
             const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
@@ -454,21 +457,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
-        if (half == 1) {
-            const uint32_t one = krole ? 0xBF80u : 0x3F80u;  // bf16 -1 / +1
-#pragma unroll
-            for (int ch = 0; ch < 8; ++ch) {
-                uint32_t w[4];
-#pragma unroll
-                for (int p = 0; p < 4; ++p) {
-                    const int s0 = 8 * ch + 2 * p, s1 = s0 + 1;
-                    const uint32_t lo = (s0 <= t && (s0 >> 4) == (t >> 4)) ? one : 0u;
-                    const uint32_t hi = (s1 <= t && (s1 >> 4) == (t >> 4)) ? one : 0u;
-                    w[p] = lo | (hi << 16);
-                }
-                sts128(sm + Lo.Y2 + tile_chunk_off(128, row, ch), make_uint4(w[0], w[1], w[2], w[3]));
-            }
-        }
         PROF(g_prof_fwd, 4);
         // ---- P4: b_proj = [tt_b;tt_b] Vb^T -> TM_X1, w_proj = [tt_w;tt_w] Vw^T -> TM_X2 (both row halves get both)
         PHASE_SYNC();
@@ -480,113 +468,93 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             }
             __syncwarp();
         }
+        PROF(g_prof_fwd, 29);
         mbar_wait(&mi.bar_fb, tma_ph);
         mbar_wait(&mi.bar_wv, tma_ph);
+        PROF(g_prof_fwd, 30);
         WAIT_MMA();
         PROF(g_prof_fwd, 5);
-        // ---- P5: gates (8 columns per step; cc = 16-byte chunk index inside the row).  Both threads of a token take
-        //      half of the part's columns and do the erase side (log a) and the write side (V' = w v) for them.
+        // ---- P5: gates and the retention prefix.  Both threads of a token (K-side lane t, Q-side lane 64+t) take half of
+        //      the part's columns (two 16-byte chunks cc0, cc0+1) and do, for them: the write side V' = sigmoid(wx + w_proj) v,
+        //      the erase side log a_t = g_t - softplus(bx + b_proj) (Eq. 9 l.151, Eq. 14 l.310), and the block-local
+        //      prefix sums lg_t - lg_a over the 16 tokens of the anchor block -- a segmented warp scan in fp32 registers
+        //      (a warp holds 32 consecutive tokens of one role), so log a never leaves the registers.
+        float lg[16];
+        const int cc0 = half * (HK / 8) + (krole ? 0 : HK / 16);
         if (warp_active) {
-            const int cc0 = half * (HK / 8) + (krole ? 0 : HK / 16);
+            const int blk = t >> 4;
             uint32_t pr16[16], pw16[16];
             tmem_ld16(tmem + TM_X1 + lane_base + 8 * cc0, pr16);
             tmem_ld16(tmem + TM_X2 + lane_base + 8 * cc0, pw16);
             tmem_wait_ld();
 #pragma unroll
-            for (int ci = 0; ci < HK / 16; ++ci) {
+            for (int ci = 0; ci < 2; ++ci) {
                 const int cc = cc0 + ci;
-                const uint32_t* pr = pr16 + 8 * ci;
-                const uint32_t* pw = pw16 + 8 * ci;
+                const uint32_t off = tile_chunk_off(64, t, cc);
                 if (live) {
-                    const uint32_t off = tile_chunk_off(64, t, cc);
-                    {
-                        float fb[8], ff[8], hi[8], lo[8], bg[8];
-                        unpack8(lds128(sm + Lo.BX + off), fb);
-                        unpack8(lds128(sm + Lo.F + off), ff);
+                    float fw[8], fv[8];
+                    unpack8(lds128(sm + Lo.WX + off), fw);
+                    unpack8(lds128(sm + Lo.V + off), fv);
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) {
-                            const int j = 8 * cc + e;
-                            // sigmoid and softplus of the same argument share exp(-|pre|): 3 transcendental ops, not 4
-                            const float pre = fb[e] + __uint_as_float(pr[e]);
-                            const float ex = __expf(-fabsf(pre)), s1p = 1.f + ex;
-                            if (rc) {
-                                const float rs = __fdividef(1.f, s1p);
-                                bg[e] = pre >= 0.f ? rs : ex * rs;
-                            }
-                            const float g = -mi.eA[j] * softplus_fast(ff[e] + mi.tau[j]);
-                            const float la = g - (fmaxf(pre, 0.f) + __logf(s1p));
-                            const float h16 = __bfloat162float(__float2bfloat16_rn(la));
-                            hi[e] = h16;
-                            lo[e] = la - h16;
-                        }
-                        sts128(sm + Lo.Y0 + off, pack8(hi));
-                        sts128(sm + Lo.Y1 + off, pack8(lo));
-                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.Bg + rp_off(t, cc)) = pack8(bg);
+                    for (int e = 0; e < 8; ++e) {
+                        fw[e] = sigmoid_tanh(fw[e] + __uint_as_float(pw16[8 * ci + e]));
+                        fv[e] *= fw[e];
                     }
-                    {
-                        float fw[8], fv[8];
-                        unpack8(lds128(sm + Lo.WX + off), fw);
-                        unpack8(lds128(sm + Lo.V + off), fv);
+                    sts128(sm + Lo.V + off, pack8(fv));
+                    if (rc) {
+                        *reinterpret_cast<uint4*>(rc + Rc.W + rp_off(t, cc)) = pack8(fw);
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) {
-                            fw[e] = sigmoid_tanh(fw[e] + __uint_as_float(pw[e]));
-                            fv[e] *= fw[e];
-                        }
-                        sts128(sm + Lo.V + off, pack8(fv));
-                        if (rc) {
-                            *reinterpret_cast<uint4*>(rc + Rc.W + rp_off(t, cc)) = pack8(fw);
+                        for (int e = 0; e < 8; ++e) fv[e] *= 1.f - fw[e];
+                        *reinterpret_cast<uint4*>(rc + Rc.VWX + rp_off(t, cc)) = pack8(fv);
+                    }
+                }
+                float fb[8], ff[8], bg[8], ea[8], ta[8];
+                unpack8(lds128(sm + Lo.BX + off), fb);
+                unpack8(lds128(sm + Lo.F + off), ff);
+                *reinterpret_cast<float4*>(ea) = *reinterpret_cast<const float4*>(&mi.eA[8 * cc]);
+                *reinterpret_cast<float4*>(ea + 4) = *reinterpret_cast<const float4*>(&mi.eA[8 * cc + 4]);
+                *reinterpret_cast<float4*>(ta) = *reinterpret_cast<const float4*>(&mi.tau[8 * cc]);
+                *reinterpret_cast<float4*>(ta + 4) = *reinterpret_cast<const float4*>(&mi.tau[8 * cc + 4]);
 #pragma unroll
-                            for (int e = 0; e < 8; ++e) fv[e] *= 1.f - fw[e];
-                            *reinterpret_cast<uint4*>(rc + Rc.VWX + rp_off(t, cc)) = pack8(fv);
-                        }
+                for (int e = 0; e < 8; ++e) {
+                    // sigmoid and softplus of the same argument share exp(-|pre|): 3 transcendental ops, not 4
+                    const float pre = fb[e] + __uint_as_float(pr16[8 * ci + e]);
+                    const float ex = ex2_ftz(-fabsf(pre) * kLog2e), s1p = 1.f + ex;
+                    if (rc) {
+                        const float rs = rcp_ftz(s1p);
+                        bg[e] = pre >= 0.f ? rs : ex * rs;
+                    }
+                    const float g = -ea[e] * softplus_fast(ff[e] + ta[e]);
+                    const float la = g - fmaf(kLn2, lg2_ftz(s1p), fmaxf(pre, 0.f));
+                    lg[8 * ci + e] = live ? la : 0.f;
+                }
+                if (rc && live) *reinterpret_cast<uint4*>(rc + Rc.Bg + rp_off(t, cc)) = pack8(bg);
+            }
+#pragma unroll
+            for (int d = 1; d < 16; d <<= 1) {
+                const bool take = (lane & 15) >= d;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    const float o = __shfl_up_sync(0xFFFFFFFFu, lg[i], d, 16);
+                    if (take) lg[i] += o;
+                }
+            }
+            if (live && (lane & 15) == 15) {   // last token of its anchor block: exp of the block totals
+                float* re = rc ? reinterpret_cast<float*>(rc + Rc.etot) : nullptr;
+#pragma unroll
+                for (int e4 = 0; e4 < 4; ++e4) {
+                    const float4 ev = make_float4(exp_fast(lg[4 * e4]), exp_fast(lg[4 * e4 + 1]), exp_fast(lg[4 * e4 + 2]), exp_fast(lg[4 * e4 + 3]));
+                    *reinterpret_cast<float4*>(&mi.etot[blk][8 * cc0 + 4 * e4]) = ev;
+                    if (re) {
+                        *reinterpret_cast<float4*>(re + blk * DK + 8 * cc0 + 4 * e4) = ev;
+                        if (t == LCc - 1)   // blocks that do not exist at L < 64 count as no decay
+                            for (int b2 = blk + 1; b2 < 4; ++b2)
+                                *reinterpret_cast<float4*>(re + b2 * DK + 8 * cc0 + 4 * e4) = make_float4(1.f, 1.f, 1.f, 1.f);
                     }
                 }
             }
         }
         PROF(g_prof_fwd, 6);
-        // ---- P6: block-local prefix sums -> TM_X2[0, DK): rows 0..63 a_b - lg_t, rows 64..127 lg_t - a_b
-        PHASE_SYNC();
-        PROF(g_prof_fwd, 25);
-        if (warp == 0) {
-            if (elect_one()) {
-                mma_rt<128, KMAJ, MNMAJ, LC>(tmem + TM_X2, DK, sb + Lo.Y2, 128, 0, sb + Lo.Y0, 64, 0, LCc, false);
-                mma_rt<128, KMAJ, MNMAJ, LC>(tmem + TM_X2, DK, sb + Lo.Y2, 128, 0, sb + Lo.Y1, 64, 0, LCc, true);
-                umma_commit(&mi.bar_mma);
-            }
-            __syncwarp();
-        }
-        WAIT_MMA();
-        PROF(g_prof_fwd, 7);
-        // ---- P7a: exp of the block totals (last token of each 16-token anchor block), then their suffix products
-        if (!krole && warp_active) {
-            const int blk = t >> 4;
-            const bool last = live && (t & 15) == 15;
-            uint32_t v[32];
-            tmem_ld32(tmem + TM_X2 + lane_base + half * HK, v);
-            tmem_wait_ld();
-            if (last) {
-#pragma unroll
-                for (int e4 = 0; e4 < 8; ++e4)
-                    *reinterpret_cast<float4*>(&mi.etot[blk][half * HK + 4 * e4]) =
-                        make_float4(__expf(__uint_as_float(v[4 * e4])), __expf(__uint_as_float(v[4 * e4 + 1])),
-                                    __expf(__uint_as_float(v[4 * e4 + 2])), __expf(__uint_as_float(v[4 * e4 + 3])));
-            }
-        }
-        __syncthreads();
-        if (tid < DK) {
-            const int nb = LCc >> 4;
-            float p = 1.f;  // suf[b] = prod of etot[b'] over b' > b
-#pragma unroll
-            for (int b2 = 3; b2 >= 0; --b2) {
-                mi.suf[b2][tid] = p;
-                if (b2 < nb) p *= mi.etot[b2][tid];
-            }
-            mi.gamL[tid] = p;
-            if (rc) {
-#pragma unroll
-                for (int b2 = 0; b2 < 4; ++b2) reinterpret_cast<float*>(rc + Rc.etot)[b2 * DK + tid] = b2 < nb ? mi.etot[b2][tid] : 1.f;
-            }
-        }
         __syncthreads();
         PROF(g_prof_fwd, 8);
         // ---- P7b: decayed operands.  Row operands exist in up to four anchorings: version 0 relative to the chunk
@@ -613,12 +581,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 const int bn = tn >> 4, krow = has_next ? tn : 0;
                 const float rnkn = a.l2norm ? rsqrtf(sumsq(krow) + a.eps) : 1.f;
                 if (rc && live && half == 0) reinterpret_cast<float*>(rc + Rc.rn)[row] = krole ? rnk : rnq;
-                const int cc0 = half * (HK / 8) + (krole ? 0 : HK / 16);
-#pragma unroll 1
-                for (int cc = cc0; cc < cc0 + HK / 16; ++cc) {
-                    uint32_t v[8];
-                    tmem_ld8(tmem + TM_X2 + lane_base + 8 * cc, v);
-                    tmem_wait_ld();
+#pragma unroll
+                for (int ci = 0; ci < 2; ++ci) {
+                    const int cc = cc0 + ci;
                     if (live) {
                         float Fp[8], qv[8], kv[8], o[8];
                         {   // column operand C_t, Ktil_t (own anchor), gamma_a/gamma_t >= 1
@@ -626,13 +591,26 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                             unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, t, cc)), kt);
                             *reinterpret_cast<float4*>(et) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc]);
                             *reinterpret_cast<float4*>(et + 4) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc + 4]);
-                            *reinterpret_cast<float4*>(sf) = *reinterpret_cast<const float4*>(&mi.suf[blk][8 * cc]);
-                            *reinterpret_cast<float4*>(sf + 4) = *reinterpret_cast<const float4*>(&mi.suf[blk][8 * cc + 4]);
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) sf[e] = 1.f;   // gamma_L / gamma_e(blk): product of etot[b'] over b' > blk
+#pragma unroll
+                            for (int b2 = 3; b2 >= 1; --b2) {
+                                if (b2 > blk) {
+                                    const float4 e0 = *reinterpret_cast<const float4*>(&mi.etot[b2][8 * cc]);
+                                    const float4 e1 = *reinterpret_cast<const float4*>(&mi.etot[b2][8 * cc + 4]);
+                                    sf[0] *= e0.x; sf[1] *= e0.y; sf[2] *= e0.z; sf[3] *= e0.w;
+                                    sf[4] *= e1.x; sf[5] *= e1.y; sf[6] *= e1.z; sf[7] *= e1.w;
+                                }
+                            }
+                            if (t == 0) {   // gamma_L of the chunk for these columns (state carry, P13)
+                                *reinterpret_cast<float4*>(&mi.gamL[8 * cc]) = make_float4(sf[0] * et[0], sf[1] * et[1], sf[2] * et[2], sf[3] * et[3]);
+                                *reinterpret_cast<float4*>(&mi.gamL[8 * cc + 4]) = make_float4(sf[4] * et[4], sf[5] * et[5], sf[6] * et[6], sf[7] * et[7]);
+                            }
 #pragma unroll
                             for (int e = 0; e < 8; ++e) {
-                                const float lgl = krole ? -__uint_as_float(v[e]) : __uint_as_float(v[e]);  // lg_t - lg_a <= 0
-                                Fp[e] = __expf(lgl);                              // gamma_t / gamma_{a_blk}
-                                const float cx = __expf(-lgl);                    // gamma_{a_blk} / gamma_t >= 1
+                                const float l2 = lg[8 * ci + e] * kLog2e;         // lg_t - lg_a <= 0
+                                Fp[e] = ex2_ftz(l2);                              // gamma_t / gamma_{a_blk}
+                                const float cx = ex2_ftz(-l2);                    // gamma_{a_blk} / gamma_t >= 1
                                 const float kh = kt[e] * rnk;
                                 ic[e] = cx;
                                 o1[e] = kh * cx;
@@ -703,6 +681,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 umma_commit(&mi.bar_mma);   // the A|P blocks: P9a starts on them while the state products still run
                 mma_rt<128, KMAJ, KMAJ, DK>(tmem + TM_ACC, DV, sb + Lo.KQbar, 128, 0, sb + Lo.Sb, DV, 0, DK, false);
                 umma_commit(&mi.bar_acc);
+                if (c + 1 < nchunks) {   // the next chunk's raw k, q -> L2 (their shared-memory tile is still the solve's scratch)
+                    const int tr = b * a.T + (c + 1) * LCc;
+                    for (int cb = 0; cb < DK / 64; ++cb) { tma_prefetch_3d(&mk, cb * 64, h, tr); tma_prefetch_3d(&mq, cb * 64, h, tr); }
+                }
             }
             __syncwarp();
         }
@@ -836,6 +818,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         // ---- P9c: WY solve U = (I + beta A)^-1 (beta R) in registers (tf32 mma.sync) -> bf16 rows over V'; T -> TP rows 0..63
         diag8_inverse(Mm, Tm, LCc, tid);
         __syncthreads();
+        PROF(g_prof_fwd, 26);
         wy_solve<DV>(Mm, Tm, LCc, warp, lane, sb + Lo.Y2, sb + Lo.Us, sb + Lo.TP);
         // the record copies issued so far have left their buffers: the next chunk's loads (P13) may overwrite them
         if (rc && tid == REC_TID) bulk_wait_read();
@@ -917,6 +900,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         tma_ph ^= 1u;
         PROF(g_prof_fwd, 17);
     }
+    PROF_FLUSH(g_prof_fwd)
     if (VS > 1) cluster_wait();   // pairs with the last arrive; also keeps this CTA's shared memory alive for the peer
     PHASE_SYNC();
     if (rec_chain && (tid == 0 || tid == REC_TID)) bulk_wait_all();   // drain the record's bulk stores

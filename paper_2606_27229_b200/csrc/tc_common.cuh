@@ -19,17 +19,27 @@
 // thread in slots 0.., thread 64 = a Q-side thread in slots 40..).
 #ifdef CARVE_PROFILE
 #define PROF_DECL(name) static __device__ unsigned long long name[80];
-#define PROF_INIT() long long prof_t_ = clock64();
+// counters accumulate in shared memory (a global read-modify-write would stall the profiled thread for an L2 round
+// trip at every point) and are added to the global array once, by PROF_FLUSH at the kernel's end
+#define PROF_INIT()                                            \
+    __shared__ unsigned long long prof_s_[80];                 \
+    if (threadIdx.x < 80) prof_s_[threadIdx.x] = 0;            \
+    __syncthreads();                                           \
+    long long prof_t_ = clock64();
 #define PROF(name, i)                                                              \
     if (blockIdx.x == 0 && (threadIdx.x == 0 || threadIdx.x == 64)) {              \
         const long long prof_n_ = clock64();                                       \
-        name[(threadIdx.x ? 40 : 0) + i] += (unsigned long long)(prof_n_ - prof_t_); \
+        prof_s_[(threadIdx.x ? 40 : 0) + i] += (unsigned long long)(prof_n_ - prof_t_); \
         prof_t_ = prof_n_;                                                         \
     }
+#define PROF_FLUSH(name)                                                           \
+    __syncthreads();                                                               \
+    if (blockIdx.x == 0 && threadIdx.x < 80) name[threadIdx.x] += prof_s_[threadIdx.x];
 #else
 #define PROF_DECL(name)
 #define PROF_INIT()
 #define PROF(name, i)
+#define PROF_FLUSH(name)
 #endif
 
 namespace carve {
@@ -96,6 +106,12 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
         ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
         : "memory");
+}
+// The same box, fetched into L2 only (no shared-memory destination, no completion signal).
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap* map, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map)
 {
