@@ -70,43 +70,50 @@ def load_peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks/throttle reasons while the timed region runs."""
-    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """Samples SM clocks and throttle reasons every ~2 ms (NVML) from before the warm-up until after the timed loop;
+    `mark()` brackets the timed region so that the summary is taken from the samples that fall inside it."""
+    NAMES = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
 
     def __init__(self, index: int):
-        self.index, self.rows, self.proc, self.thr = index, [], None, None
+        self.index, self.rows, self.stop_flag, self.thr, self.marks, self.err = index, [], False, None, [], None
+        self.max_sm = None
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-        except OSError:
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_sm = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # noqa: BLE001
+            self.err = f"nvml unavailable: {e}"
             return
-        self.thr = threading.Thread(target=lambda: self.rows.extend(self.proc.stdout), daemon=True)
+
+        def loop():
+            while not self.stop_flag:
+                try:
+                    sm = float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                    rs = int(pynvml.nvmlDeviceGetCurrentClocksEventReasons(h))
+                    self.rows.append((time.perf_counter(), sm, rs))
+                except Exception:  # noqa: BLE001
+                    pass
+                time.sleep(0.002)
+        self.thr = threading.Thread(target=loop, daemon=True)
         self.thr.start()
 
+    def mark(self):
+        self.marks.append(time.perf_counter())
+
     def stop(self) -> dict:
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
+        if self.thr is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "samples": 0, "reasons": [self.err or "sampler not started"]}
+        self.stop_flag = True
         self.thr.join(timeout=2)
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.rows:
-            parts = [p.strip() for p in ln.split(",")]
-            if len(parts) < 6:
-                continue
-            try:
-                sm.append(float(parts[0])); mx.append(float(parts[1]))
-            except ValueError:
-                continue
-            for n, v in zip(names, parts[2:6]):
-                if v.lower().startswith("active"):
-                    reasons.add(n)
-        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+        lo, hi = (self.marks[0], self.marks[1]) if len(self.marks) >= 2 else (0.0, float("inf"))
+        inside = [r for r in self.rows if lo <= r[0] <= hi] or self.rows
+        sm = [r[1] for r in inside]
+        reasons = sorted(n for n, bit in self.NAMES.items() if any(r[2] & bit for r in inside))
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": self.max_sm, "samples": len(sm),
+                "samples_total": len(self.rows), "reasons": reasons}
 
 
 # ---- CPU oracle leg ------------------------------------------------------------------------------
@@ -255,20 +262,22 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
     kev = [[ev(), ev(), ev()] for _ in range(args.steps)]
     t_begin, t_end = ev(), ev()
     barrier()
+    sampler.mark()
     t_begin.record(stream)
     for i in range(args.steps):
         step(kev[i])
     t_end.record(stream)
     barrier()
+    sampler.mark()
     ms_total = t_begin.elapsed_time(t_end)
     clocks = sampler.stop() if rank == 0 else None
     fwd_ms = statistics.mean(k[0].elapsed_time(k[1]) for k in kev)
@@ -317,8 +326,10 @@ def run_ours(args):
         dom_ms = bwd_ms if dom == "bwd" else fwd_ms
         dom_bytes = alg[f"{dom}_bytes"]
         achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
-        traffic = None      # DRAM bytes of that call from the committed ncu capture (config 1, tensor path only)
-        tpath = os.path.join(ROOT, "profiles", "r1_tc_traffic.csv")
+        traffic = None      # DRAM bytes of that call from the newest committed ncu capture (config 1, tensor path only)
+        tpath = os.path.join(ROOT, "profiles", "r2_tc_traffic.csv")
+        if not os.path.exists(tpath):
+            tpath = os.path.join(ROOT, "profiles", "r1_tc_traffic.csv")
         if cfg.name == synth.CFG1.name and not args.fwd_only and os.path.exists(tpath):
             for ln in open(tpath).read().splitlines()[1:]:
                 f = ln.split(",")
@@ -341,6 +352,8 @@ def run_ours(args):
                                                            if dom == "bwd" and path == 2 else "")),
                          "achieved": achieved, "peak": peaks["hbm_gbs"],
                          "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"], "traffic": traffic,
+                         "traffic_source": (f"profiles/{os.path.basename(tpath)} (ncu --set full capture of this command; "
+                                            "dram__bytes_read.sum + dram__bytes_write.sum per launch)") if traffic else None,
                          "peak_source": f"{peaks['source']} (MEASURED_PEAKS.json hbm_gbs)" if peaks["source"] == "measured"
                          else "fallback 6650 GB/s",
                          "algorithmic_bytes_per_launch": dom_bytes},
@@ -351,7 +364,7 @@ def run_ours(args):
                                "algorithmic_flops": alg["fwd_flops"] + alg["bwd_flops"]},
         })
         if world == 1 and not args.no_cpu_baseline:
-            cb, _ = time_oracle(cfg, x, ct, 1, 0)
+            cb, _ = time_oracle(cfg, x, ct, 1, 1)     # one warm-up pass (page faults, thread pool), one timed
             line["cpu_baseline"] = cb
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -368,6 +381,21 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fwd-only", action="store_true", help="time carve_fwd alone (inference call, nothing saved)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        # plain `python bench.py --gpus N`: start the N ranks ourselves (one process per GPU, NCCL), the same way the
+        # driver does with torchrun
+        import socket
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            raise SystemExit(f"bench.py --gpus {args.gpus}: only {have} CUDA device(s) visible")
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        env = dict(os.environ, NCCL_DEBUG=os.environ.get("NCCL_DEBUG", "WARN"))
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd, env=env))
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -22,11 +22,12 @@ _SO = os.path.join(_HERE, "libcarve_oracle.so")
 
 
 def build(force: bool = False) -> str:
-    """Compile carve_oracle.c -> libcarve_oracle.so (gcc -O2 -fopenmp)."""
+    """Compile carve_oracle.c -> libcarve_oracle.so: gcc -O3 -fopenmp.  No -march=native (the object built on the CPU box
+    also has to run on the host cores of the GPU box) and no fast-math (the fp64 arithmetic is that of the source)."""
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
         tmp = _SO + f".tmp{os.getpid()}"
         subprocess.check_call(
-            ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall", "-o", tmp, _SRC, "-lm"]
+            ["gcc", "-O3", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall", "-o", tmp, _SRC, "-lm"]
         )
         os.replace(tmp, _SO)
     return _SO

@@ -959,8 +959,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         // ---- L10: the adjoint of the state entering the chunk
         PROF(g_prof_bwd, 11);
         finalize(true, c == 0);
-        if (tid == 0) {   // every output row of this chunk was stored before the barrier inside finalize: publish it
-            __threadfence();
+        if (tid == 0 && c > 0) {   // every output row of this chunk was stored before the barrier inside finalize: publish it
+            __threadfence();        // (chunk 0 is published below, after the per-chain weight-gradient partials)
             asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.flags + chain), "r"(nchunks - c) : "memory");
         }
         PROF(g_prof_bwd, 12);
@@ -985,6 +985,10 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         }
     }
     PHASE_SYNC();
+    if (tid == 0) {   // last publish: chunk 0 AND the partials above are in memory (the reductions run behind the epilogue grid)
+        __threadfence();
+        asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.flags + chain), "r"(nchunks) : "memory");
+    }
     if (warp == 0) tmem_dealloc(tmem, TM_COLS);
 }
 
@@ -1088,6 +1092,10 @@ carve_bwd_tc_epilogue_kernel(const __nv_bfloat16* __restrict__ gq, const __nv_bf
         for (int w = 0; w < 8; ++w) s += red[w][i / D][i % D];
         partAT[((size_t)chain * nchunks + c) * 2 * D + i] = s;
     }
+    // Launched with programmatic stream serialization: the grid must not complete before the reverse kernel has (the
+    // reductions that follow in the stream read its per-chain partials).  The chunk-0 blocks -- last in block order, so
+    // they hold no SM while earlier chunks still have work -- wait for the primary grid here; a no-op for a plain launch.
+    if (c == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 // part[chain][nW + which*dk + j] = sum over the chain's chunks of partAT (fixed order: deterministic).

@@ -311,6 +311,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             tma_load_3d(sm + Lo.V + cb * 64 * 128, &mv, &mi.bar_wv, vofs + cb * 64, h, tr);
         }
     };
+    if (VS > 1) { cluster_arrive(); cluster_wait(); }   // every CTA of the cluster runs before any distributed-shared-memory access
     if (tid == 0) { fence_async_smem(); issue_kq(0); issue_fb(0); issue_wv(0); }
 
     uint32_t mma_ph = 0, tma_ph = 0, acc_ph = 0;
