@@ -119,6 +119,23 @@ carve_status_t carve_bwd(const carve_params_t *p, const void *q, const void *k, 
                          float *dVb, float *dVw, float *dS0, void *workspace, size_t workspace_bytes,
                          void *cuda_stream);
 
+/*
+ * Recurrent (decode) step: a few new tokens per sequence, state in and out (P Table 1 l.432 "Infer/tok O(d_v d_k)",
+ * l.27; chunk mode == sequential at chunk size 1, Table 2 l.450).
+ *   p->T = n new tokens per sequence, 1 <= n <= 16; they form ONE gate chunk (p->L is ignored): the content gates
+ *   of all n tokens read the incoming state, G = [Ub;Uw] S (Eq. 7 l.134), and each token applies Eq. 5 (l.108).
+ *   n = 1 is exact per-token content gating.  The result equals carve_fwd with T = L = n and S0 = S.
+ *   q,k,f,bx [B,n,H,dk]; v,wx [B,n,H,dv]; beta [B,n,H] (dtype); weights as carve_fwd (A, tau may be NULL).
+ *   S [B,H,dv,dk] float, IN/OUT: the state before the step, overwritten by the state after it (never NULL).
+ *   O [B,n,H,dv] dtype, out.
+ * Shapes: dk in {64,128}, dv in {64,128} (or dv = 256 with dk = 128), r in {8,16,32}; fp32 arithmetic for both
+ * dtypes; one kernel launch; no workspace.  Errors as carve_fwd (CARVE_ERR_SHAPE for n > 16 or n < 1).
+ */
+carve_status_t carve_step(const carve_params_t *p, const void *q, const void *k, const void *v, const void *f,
+                          const void *bx, const void *wx, const void *beta, const float *A, const float *tau,
+                          const float *Ub, const float *Uw, const float *Vb, const float *Vw, float *S, void *O,
+                          void *cuda_stream);
+
 /* Bytes of device arena carve_fwd_bwd_host needs (device copies of every tensor + workspace). */
 size_t carve_host_arena_bytes(const carve_params_t *p, int with_bwd);
 

@@ -19,7 +19,7 @@ CARVE_F32, CARVE_BF16 = 0, 1
 CARVE_PATH_AUTO, CARVE_PATH_SIMT, CARVE_PATH_TENSOR = 0, 1, 2
 
 # Every symbol include/carve.h declares (tests check the library exports them all).
-SYMBOLS = ("carve_workspace_bytes", "carve_fwd", "carve_bwd", "carve_host_arena_bytes", "carve_fwd_bwd_host",
+SYMBOLS = ("carve_workspace_bytes", "carve_fwd", "carve_bwd", "carve_step", "carve_host_arena_bytes", "carve_fwd_bwd_host",
            "carve_num_launches", "carve_resolved_path", "carve_status_string", "carve_version")
 
 
@@ -83,6 +83,8 @@ def load_library() -> ctypes.CDLL:
         lib.carve_version.restype = ctypes.c_char_p
         lib.carve_fwd.restype = ci
         lib.carve_fwd.argtypes = [pp] + [vp] * 16 + [vp, sz, vp]
+        lib.carve_step.restype = ci
+        lib.carve_step.argtypes = [pp] + [vp] * 15 + [vp]
         lib.carve_bwd.restype = ci
         lib.carve_bwd.argtypes = [pp] + [vp] * 30 + [vp, sz, vp]
         lib.carve_fwd_bwd_host.restype = ci
@@ -143,6 +145,14 @@ def carve_fwd(p: Params, x: dict, O, S_final, workspace=None, stream: int = 0) -
     cp = p.c()
     _check(load_library().carve_fwd(ctypes.byref(cp), *[_ptr(x.get(n)) for n in _FWD_IN], _ptr(O), _ptr(S_final),
                                     _ptr(workspace), _nbytes(workspace), ctypes.c_void_p(stream)))
+
+
+def carve_step(p: Params, x: dict, S, O, stream: int = 0) -> None:
+    """carve_step of carve.h: p.T = n <= 16 new tokens per sequence; `x` as for carve_fwd (S0 is not used);
+    S [B,H,dv,dk] float32 is read and overwritten in place; O [B,n,H,dv] is written."""
+    cp = p.c()
+    _check(load_library().carve_step(ctypes.byref(cp), *[_ptr(x.get(n)) for n in _FWD_IN[:-1]], _ptr(S), _ptr(O),
+                                     ctypes.c_void_p(stream)))
 
 
 def carve_bwd(p: Params, x: dict, dO, dS_final, grads: dict, workspace, stream: int = 0) -> None:

@@ -171,6 +171,27 @@ carve_status_t carve_fwd(const carve_params_t* p, const void* q, const void* k, 
                                                                                               : CARVE_ERR_CUDA;
 }
 
+carve_status_t carve_step(const carve_params_t* p, const void* q, const void* k, const void* v, const void* f,
+                          const void* bx, const void* wx, const void* beta, const float* A, const float* tau,
+                          const float* Ub, const float* Uw, const float* Vb, const float* Vw, float* S, void* O,
+                          void* cuda_stream)
+{
+    if (!p) return CARVE_ERR_NULL;
+    if (p->dtype != CARVE_F32 && p->dtype != CARVE_BF16) return CARVE_ERR_DTYPE;
+    if (p->B <= 0 || p->H <= 0 || p->T < 1 || p->T > 16) return CARVE_ERR_SHAPE;
+    if (!step_supported(p->dk, p->dv) || !one_of(p->r, {8, 16, 32})) return CARVE_ERR_SHAPE;
+    if (!q || !k || !v || !f || !bx || !wx || !beta || !Ub || !Uw || !Vb || !Vw || !S || !O) return CARVE_ERR_NULL;
+    for (const void* ptr : {q, k, v, f, bx, wx, beta, (const void*)A, (const void*)tau, (const void*)Ub, (const void*)Uw,
+                            (const void*)Vb, (const void*)Vw, (const void*)S, (const void*)O})
+        if (!aligned16(ptr)) return CARVE_ERR_ALIGN;
+    const carve_status_t s = check_arch();
+    if (s != CARVE_OK) return s;
+    return step_launch(*p, q, k, v, f, bx, wx, beta, A, tau, Ub, Uw, Vb, Vw, S, O, static_cast<cudaStream_t>(cuda_stream)) ==
+                   cudaSuccess
+               ? CARVE_OK
+               : CARVE_ERR_CUDA;
+}
+
 // carve_bwd; `epilogue_after`: the tensor path launches its chunk-local epilogue as a plain dependent kernel
 // instead of overlapping it with the reverse kernel (see Args::epilogue_after).
 static carve_status_t bwd_impl(const carve_params_t* p, const void* q, const void* k, const void* v, const void* f,

@@ -1,0 +1,194 @@
+// carve_step.cu -- the recurrent (decode) form of the CARVE layer operator: a few new tokens per sequence, state in
+// and out (Table 1 l.432 "Infer/tok O(d_v d_k)", l.27; "chunk mode vs sequential at chunk size 1", l.450).
+//
+// The n <= 16 new tokens of a sequence form ONE gate chunk: the content gates read the incoming state once,
+// G = [Ub;Uw] S (Eq. 7 l.134), and every token then applies Eq. 5 (l.108) in its per-token form with those gates:
+//     a_t = exp(g_t) (1 - b_t),   e_t = w_t . v_t - S_{t-1} k^_t,   u_t = beta_t e_t,
+//     S_t = S_{t-1} diag(a_t) + u_t k^_t^T,   o_t = scale S_t q^_t.
+// With n = 1 this is exact per-token content gating.  It is the same function as carve_fwd with T = L = n (the chunked
+// WY form equals this recurrence), evaluated without the solve because n is small.
+//
+// One CTA per (batch, head) chain; the state makes one round trip HBM -> shared memory -> HBM per call, which is the
+// algorithmic traffic of a decode step (2 x 4 d_v d_k bytes per chain).  fp32 arithmetic throughout, plain FFMA.
+#include "simt_common.cuh"
+
+namespace carve {
+namespace {
+
+struct StepArgs {
+    int B, H, n, r, l2norm;
+    float scale, eps;
+    const void *q, *k, *v, *f, *bx, *wx, *beta;
+    const float *A, *tau, *Ub, *Uw, *Vb, *Vw;
+    float* S;
+    void* O;
+};
+
+template <typename T, int DK, int DV>
+__global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
+{
+    extern __shared__ __align__(16) float smem[];
+    constexpr int SP = DK + 4;
+    const int r = a.r, R2 = 2 * r;
+    float* sS = smem;                  // [DV][SP]
+    float* sG = sS + DV * SP;          // [R2][SP]
+    float* sQ = sG + R2 * SP;          // [DK] q^
+    float* sK = sQ + DK;               // [DK] k^
+    float* sA = sK + DK;               // [DK] a_t
+    float* sU = sA + DK;               // [DV] u_t
+    float* sW = sU + DV;               // [DV] w_t v_t
+    float* sT = sW + DV;               // [R2] tanh bottleneck
+    float* sRed = sT + 64;             // [2] 1/|q|, 1/|k|
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int chain = blockIdx.x, b = chain / a.H, h = chain % a.H;
+    const T* gq = static_cast<const T*>(a.q);
+    const T* gk = static_cast<const T*>(a.k);
+    const T* gv = static_cast<const T*>(a.v);
+    const T* gf = static_cast<const T*>(a.f);
+    const T* gbx = static_cast<const T*>(a.bx);
+    const T* gwx = static_cast<const T*>(a.wx);
+    const T* gbeta = static_cast<const T*>(a.beta);
+    T* gO = static_cast<T*>(a.O);
+    float* gS = a.S + (size_t)chain * DV * DK;
+
+    for (int i = tid; i < DV * DK / 4; i += NT) {
+        const int x = i / (DK / 4), j4 = i % (DK / 4);
+        st4s(sS + x * SP + 4 * j4, ldg4(gS + (size_t)i * 4));
+    }
+    __syncthreads();
+    // fold: G[i][j] = sum_x Ucat[i][x] S[x][j]   (once per call: the gates of all n tokens read the incoming state)
+    for (int o = tid; o < R2 * DK; o += NT) {
+        const int i = o / DK, j = o % DK;
+        const float* urow = i < r ? a.Ub + (size_t)i * DV : a.Uw + (size_t)(i - r) * DV;
+        float acc = 0.f;
+#pragma unroll 4
+        for (int x = 0; x < DV; ++x) acc = fmaf(__ldg(urow + x), sS[x * SP + j], acc);
+        sG[i * SP + j] = acc;
+    }
+    __syncthreads();
+
+    for (int t = 0; t < a.n; ++t) {
+        const size_t tok = ((size_t)b * a.n + t) * a.H + h;
+        // q^, k^ (D1)
+        if (warp < 2) {
+            const T* src = warp == 0 ? gq : gk;
+            float ss = 0.f;
+            for (int j = lane; j < DK; j += 32) { const float x = ldf<T>(src, tok * DK + j); ss = fmaf(x, x, ss); }
+            ss = warp_sum(ss);
+            if (lane == 0) sRed[warp] = a.l2norm ? rsqrtf(ss + a.eps) : 1.f;
+        }
+        __syncthreads();
+        for (int j = tid; j < 2 * DK; j += NT) {
+            if (j < DK) sQ[j] = ldf<T>(gq, tok * DK + j) * sRed[0];
+            else sK[j - DK] = ldf<T>(gk, tok * DK + (j - DK)) * sRed[1];
+        }
+        __syncthreads();
+        // tt = tanh(G q^) (Eq. 7)
+        for (int i = warp; i < R2; i += NT / 32) {
+            float acc = 0.f;
+            for (int j = lane; j < DK; j += 32) acc = fmaf(sG[i * SP + j], sQ[j], acc);
+            acc = warp_sum(acc);
+            if (lane == 0) sT[i] = tanhf(acc);
+        }
+        __syncthreads();
+        // gates (Eq. 8-9): a_t = exp(g)(1 - b), w_t v_t
+        for (int j = tid; j < DK + DV; j += NT) {
+            if (j < DK) {
+                float pre = ldf<T>(gbx, tok * DK + j);
+                for (int i = 0; i < r; ++i) pre = fmaf(__ldg(a.Vb + (size_t)j * r + i), sT[i], pre);
+                const float eA = a.A ? expf(__ldg(a.A + h * DK + j)) : 1.f;
+                const float ta = a.tau ? __ldg(a.tau + h * DK + j) : 0.f;
+                const float g = -eA * softplusf(ldf<T>(gf, tok * DK + j) + ta);
+                sA[j] = expf(g - softplusf(pre));          // exp(g) (1 - sigmoid(pre)),  log(1 - sigmoid(x)) = -softplus(x)
+            } else {
+                const int x = j - DK;
+                float pre = ldf<T>(gwx, tok * DV + x);
+                for (int i = 0; i < r; ++i) pre = fmaf(__ldg(a.Vw + (size_t)x * r + i), sT[r + i], pre);
+                sW[x] = sigmoidf_(pre) * ldf<T>(gv, tok * DV + x);
+            }
+        }
+        __syncthreads();
+        // u_t = beta (w v - S k^): two threads per state row, half of the key channels each
+        const float beta = ldf<T>(gbeta, tok);
+        for (int p = tid; p < 2 * DV; p += NT) {
+            const int x = p >> 1, hf = p & 1;
+            const float* srow = sS + x * SP + hf * (DK / 2);
+            const float* kk = sK + hf * (DK / 2);
+            float acc = 0.f;
+#pragma unroll 4
+            for (int j = 0; j < DK / 2; j += 4) acc += dot4(ld4s(srow + j), ld4s(kk + j));
+            acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+            if (hf == 0) sU[x] = beta * (sW[x] - acc);
+        }
+        __syncthreads();
+        // S_t = S diag(a) + u k^^T;  o_t = scale S_t q^
+        for (int p = tid; p < 2 * DV; p += NT) {
+            const int x = p >> 1, hf = p & 1;
+            float* srow = sS + x * SP + hf * (DK / 2);
+            const float* kk = sK + hf * (DK / 2);
+            const float* qq = sQ + hf * (DK / 2);
+            const float* aa = sA + hf * (DK / 2);
+            const float u = sU[x];
+            float acc = 0.f;
+#pragma unroll 4
+            for (int j = 0; j < DK / 2; j += 4) {
+                float4 s4 = ld4s(srow + j);
+                const float4 a4 = ld4s(aa + j), k4 = ld4s(kk + j);
+                s4.x = fmaf(s4.x, a4.x, u * k4.x); s4.y = fmaf(s4.y, a4.y, u * k4.y);
+                s4.z = fmaf(s4.z, a4.z, u * k4.z); s4.w = fmaf(s4.w, a4.w, u * k4.w);
+                st4s(srow + j, s4);
+                acc += dot4(s4, ld4s(qq + j));
+            }
+            acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+            if (hf == 0) stf<T>(gO, tok * DV + x, a.scale * acc);
+        }
+        __syncthreads();
+    }
+    for (int i = tid; i < DV * DK / 4; i += NT) {
+        const int x = i / (DK / 4), j4 = i % (DK / 4);
+        *reinterpret_cast<float4*>(gS + (size_t)i * 4) = ld4s(sS + x * SP + 4 * j4);
+    }
+}
+
+template <typename T, int DK, int DV>
+cudaError_t launch_step(const StepArgs& a, cudaStream_t st)
+{
+    const size_t smem = ((size_t)(DV + 2 * a.r) * (DK + 4) + 3 * DK + 2 * DV + 64 + 8) * sizeof(float);
+    auto kern = carve_step_kernel<T, DK, DV>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<a.B * a.H, NT, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t dispatch_step(const StepArgs& a, int dk, int dv, cudaStream_t st)
+{
+    if (dk == 64 && dv == 64) return launch_step<T, 64, 64>(a, st);
+    if (dk == 128 && dv == 128) return launch_step<T, 128, 128>(a, st);
+    if (dk == 64 && dv == 128) return launch_step<T, 64, 128>(a, st);
+    if (dk == 128 && dv == 64) return launch_step<T, 128, 64>(a, st);
+    if (dk == 128 && dv == 256) return launch_step<T, 128, 256>(a, st);
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+bool step_supported(int dk, int dv)
+{
+    return (dk == 64 || dk == 128) && (dv == 64 || dv == 128 || (dk == 128 && dv == 256));
+}
+
+cudaError_t step_launch(const carve_params_t& p, const void* q, const void* k, const void* v, const void* f, const void* bx,
+                        const void* wx, const void* beta, const float* A, const float* tau, const float* Ub, const float* Uw,
+                        const float* Vb, const float* Vw, float* S, void* O, cudaStream_t st)
+{
+    StepArgs a{};
+    a.B = p.B; a.H = p.H; a.n = p.T; a.r = p.r; a.l2norm = p.qk_l2norm; a.scale = p.scale; a.eps = p.eps;
+    a.q = q; a.k = k; a.v = v; a.f = f; a.bx = bx; a.wx = wx; a.beta = beta;
+    a.A = A; a.tau = tau; a.Ub = Ub; a.Uw = Uw; a.Vb = Vb; a.Vw = Vw; a.S = S; a.O = O;
+    return p.dtype == CARVE_BF16 ? dispatch_step<__nv_bfloat16>(a, p.dk, p.dv, st) : dispatch_step<float>(a, p.dk, p.dv, st);
+}
+
+}  // namespace carve
