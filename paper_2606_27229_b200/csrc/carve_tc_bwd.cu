@@ -360,6 +360,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         LEADER_END
         if (krole) {
             WAIT_MMA();
+            PROF(g_prof_bwd, 13);
             if (warp_active) {
 #pragma unroll
                 for (int s = 0; s < HK; s += 32) {
@@ -383,12 +384,14 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROF(g_prof_bwd, 1);
         // ---- L2: dX = T^T dU: columns x < D/2 -> BM_A rows 0..63 (K-side lanes), x >= D/2 -> rows 64..127 (Q-side lanes)
         PHASE_SYNC();
+        PROF(g_prof_bwd, 14);
         LEADER_BEGIN
             mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_A + D / 2, D / 2, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[0], 64, D / 2, 0, LCc, false);
             mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_A, D / 2, sb + Lo.S[1], 64, 64, 0, sb + Lo.S[0], 64, 0, 0, LCc, false);
             umma_commit(&mi.bar_mma);
         LEADER_END
         WAIT_MMA();
+        PROF(g_prof_bwd, 15);
         if (tid == 0) {  // PT is dead: fetch the block-anchored column operand of L4
             mbar_expect_tx(&mi.bar_g4a, TB);
             bulk_g2s(sm + Lo.S[1], rc + Rc.CC, TB, &mi.bar_g4a);
@@ -429,6 +432,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROF(g_prof_bwd, 2);
         // ---- L3: [dA;dP] raw, SP = [-dR;dO] S, dS += [-dR;dO]^T [Kbar; scale Qbar]
         PHASE_SYNC();
+        PROF(g_prof_bwd, 16);
         LEADER_BEGIN
             mbar_wait(&mi.bar_sb, ph);
             mbar_wait(&mi.bar_g3, ph);
@@ -447,6 +451,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             a.dbeta[(tok0 + t) * a.H + h] = __float2bfloat16_rn(sdb);
         }
         WAIT_MMA();
+        PROF(g_prof_bwd, 17);
         if (tid == 0) {  // DRO and U are dead
             mbar_expect_tx(&mi.bar_g4b, 2 * TB);
             bulk_g2s(sm + Lo.S[2], rc + Rc.KQo, 2 * TB, &mi.bar_g4b);
@@ -496,6 +501,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         //      (t,s) enters +Kbar_own_t C_s dA_ts G in row t and -C_s Kbar_own_t dA_ts G in row s with bit-identical
         //      operands, so the pairs that do not straddle a token cancel to fp32 rounding in the reverse cumulative sum.
         __syncthreads();
+        PROF(g_prof_bwd, 18);
         if (tid == 0) {   // dS' (DSB) is consumed: stage gamma_t/gamma_a and its inverse there for L5
             mbar_expect_tx(&mi.bar_fi, 2 * TB);
             bulk_g2s(sm + Lo.FI, rc + Rc.FQ, TB, &mi.bar_fi);
@@ -526,6 +532,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                     et[b2][nt][0] = e2.x; et[b2][nt][1] = e2.y;
                 }
             mbar_wait(&mi.bar_g4a, ph);
+            PROF(g_prof_bwd, 19);
             uint32_t bC[4][NTW][2];
 #pragma unroll
             for (int jb = 0; jb < 4; ++jb) {
@@ -567,6 +574,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                     }
                 }
             mbar_wait(&mi.bar_g4b, ph);
+            PROF(g_prof_bwd, 20);
             float accII[4][NTW][4];
 #pragma unroll
             for (int jb = 0; jb < 4; ++jb)
@@ -651,6 +659,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                     }
                 }
             __syncthreads();  // every warp is done reading DAP / C / KQo
+            PROF(g_prof_bwd, 21);
 #pragma unroll
             for (int side = 0; side < 2; ++side)       // H raw -> S[2..3] ([128][D] tile, over KQo): for dk^, dq^
 #pragma unroll
@@ -683,6 +692,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         // ---- L5: assemble dk^, dq^ (state part) and the state-read / state-write contributions to d log gamma
         __syncthreads();
         mbar_wait(&mi.bar_fi, ph);
+        PROF(g_prof_bwd, 22);
         if (warp_active) {
             if (krole) {
                 const bool bstart = (t & 15) == 0;
@@ -761,6 +771,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         //      key channels j < D/2 in rows 0..63 (K-side lanes), j >= D/2 in rows 64..127 (Q-side lanes: the 0/1 tile
         //      used as the upper half of the M = 128 operand), so both threads of a token share the epilogue
         PHASE_SYNC();
+        PROF(g_prof_bwd, 23);
         LEADER_BEGIN
             const uint32_t tri = sb + Lo.TRI, trh = tri - 8192;
             mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT, D / 2, tri, 64, 0, 0, sb + Lo.S[2], 128, 0, 0, LCc, false);
@@ -789,6 +800,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 for (int i = 0; i < 4; ++i) t4[i] = ldg128(rc + Rc.tt + t * 64 + 16 * i);
             }
             WAIT_MMA();
+            PROF(g_prof_bwd, 24);
             if (!krole && live) {
 #pragma unroll
                 for (int i = 0; i < HK / 8; ++i) sts128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, half * (HK / 8) + i), d4[i]);
@@ -803,6 +815,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 }
             }
             mbar_wait(&mi.bar_bg, ph);
+            PROF(g_prof_bwd, 25);
             if (warp_active) {
                 __nv_bfloat16* gdf = a.df + ((tok0 + t) * a.H + h) * D;
                 __nv_bfloat16* gdbx = a.dbx + ((tok0 + t) * a.H + h) * D;
@@ -833,6 +846,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROF(g_prof_bwd, 7);
         // ---- L7: ZZ = [db_pre; dw_pre] [Vb | Vw] -> BM_DAP;  dVb | dVw += [db_pre; dw_pre]^T TT2 -> BM_WG
         PHASE_SYNC();
+        PROF(g_prof_bwd, 26);
         LEADER_BEGIN
             mma_k<KMAJ, KMAJ, D>(tmem + BM_DAP, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.VcT, 32, 0, 0, D, false);
             mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_WG, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[1], 128, 0, 0, LCc, !first);
@@ -849,6 +863,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             if (!krole && half < 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(rn_ + Rc.tt + t * 64));
         }
         WAIT_MMA();
+        PROF(g_prof_bwd, 27);
         if (half == 0 && warp_active) {
             // dz = ZZ (1 - tt^2): K side owns the erase half (cols 0..r), Q side the write half (cols r..2r)
             const int c0 = krole ? 0 : r;
@@ -880,6 +895,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROF(g_prof_bwd, 8);
         // ---- L8: dq^ += dz G -> BM_A rows 64..127;  dG^T = q^T (dz/|q|) -> BM_DAP + 32
         PHASE_SYNC();
+        PROF(g_prof_bwd, 28);
         LEADER_BEGIN
             mbar_wait(&mi.bar_g8, ph);
             mbar_wait(&mi.bar_g5, ph);
@@ -889,6 +905,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             umma_commit(&mi.bar_mma);
         LEADER_END
         WAIT_MMA();
+        PROF(g_prof_bwd, 29);
         if (tid == 0 && c > 0) issue_l1(c - 1);   // DZ, DZQ, GW, G^T, q are dead
         if (!krole && warp_active) {
             __nv_bfloat16* gdq = a.dq + ((tok0 + t) * a.H + h) * D;
@@ -942,12 +959,14 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         // ---- L9: fold glue: dS += [Ub;Uw]^T dG;  d[Ub;Uw]^T += S dG^T -> BM_WU
         if (gate_start) {
             PHASE_SYNC();
+            PROF(g_prof_bwd, 30);
             LEADER_BEGIN
                 mma_k<MNMAJ, KMAJ, 32>(tmem + BM_DS, D, sb + Lo.Ucat, 32, 0, 0, sb + Lo.S[1], D, 0, 0, R2, true);
                 mma_k<KMAJ, MNMAJ, D>(tmem + BM_WU, 32, sb + Lo.SBq, D, 0, 0, sb + Lo.S[1], D, 0, 0, D, !first_glue);
                 umma_commit(&mi.bar_mma);
             LEADER_END
             WAIT_MMA();
+            PROF(g_prof_bwd, 31);
             first_glue = false;
         }
         if (tid == 0 && c > 0) {   // SBq and the dG tile are free: the state entering the next chunk, its [P;T]

@@ -186,7 +186,8 @@ template <int DK, int DV, int NP, int VS>
 __global__ void __launch_bounds__(128 * NP, 1)
 carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, const __grid_constant__ CUtensorMap mk,
                     const __grid_constant__ CUtensorMap mv, const __grid_constant__ CUtensorMap mf,
-                    const __grid_constant__ CUtensorMap mbx, const __grid_constant__ CUtensorMap mwx)
+                    const __grid_constant__ CUtensorMap mbx, const __grid_constant__ CUtensorMap mwx,
+                    const __grid_constant__ CUtensorMap mo)
 {
     static_assert(DK == DV, "the shared-memory map assumes dk == dv");
     constexpr int DM = DK > DV ? DK : DV;
@@ -226,7 +227,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         mbar_init(&mi.bar_mma, 1); mbar_init(&mi.bar_acc, 1); mbar_init(&mi.bar_kq, 1); mbar_init(&mi.bar_fb, 1); mbar_init(&mi.bar_wv, 1);
         mbar_fence_init();
         tma_prefetch_desc(&mq); tma_prefetch_desc(&mk); tma_prefetch_desc(&mv);
-        tma_prefetch_desc(&mf); tma_prefetch_desc(&mbx); tma_prefetch_desc(&mwx);
+        tma_prefetch_desc(&mf); tma_prefetch_desc(&mbx); tma_prefetch_desc(&mwx); tma_prefetch_desc(&mo);
     }
     if (warp == 0) tmem_alloc(&mi.tmem_base, TM_COLS);
     for (int i = tid; i < R2 * DV; i += NTH) {
@@ -326,6 +327,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 0);
         // ---- P0: fold G^T = S^T Ucat^T -> TM_X2[0, R2)
         PHASE_SYNC();
+        if (tid == 0 && c > 0) {   // the previous chunk's outputs (staged in Y2 by P13)
+            for (int cb = 0; cb < DV / 64; ++cb) tma_store_3d(&mo, sb + Lo.Y2 + cb * 8192, vofs + cb * 64, h, b * a.T + (c - 1) * LCc);
+            bulk_commit();
+        }
         PROF(g_prof_fwd, 20);
         if (rc && tid == REC_TID) {   // record: state entering the chunk (Sb stays intact until P13)
             bulk_s2g(rc + Rc.SB, sb + Lo.Sb, (uint32_t)state_tile);
@@ -426,35 +431,31 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         WAIT_MMA();
         PROF(g_prof_fwd, 3);
-        // ---- P3: tt = tanh(Z rnorm_q) -> [tt_b pad 16 | tt_w pad 16] (both row halves)
-        if (!krole && half == 0 && warp_active) {
+        // ---- P3: tt = tanh(Z rnorm_q) -> [tt_b pad 16 | tt_w pad 16] (both row halves); the 2r <= 32 bottleneck columns
+        //      are spread over the Q-side warps of all column parts, 8 columns (one 16-byte chunk) at a time
+        if (!krole && warp_active) {
             const float rnq = a.l2norm ? rsqrtf(sumsq(row) + a.eps) : 1.f;
             const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
-            for (int c0 = 0; c0 < R2; c0 += 16) {
-                uint32_t v[16];
-                tmem_ld16(tmem + TM_X2 + 32 + lane_base + c0, v);
-                tmem_wait_ld();
-                if (live) {
-                    float f[16];
 #pragma unroll
-                    for (int e = 0; e < 16; ++e) f[e] = tanh_fast(__uint_as_float(v[e]) * rnq);
-                    if (rc) {
-                        *reinterpret_cast<uint4*>(rc + Rc.tt + t * 64 + c0 * 2) = pack8(f);
-                        *reinterpret_cast<uint4*>(rc + Rc.tt + t * 64 + c0 * 2 + 16) = pack8(f + 8);
-                    }
+            for (int sc = half * (4 / NP); sc < (half + 1) * (4 / NP); ++sc) {
+                if (8 * sc < R2) {
+                    uint32_t v[8];
+                    tmem_ld8(tmem + TM_X2 + 32 + lane_base + 8 * sc, v);
+                    tmem_wait_ld();
+                    if (live) {
+                        float f[8];
 #pragma unroll
-                    for (int k8 = 0; k8 < 2; ++k8) {
-                        const int col = c0 + 8 * k8;       // tt columns [col, col+8)
-                        const uint4 w = pack8(f + 8 * k8);
-                        const bool is_b = col < r;         // erase-gate half of the bottleneck
-                        const int dst = is_b ? col / 8 : 2 + (col - r) / 8;   // [tt_b pad 16 | tt_w pad 16], both row halves
+                        for (int e = 0; e < 8; ++e) f[e] = tanh_fast(__uint_as_float(v[e]) * rnq);
+                        const uint4 w = pack8(f);
+                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.tt + t * 64 + sc * 16) = w;
+                        const int dst = 8 * sc < r ? sc : 2 + (8 * sc - r) / 8;   // erase half | write half, each padded to 16
                         sts128(sm + Lo.Y1 + tile_chunk_off(128, 64 + t, dst), w);
                         sts128(sm + Lo.Y1 + tile_chunk_off(128, t, dst), w);
                     }
-                    if (r < 16) {
-                        sts128(sm + Lo.Y1 + tile_chunk_off(128, 64 + t, 1), z4); sts128(sm + Lo.Y1 + tile_chunk_off(128, t, 1), z4);
-                        sts128(sm + Lo.Y1 + tile_chunk_off(128, 64 + t, 3), z4); sts128(sm + Lo.Y1 + tile_chunk_off(128, t, 3), z4);
-                    }
+                } else if (live) {   // r = 8: the padding chunks 1 and 3
+                    const int dst = 2 * (sc - R2 / 8) + 1;
+                    sts128(sm + Lo.Y1 + tile_chunk_off(128, 64 + t, dst), z4);
+                    sts128(sm + Lo.Y1 + tile_chunk_off(128, t, dst), z4);
                 }
             }
         }
@@ -556,6 +557,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             }
         }
         PROF(g_prof_fwd, 6);
+        if (tid == 0) bulk_wait_read();   // the output tile has left Y2 (rewritten below)
         __syncthreads();
         PROF(g_prof_fwd, 8);
         // ---- P7b: decayed operands.  Row operands exist in up to four anchorings: version 0 relative to the chunk
@@ -849,7 +851,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 16);
         // ---- P13: outputs and the state carry
         if (!krole && warp_active) {
-            __nv_bfloat16* dst = a.O + ((tok0 + t) * a.H + h) * a.dvf + vofs;
             uint32_t v[32];
             tmem_ld32(tmem + TM_ACC + lane_base + half * HV, v);
             tmem_wait_ld();
@@ -859,7 +860,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     float f[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e) f[e] = a.scale * __uint_as_float(v[8 * ch + e]);
-                    *reinterpret_cast<uint4*>(dst + 8 * (half * 4 + ch)) = pack8(f);
+                    // staged as a bf16 row tile over beta R (dead since the solve); a TMA store sends it to HBM after the
+                    // next barrier: 16 KB of STG from one SM would hold the warps for ~500 cycles (27-32 B/clk per SM)
+                    sts128(sm + Lo.Y2 + tile_chunk_off(64, t, half * 4 + ch), pack8(f));
                 }
             }
         }
@@ -904,6 +907,11 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     PROF_FLUSH(g_prof_fwd)
     if (VS > 1) cluster_wait();   // pairs with the last arrive; also keeps this CTA's shared memory alive for the peer
     PHASE_SYNC();
+    if (tid == 0) {   // the last chunk's outputs
+        for (int cb = 0; cb < DV / 64; ++cb) tma_store_3d(&mo, sb + Lo.Y2 + cb * 8192, vofs + cb * 64, h, b * a.T + (nchunks - 1) * LCc);
+        bulk_commit();
+        bulk_wait_all();
+    }
     if (rec_chain && (tid == 0 || tid == REC_TID)) bulk_wait_all();   // drain the record's bulk stores
     if (warp == 0) tmem_dealloc(tmem, TM_COLS);
 }
@@ -966,7 +974,8 @@ template <int D, int VS>
 static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
 {
     const int LCc = a.L < tcp::LC ? a.L : tcp::LC;
-    CUtensorMap mq, mk, mv, mf, mbx, mwx;
+    CUtensorMap mq, mk, mv, mf, mbx, mwx, mo;
+    if (!tc_make_token_map(&mo, a.O, a.B, a.T, a.H, a.dv, LCc)) return cudaErrorInvalidValue;
     if (!tc_make_token_map(&mq, a.q, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mk, a.k, a.B, a.T, a.H, D, LCc) ||
         !tc_make_token_map(&mv, a.v, a.B, a.T, a.H, a.dv, LCc) || !tc_make_token_map(&mf, a.f, a.B, a.T, a.H, D, LCc) ||
         !tc_make_token_map(&mbx, a.bx, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mwx, a.wx, a.B, a.T, a.H, a.dv, LCc))
@@ -992,7 +1001,7 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
     attr[0].val.clusterDim.x = VS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kern, t, mq, mk, mv, mf, mbx, mwx);
+    return cudaLaunchKernelEx(&cfg, kern, t, mq, mk, mv, mf, mbx, mwx, mo);
 }
 
 cudaError_t tc_fwd_launch(const Args& a, uint8_t* rec, cudaStream_t st)
