@@ -4,21 +4,20 @@
 // One persistent CTA per (batch, head) chain walks the sequence in solve chunks of LC = 64 tokens
 // (a gate chunk of L = 128 is two solve chunks that share one folded readout G_c; L = 16, 32 run
 // as short solve chunks).  Per solve chunk, in the order of PAPER.md Alg. 1-2 (l.160-196, l.315-365):
-//   P0  G^T = S^T [Ub;Uw]^T                       fold, Eq. 7 (l.134)                       [MMA]
-//   P2  Z = [k;q] G^T, tt = tanh(Z rnorm_q)       bottleneck, Eq. 7                          [MMA]
-//   P4  [w_proj; b_proj] = [0 tt_w; tt_b 0] [Vb|Vw]^T   up-projections, Eq. 8 (l.140)       [MMA]
-//   P5  la = g - softplus(bx + b_proj)  (= log a_t, Eq. 9 l.151, Eq. 14 l.310);  V' = sigmoid(wx + w_proj) v
-//   P6  block-local prefix sums of la over tokens (Eq. 14) as a product with a 0/+-1 triangular
-//       matrix, la split in bf16 hi + lo so the sums keep fp32 accuracy                      [MMA]
-//   P7  decayed operands, every exponent relative to the start of its 32-token block:
+//   P0  G^T = S^T [Ub;Uw]^T                       fold, Eq. 7 (l.134)                       [tcgen05]
+//   P2  Z = [k;q] G^T, tt = tanh(Z rnorm_q)       bottleneck, Eq. 7                          [tcgen05]
+//   P4  [b_proj | w_proj] = [tt_b | tt_w] [Vb | Vw]^T    up-projections, Eq. 8 (l.140)      [tcgen05]
+//   P5  V' = sigmoid(wx + w_proj) v;  la = g - softplus(bx + b_proj)  (= log a_t, Eq. 9 l.151, Eq. 14 l.310);
+//       block-local prefix sums of la over the 16 tokens of an anchor block: segmented warp scan in fp32 registers
+//   P7  decayed operands, every exponent relative to the start of a 16-token anchor block:
 //       Kbar_t = k^_t gamma_{t-1}, Qbar_t = q^_t gamma_t, C_s = k^_s gamma_a/gamma_s, Ktil_t = k^_t gamma_L/gamma_t
-//   P8  A|P blocks = [Kbar;Qbar] C^T (Eq. 15 l.342);  [Kbar;Qbar] S^T (Alg. 2 steps 5, 8)   [MMA]
-//   P9  T = (I + diag(beta) A)^-1 by blocked forward substitution (Alg. 2 step 7);  beta R = beta (V' - Kbar S^T)
-//   P10 U = T (beta R)                                                                     [MMA]
-//   P12 O += P U (step 8);  W = U^T Ktil (step 9)                                          [MMA]
-//   P13 O -> HBM;  S <- S diag(gamma_L) + W  (fp32, TMEM), bf16 copy for the next chunk's MMAs
+//   P8  A|P blocks = [Kbar;Qbar] C^T (Eq. 15 l.342);  [Kbar;Qbar] S^T (Alg. 2 steps 5, 8)   [tcgen05]
+//   P9  beta A, P (masked), beta R = beta (V' - Kbar S^T);  WY solve U = (I + diag(beta) A)^-1 beta R by blocked forward
+//       substitution in registers (Alg. 2 step 7), T = (I + diag(beta) A)^-1 for the chunk record   [mma.sync tf32]
+//   P12 O += P U (step 8);  W = U^T Ktil (step 9)                                          [tcgen05]
+//   P13 O -> bf16 tile -> TMA store;  S <- S diag(gamma_L) + W  (fp32, TMEM), bf16 copy for the next chunk's MMAs
 // Decay ratios: with log a ~ -1.6 per token gamma_L reaches e^-100 per chunk, so no 1/gamma is ever
-// formed over more than one 32-token block; across blocks only ratios <= 1 are multiplied in.
+// formed over more than one 16-token block; across blocks only ratios <= 1 are multiplied in.
 #include <mutex>
 
 #include "carve_tc.cuh"

@@ -96,16 +96,20 @@ def test_stress_conditioning(oracle):
 
 
 def test_extreme_decay_no_overflow(oracle):
-    """Strong decay/erase (log gamma_L ~ -600 per chunk): every ratio is formed as exp(<=0).
-    Gradient tolerance 5e-4: an fp32 prefix sum of magnitude ~150 puts ~8e-6 absolute error
-    into every exp(lg_a - lg_b), and df sums ~1e2 such terms of both signs.  dA and dtau are sums of dg.g / df over
-    all T tokens (Eq. 9 l.151) that cancel to ~1/10 of their terms here, so they carry 10x that: 5e-3; the same
-    holds for the other token-summed weight gradients fed by d log a (dUb, dVb through db_pre, Alg. 5 l.846)."""
+    """Strong decay/erase (log gamma_L ~ -600 per chunk, |lg| ~ 150 inside one 16-token sub-chunk): every ratio is formed
+    as exp(<= 0), nothing overflows.  Not a BASELINE config.  Tolerances per tensor (measured on
+    B200 next to each bound): everything that does not pass through d log a keeps north_star's 1e-4 (measured <= 5e-7,
+    dUw and dVw included: the write gate is not fed by d log a).  df and dbx ARE d log a times a local factor: an fp32
+    prefix sum of magnitude 150 carries ulp/2 ~ 8e-6 absolute error into every exp(lg_a - lg_b), and d log a sums ~1e2
+    such terms of both signs: 5e-4 (measured 2.3e-4, 2.5e-4).  dA, dtau (Eq. 9 l.151) and dUb, dVb (the erase gate's
+    projections, fed by db_pre = -d log a . b, Alg. 5 l.846) are sums of those over all T tokens that cancel to ~1/10 of
+    their terms: 5e-3 (measured 2.9e-3, 2.2e-3, 1.2e-3, 1.5e-3)."""
     cfg = synth.Config("t", B=1, H=1, T=128, L=64, dk=64, dv=64, r=8, dtype="f32", wstd=0.1, s0_std=0.1, seed=4)
     x = synth.make_inputs(cfg)
     x["f"] = x["f"] + 5.0
     x["bx"] = x["bx"] + 5.0
-    _check_fwd_bwd(oracle, cfg, x, tol=dict(O=1e-4, S=1e-4, g=5e-4, dA=5e-3, dtau=5e-3, dUb=5e-3, dVb=5e-3, dUw=5e-3, dVw=5e-3))
+    errs = _check_fwd_bwd(oracle, cfg, x, tol=dict(O=1e-4, S=1e-4, g=1e-4, df=5e-4, dbx=5e-4, dA=5e-3, dtau=5e-3, dUb=5e-3, dVb=5e-3))
+    print("extreme decay, measured:", {n: f"{v:.1e}" for n, v in errs.items()})
 
 
 # ---- invariants that need no oracle -------------------------------------------------------------
