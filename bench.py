@@ -45,12 +45,12 @@ def get_cfg(name: str) -> synth.Config:
 
 
 # ---- algorithmic bytes / flops -------------------------------
-def algorithmic(cfg: synth.Config):
+def algorithmic(cfg: synth.Config, scalar_write: bool = False):
     e = 2 if cfg.dtype == "bf16" else 4
     dk, dv, r, L = cfg.dk, cfg.dv, cfg.r, cfg.L
     tokh = cfg.B * cfg.T * cfg.H
     chains = cfg.B * cfg.H
-    n_in = 2 * dk + dv + dk + dk + dv + 1
+    n_in = 2 * dk + dv + dk + dk + (0 if scalar_write else dv) + 1      # scalar-write variant: no wx in, no dwx out
     fwd_b = tokh * (e * n_in + e * dv) + chains * 4 * dv * dk * 2
     bwd_b = tokh * (e * n_in + e * dv + e * n_in) + chains * 4 * dv * dk * 2
     fwd_f = (4 * r * dv * dk + 4 * L * r * dk + 2 * L * r * (dk + dv) + L * (L - 1) * dk + L * (L + 1) * dk +
@@ -154,7 +154,8 @@ def base_line(cfg: synth.Config, args, n_gpus: int) -> dict:
             "dtype": "bf16 tokens, f32 state/accumulate" if cfg.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": f"{cfg.name}: B={cfg.B} (per GPU),H={cfg.H},T={cfg.T},L={cfg.L},dk={cfg.dk},"
                                    f"dv={cfg.dv},r={cfg.r},{cfg.dtype},S0={'N(0,%g)' % cfg.s0_std if cfg.s0_std else 0}"
-                                   f"{', fwd only' if cfg.fwd_only else ', fwd+bwd'}",
+                                   f"{', fwd only' if cfg.fwd_only else ', fwd+bwd'}"
+                                   f"{', scalar-write variant (w == 1)' if getattr(args, 'scalar_write', False) else ''}",
                        "seed": cfg.seed, "parallelism": f"dp{n_gpus} over batch (independent chains)",
                        "l2": "inputs (>=0.8 GB per pass) exceed the 126 MB L2; no explicit flush"},
             "context": PAPER_CONTEXT}
@@ -215,6 +216,9 @@ def run_ours(args):
 
     xh = {n: host_t(n, a) for n, a in x.items()}
     dOh, dSfh = host_t("dO", ct["dO"]), host_t("dS_final", ct["dS_final"])
+    if args.scalar_write:      # P section 4.2 l.145: w == 1, the scalar write gate is inside beta (carve.h)
+        for n in ("wx", "Uw", "Vw"):
+            xh[n] = None
     xd = {n: (None if t is None else t.cuda()) for n, t in xh.items()}
     dOd, dSfd = dOh.cuda(), dSfh.cuda()
     dev = torch.device("cuda", local)
@@ -243,6 +247,9 @@ def run_ours(args):
         return g
 
     grads = mk_grads(dev) if with_bwd else None
+    if args.scalar_write and grads:
+        for n in ("dwx", "dUw", "dVw"):
+            grads[n] = None
     ws = torch.empty(carve.carve_workspace_bytes(p, True), dtype=torch.uint8, device=dev) if with_bwd else None
     stream = torch.cuda.current_stream()
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -299,12 +306,13 @@ def run_ours(args):
     nb = lambda t: 0 if t is None else t.numel() * t.element_size()
     h2d = sum(nb(t) for t in xh.values()) + (nb(dOh) + nb(dSfh) if with_bwd else 0)
     d2h = nb(Oh) + nb(Sfh) + (sum(nb(t) for t in gh.values()) if with_bwd else 0)
-    e2e_steps = max(1, min(args.steps, 5))
+    e2e_steps = 0 if args.scalar_write else max(1, min(args.steps, 5))   # the host entry point takes the full write gate only
 
     def e2e_step():
         carve.carve_fwd_bwd_host(p, with_bwd, xh, Oh, Sfh, dOh if with_bwd else None, dSfh if with_bwd else None,
                                  gh, arena, stream.cuda_stream)
-    e2e_step()
+    if e2e_steps:
+        e2e_step()
     barrier()
     e0, e1 = ev(), ev()
     e0.record(stream)
@@ -317,10 +325,10 @@ def run_ours(args):
         t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_ms = float(t.item())
-    e2e_value = tokens_job / (e2e_ms / e2e_steps * 1e-3)
+    e2e_value = tokens_job / (e2e_ms / e2e_steps * 1e-3) if e2e_steps else None
 
     if rank == 0:
-        alg = algorithmic(cfg)
+        alg = algorithmic(cfg, args.scalar_write)
         peaks = load_peaks()
         dom = "bwd" if (with_bwd and bwd_ms >= fwd_ms) else "fwd"
         dom_ms = bwd_ms if dom == "bwd" else fwd_ms
@@ -330,7 +338,7 @@ def run_ours(args):
         tpath = os.path.join(ROOT, "profiles", "r2_tc_traffic.csv")
         if not os.path.exists(tpath):
             tpath = os.path.join(ROOT, "profiles", "r1_tc_traffic.csv")
-        if cfg.name == synth.CFG1.name and not args.fwd_only and os.path.exists(tpath):
+        if cfg.name == synth.CFG1.name and not args.fwd_only and not args.scalar_write and os.path.exists(tpath):
             for ln in open(tpath).read().splitlines()[1:]:
                 f = ln.split(",")
                 if f[0] == f"carve_{dom}":
@@ -342,7 +350,7 @@ def run_ours(args):
         line.update({
             "value": value, "ms_per_step": ms_step, "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "tokens/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+                    "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps if e2e_steps else None},
             "gpu_launches": args.steps * (carve.carve_num_launches(p, False) +
                                           (carve.carve_num_launches(p, True) if with_bwd else 0)),
             "kernel_path": {1: "simt-fp32", 2: "tensor-tcgen05"}.get(path, str(path)),
@@ -380,6 +388,8 @@ def main():
     ap.add_argument("--config", default="cfg1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fwd-only", action="store_true", help="time carve_fwd alone (inference call, nothing saved)")
+    ap.add_argument("--scalar-write", action="store_true",
+                    help="the scalar-write variant (wx = Uw = Vw = NULL, PAPER.md section 4.2): not the BASELINE.json metric's workload")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
         # plain `python bench.py --gpus N`: start the N ranks ourselves (one process per GPU, NCCL), the same way the

@@ -95,6 +95,11 @@ size_t carve_workspace_bytes(const carve_params_t *p, int need_bwd);
  *   S_final [B,H,dv,dk] float   out
  *   workspace                   NULL: inference, nothing saved.  Otherwise >= carve_workspace_bytes(p,1)
  *                               bytes; it is filled for the matching carve_bwd call.
+ * Scalar-write variant (P section 4.2 l.145, Thm 15 l.762-764: the per-head scalar write gate w_{h,t} = sigmoid(w^_{h,t}),
+ * broadcast over d_v, is sufficient; reading A1: that scalar multiplies the whole error, so it is passed inside beta):
+ * wx = Uw = Vw = NULL (all three) selects kernels' w == 1 path: V' = v, no write-gate load, projection or sigmoid, and
+ * the training forward saves nothing for it.  carve_bwd / carve_step take the same three NULLs; carve_bwd then does not
+ * write dwx, dUw, dVw (they may be NULL).  Only some of the three NULL is CARVE_ERR_NULL.
  */
 carve_status_t carve_fwd(const carve_params_t *p, const void *q, const void *k, const void *v,
                          const void *f, const void *bx, const void *wx, const void *beta,

@@ -49,6 +49,13 @@ int resolve_path(const carve_params_t* p, bool bwd)
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// Scalar-write variant (carve.h): wx, Uw, Vw all NULL.  Returns false when only some of the three are NULL.
+bool write_gate_args_ok(const void* wx, const float* Uw, const float* Vw)
+{
+    const int n = (wx == nullptr) + (Uw == nullptr) + (Vw == nullptr);
+    return n == 0 || n == 3;
+}
+
 carve_status_t check_arch()
 {
     int dev = 0;
@@ -142,7 +149,7 @@ carve_status_t carve_fwd(const carve_params_t* p, const void* q, const void* k, 
 {
     carve_status_t s = check_params(p, workspace != nullptr);
     if (s != CARVE_OK) return s;
-    if (!q || !k || !v || !f || !bx || !wx || !beta || !Ub || !Uw || !Vb || !Vw || !O || !S_final) return CARVE_ERR_NULL;
+    if (!q || !k || !v || !f || !bx || !beta || !Ub || !Vb || !O || !S_final || !write_gate_args_ok(wx, Uw, Vw)) return CARVE_ERR_NULL;
     for (const void* ptr : {q, k, v, f, bx, wx, beta, (const void*)A, (const void*)tau, (const void*)Ub,
                             (const void*)Uw, (const void*)Vb, (const void*)Vw, (const void*)S0, (const void*)O,
                             (const void*)S_final, (const void*)workspace})
@@ -180,7 +187,7 @@ carve_status_t carve_step(const carve_params_t* p, const void* q, const void* k,
     if (p->dtype != CARVE_F32 && p->dtype != CARVE_BF16) return CARVE_ERR_DTYPE;
     if (p->B <= 0 || p->H <= 0 || p->T < 1 || p->T > 16) return CARVE_ERR_SHAPE;
     if (!step_supported(p->dk, p->dv) || !one_of(p->r, {8, 16, 32})) return CARVE_ERR_SHAPE;
-    if (!q || !k || !v || !f || !bx || !wx || !beta || !Ub || !Uw || !Vb || !Vw || !S || !O) return CARVE_ERR_NULL;
+    if (!q || !k || !v || !f || !bx || !beta || !Ub || !Vb || !S || !O || !write_gate_args_ok(wx, Uw, Vw)) return CARVE_ERR_NULL;
     for (const void* ptr : {q, k, v, f, bx, wx, beta, (const void*)A, (const void*)tau, (const void*)Ub, (const void*)Uw,
                             (const void*)Vb, (const void*)Vw, (const void*)S, (const void*)O})
         if (!aligned16(ptr)) return CARVE_ERR_ALIGN;
@@ -204,9 +211,11 @@ static carve_status_t bwd_impl(const carve_params_t* p, const void* q, const voi
 {
     carve_status_t s = check_params(p, true);
     if (s != CARVE_OK) return s;
-    if (!q || !k || !v || !f || !bx || !wx || !beta || !Ub || !Uw || !Vb || !Vw || !dO || !dq || !dk || !dv || !df ||
-        !dbx || !dwx || !dbeta || !dUb || !dUw || !dVb || !dVw || !dS0)
+    if (!q || !k || !v || !f || !bx || !beta || !Ub || !Vb || !dO || !dq || !dk || !dv || !df || !dbx || !dbeta || !dUb ||
+        !dVb || !dS0 || !write_gate_args_ok(wx, Uw, Vw))
         return CARVE_ERR_NULL;
+    if (wx && (!dwx || !dUw || !dVw)) return CARVE_ERR_NULL;   // (scalar-write variant: dwx, dUw, dVw are not written)
+    if (!wx) { dwx = nullptr; dUw = nullptr; dVw = nullptr; }
     for (const void* ptr : {q, k, v, f, bx, wx, beta, (const void*)A, (const void*)tau, (const void*)Ub,
                             (const void*)Uw, (const void*)Vb, (const void*)Vw, (const void*)S0, dO,
                             (const void*)dS_final, (const void*)dq, (const void*)dk, (const void*)dv,
@@ -319,7 +328,7 @@ carve_status_t carve_fwd_bwd_host(const carve_params_t* p, int with_bwd, const v
     if (s != CARVE_OK) return s;
     if (!device_arena || arena_bytes < carve_host_arena_bytes(p, with_bwd)) return CARVE_ERR_WORKSPACE;
     if (!aligned16(device_arena)) return CARVE_ERR_ALIGN;
-    if (!q || !k || !v || !f || !bx || !wx || !beta || !Ub || !Uw || !Vb || !Vw || !O || !S_final) return CARVE_ERR_NULL;
+    if (!q || !k || !v || !f || !bx || !wx || !beta || !Ub || !Uw || !Vb || !Vw || !O || !S_final) return CARVE_ERR_NULL;   // (full write gate only)
     if (with_bwd && (!dO || !dq || !dk || !dv || !df || !dbx || !dwx || !dbeta || !dUb || !dUw || !dVb || !dVw || !dS0))
         return CARVE_ERR_NULL;
     if (resolve_path(p, with_bwd != 0) < 0) return CARVE_ERR_SHAPE;

@@ -120,14 +120,14 @@ __global__ void __launch_bounds__(NT, 1) carve_fwd_simt_kernel(const Args a)
 #pragma unroll
                 for (int ii = 0; ii < 4; ++ii) {
                     const int i = 4 * ib + ii;
-                    Urow[ii] = (i < r) ? a.Ub + (size_t)i * DV : a.Uw + (size_t)(i - r) * DV;
+                    Urow[ii] = (i < r) ? a.Ub + (size_t)i * DV : (a.Uw ? a.Uw + (size_t)(i - r) * DV : nullptr);
                 }
                 for (int x = 0; x < DV; x += 4) {
                     const float4 s0 = ld4s(sS + (x + 0) * SP + 4 * j4), s1 = ld4s(sS + (x + 1) * SP + 4 * j4),
                                  s2 = ld4s(sS + (x + 2) * SP + 4 * j4), s3 = ld4s(sS + (x + 3) * SP + 4 * j4);
 #pragma unroll
                     for (int ii = 0; ii < 4; ++ii) {
-                        const float4 u = ldg4(Urow[ii] + x);
+                        const float4 u = Urow[ii] ? ldg4(Urow[ii] + x) : make_float4(0.f, 0.f, 0.f, 0.f);   // scalar-write variant: no Uw
                         acc[ii].x += u.x * s0.x + u.y * s1.x + u.z * s2.x + u.w * s3.x;
                         acc[ii].y += u.x * s0.y + u.y * s1.y + u.z * s2.y + u.w * s3.y;
                         acc[ii].z += u.x * s0.z + u.y * s1.z + u.z * s2.z + u.w * s3.z;
@@ -201,10 +201,14 @@ __global__ void __launch_bounds__(NT, 1) carve_fwd_simt_kernel(const Args a)
         for (int it = tid; it < SC * DV; it += NT) {
             const int x = it % DV, t = it / DV;
             const size_t go = tokoff(t0 + t) * DV + x;
-            float wp = ldf(gwx, go);
-            for (int i4 = 0; i4 < r / 4; ++i4)
-                wp += dot4(ldg4(a.Vw + (size_t)x * r + 4 * i4), ld4s(sT + t * R2 + r + 4 * i4));
-            sU[t * DV + x] = sigmoidf_(wp) * ldf(gv, go);
+            float w = 1.f;   // scalar-write variant (wx = NULL, P l.145): the write gate is the scalar already in beta
+            if (gwx) {
+                float wp = ldf(gwx, go);
+                for (int i4 = 0; i4 < r / 4; ++i4)
+                    wp += dot4(ldg4(a.Vw + (size_t)x * r + 4 * i4), ld4s(sT + t * R2 + r + 4 * i4));
+                w = sigmoidf_(wp);
+            }
+            sU[t * DV + x] = w * ldf(gv, go);
         }
         __syncthreads();
         // ---- F4: retention prefix (Eq. 14) and the decayed operands

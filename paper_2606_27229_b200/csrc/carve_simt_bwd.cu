@@ -371,13 +371,17 @@ __global__ void __launch_bounds__(NT, 1) carve_bwd_simt_kernel(const Args a)
         for (int it = tid; it < SC * DV; it += NT) {
             const int x = it % DV, t = it / DV;
             const size_t go = tokoff(t0 + t) * DV + x;
-            float wp = ldf(gwx, go);
-            for (int i4 = 0; i4 < r / 4; ++i4)
-                wp += dot4(ldg4(a.Vw + (size_t)x * r + 4 * i4), ld4s(sT + t * R2 + r + 4 * i4));
-            const float w = sigmoidf_(wp), dr = sDU[it];
-            const float dwp = dr * ldf(gv, go) * w * (1.f - w);
+            float w = 1.f;   // scalar-write variant (wx = NULL): w == 1, no write-gate adjoint
+            if (gwx) {
+                float wp = ldf(gwx, go);
+                for (int i4 = 0; i4 < r / 4; ++i4)
+                    wp += dot4(ldg4(a.Vw + (size_t)x * r + 4 * i4), ld4s(sT + t * R2 + r + 4 * i4));
+                w = sigmoidf_(wp);
+            }
+            const float dr = sDU[it];
+            const float dwp = gwx ? dr * ldf(gv, go) * w * (1.f - w) : 0.f;
             stf(gdv, go, dr * w);
-            stf(gdwx, go, dwp);
+            if (gwx) stf(gdwx, go, dwp);
             sU[it] = dwp;
         }
         //      pairwise terms.  role 0 (thread j < DK): row sums, kept in registers;
@@ -467,7 +471,8 @@ __global__ void __launch_bounds__(NT, 1) carve_bwd_simt_kernel(const Args a)
         for (int it = tid; it < SC * r; it += NT) {
             const int i = it % r, t = it / r;
             float s = 0.f;
-            for (int x = 0; x < DV; ++x) s += sU[t * DV + x] * __ldg(a.Vw + (size_t)x * r + i);
+            if (a.Vw)
+                for (int x = 0; x < DV; ++x) s += sU[t * DV + x] * __ldg(a.Vw + (size_t)x * r + i);
             const float tv = sT[t * R2 + r + i];
             sDz[t * R2 + r + i] = s * (1.f - tv * tv);
         }
@@ -574,7 +579,7 @@ __global__ void __launch_bounds__(NT, 1) carve_bwd_simt_kernel(const Args a)
             for (int j4 = ptg * (JR / 4); j4 < (ptg + 1) * (JR / 4); ++j4) {
                 float4 d4 = ld4s(sDS + px * SP + 4 * j4);
                 for (int i = 0; i < R2; ++i) {
-                    const float u = (i < r) ? __ldg(a.Ub + (size_t)i * DV + px) : __ldg(a.Uw + (size_t)(i - r) * DV + px);
+                    const float u = (i < r) ? __ldg(a.Ub + (size_t)i * DV + px) : (a.Uw ? __ldg(a.Uw + (size_t)(i - r) * DV + px) : 0.f);
                     const float4 g4 = ld4s(sDG + i * DK + 4 * j4);
                     d4.x += u * g4.x; d4.y += u * g4.y; d4.z += u * g4.z; d4.w += u * g4.w;
                 }
@@ -604,9 +609,9 @@ __global__ void carve_reduce_weights_kernel(const float* __restrict__ part, int 
         float s = 0.f;
         for (int c = 0; c < chains; ++c) s += part[(size_t)c * stride + idx];
         if (idx < nU) dUb[idx] = s;
-        else if (idx < 2 * nU) dUw[idx - nU] = s;
+        else if (idx < 2 * nU) { if (dUw) dUw[idx - nU] = s; }   // NULL in the scalar-write variant
         else if (idx < 2 * nU + nVb) dVb[idx - 2 * nU] = s;
-        else dVw[idx - 2 * nU - nVb] = s;
+        else if (dVw) dVw[idx - 2 * nU - nVb] = s;
     } else if (idx < nW + 2 * H * dk) {
         const int k = idx - nW, which = k / (H * dk), hj = k % (H * dk), h = hj / dk, j = hj % dk;
         float* out = which ? dtau : dA;

@@ -60,10 +60,12 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
     // fold: G[i][j] = sum_x Ucat[i][x] S[x][j]   (once per call: the gates of all n tokens read the incoming state)
     for (int o = tid; o < R2 * DK; o += NT) {
         const int i = o / DK, j = o % DK;
-        const float* urow = i < r ? a.Ub + (size_t)i * DV : a.Uw + (size_t)(i - r) * DV;
+        const float* urow = i < r ? a.Ub + (size_t)i * DV : (a.Uw ? a.Uw + (size_t)(i - r) * DV : nullptr);
         float acc = 0.f;
+        if (urow) {
 #pragma unroll 4
-        for (int x = 0; x < DV; ++x) acc = fmaf(__ldg(urow + x), sS[x * SP + j], acc);
+            for (int x = 0; x < DV; ++x) acc = fmaf(__ldg(urow + x), sS[x * SP + j], acc);
+        }
         sG[i * SP + j] = acc;
     }
     __syncthreads();
@@ -103,9 +105,13 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
                 sA[j] = expf(g - softplusf(pre));          // exp(g) (1 - sigmoid(pre)),  log(1 - sigmoid(x)) = -softplus(x)
             } else {
                 const int x = j - DK;
-                float pre = ldf<T>(gwx, tok * DV + x);
-                for (int i = 0; i < r; ++i) pre = fmaf(__ldg(a.Vw + (size_t)x * r + i), sT[r + i], pre);
-                sW[x] = sigmoidf_(pre) * ldf<T>(gv, tok * DV + x);
+                float w = 1.f;   // scalar-write variant (wx = NULL, P l.145)
+                if (gwx) {
+                    float pre = ldf<T>(gwx, tok * DV + x);
+                    for (int i = 0; i < r; ++i) pre = fmaf(__ldg(a.Vw + (size_t)x * r + i), sT[r + i], pre);
+                    w = sigmoidf_(pre);
+                }
+                sW[x] = w * ldf<T>(gv, tok * DV + x);
             }
         }
         __syncthreads();

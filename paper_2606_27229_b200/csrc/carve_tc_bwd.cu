@@ -38,6 +38,7 @@ PROF_DECL(g_prof_bwd)
 struct BwdArgs {
     int B, H, T, L, r;
     int l2norm;
+    int sw;       // scalar-write variant (wx = Uw = Vw = NULL): w == 1, no write-gate adjoint, dwx / dUw / dVw not produced
     float scale, eps;
     const uint8_t* rec;
     const float* dS_final;
@@ -175,7 +176,7 @@ __device__ __forceinline__ void warp_colsum(float (&v)[N], int lane)
     } while (0)
 
 // NP = column parts per tile row = warpgroups per CTA (threads = 128 NP): 32 columns per thread.
-template <int D, int NP>
+template <int D, int NP, int SW>   // SW = 1: scalar-write variant (w == 1), compiled separately
 __global__ void __launch_bounds__(128 * NP, 1)
 carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, const __grid_constant__ CUtensorMap mq)
 {
@@ -221,7 +222,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         const int ii = i / D, n = i % D;
         float vc = 0.f, uc = 0.f;
         if (ii < r) { vc = __ldg(a.Vb + (size_t)n * r + ii); uc = __ldg(a.Ub + (size_t)ii * D + n); }
-        else if (ii < R2) { vc = __ldg(a.Vw + (size_t)n * r + (ii - r)); uc = __ldg(a.Uw + (size_t)(ii - r) * D + n); }
+        else if (ii < R2 && !SW) { vc = __ldg(a.Vw + (size_t)n * r + (ii - r)); uc = __ldg(a.Uw + (size_t)(ii - r) * D + n); }
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.VcT + tile_off(32, ii, n)) = __float2bfloat16_rn(vc);
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Ucat + tile_off(32, ii, n)) = __float2bfloat16_rn(uc);
     }
@@ -340,12 +341,18 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         const int cq0 = ((krole ? 0 : D / 2) + half * QW) / 8;
         // row-private record data of L2 straight from global memory, issued now so that the latency hides behind L1
         uint4 x4[QW / 8], w4[QW / 8];
-        if (live) {
+        if (live && !SW) {
 #pragma unroll
             for (int i = 0; i < QW / 8; ++i) {
                 const uint32_t off = rp_off(t, cq0 + i);
                 x4[i] = ldg128(rc + Rc.VWX + off);
                 w4[i] = ldg128(rc + Rc.W + off);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < QW / 8; ++i) {   // w == 1, w v (1 - w) == 0
+                x4[i] = make_uint4(0u, 0u, 0u, 0u);
+                w4[i] = make_uint4(0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u);
             }
         }
         // ---- L1: dU = Ktil dS'^T + (scale P)^T dO -> BM_A rows 0..63;  dKtil = U dS' -> BM_KT rows 0..63
@@ -424,7 +431,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                     }
                     sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8(ndr));
                     stg128(gdv + 8 * cc, pack8(o1));
-                    stg128(gdwx + 8 * cc, pack8(o2));
+                    if (!SW) stg128(gdwx + 8 * cc, pack8(o2));
                 }
                 mi.dbp[(krole ? 0 : NP) + half][t] = dbs;
             }
@@ -795,7 +802,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             if (!krole && live) {
                 const __nv_bfloat16* gdwx = a.dwx + ((tok0 + t) * a.H + h) * D;
 #pragma unroll
-                for (int i = 0; i < HK / 8; ++i) d4[i] = *reinterpret_cast<const uint4*>(gdwx + 8 * (half * (HK / 8) + i));
+                for (int i = 0; i < HK / 8; ++i)
+                    d4[i] = SW ? make_uint4(0u, 0u, 0u, 0u) : *reinterpret_cast<const uint4*>(gdwx + 8 * (half * (HK / 8) + i));
 #pragma unroll
                 for (int i = 0; i < 4; ++i) t4[i] = ldg128(rc + Rc.tt + t * 64 + 16 * i);
             }
@@ -1127,7 +1135,7 @@ __global__ void carve_reduce_at_kernel(const float* __restrict__ partAT, float* 
     part[(size_t)chain * stride + nW + i] = s;
 }
 
-template <int D>
+template <int D, int SW>
 cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float* dA, float* dtau, float* dUb, float* dUw,
                           float* dVb, float* dVw, cudaStream_t st)
 {
@@ -1137,7 +1145,7 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
         return cudaErrorInvalidValue;
     BwdArgs t{};
     t.B = a.B; t.H = a.H; t.T = a.T; t.L = a.L; t.r = a.r; t.l2norm = a.l2norm; t.scale = a.scale; t.eps = a.eps;
-    t.rec = ws + w.rec; t.dS_final = a.dS_final;
+    t.rec = ws + w.rec; t.dS_final = a.dS_final; t.sw = a.wx == nullptr;
     t.Ub = a.Ub; t.Uw = a.Uw; t.Vb = a.Vb; t.Vw = a.Vw;
     t.dq = static_cast<__nv_bfloat16*>(a.dq); t.dk = static_cast<__nv_bfloat16*>(a.dk_);
     t.dv = static_cast<__nv_bfloat16*>(a.dv_); t.df = static_cast<__nv_bfloat16*>(a.df);
@@ -1148,7 +1156,7 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
     t.flags = reinterpret_cast<int*>(ws + w.flags);
     const size_t smem = BLayout(D).total;
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
-    auto kern = carve_bwd_tc_kernel<D, NP>;
+    auto kern = carve_bwd_tc_kernel<D, NP, SW>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int chains = a.B * a.H, nchunks = a.T / LCc;
@@ -1195,8 +1203,9 @@ bool tc_bwd_supported(const carve_params_t& p) { return tc_fwd_supported(p) && p
 cudaError_t tc_bwd_launch(const Args& a, uint8_t* ws, const TcWsLayout& w, float* dA, float* dtau, float* dUb, float* dUw,
                           float* dVb, float* dVw, cudaStream_t st)
 {
-    if (a.dk == 128) return launch_tc_bwd<128>(a, ws, w, dA, dtau, dUb, dUw, dVb, dVw, st);
-    if (a.dk == 64) return launch_tc_bwd<64>(a, ws, w, dA, dtau, dUb, dUw, dVb, dVw, st);
+    const bool sw = a.wx == nullptr;
+    if (a.dk == 128) return sw ? launch_tc_bwd<128, 1>(a, ws, w, dA, dtau, dUb, dUw, dVb, dVw, st) : launch_tc_bwd<128, 0>(a, ws, w, dA, dtau, dUb, dUw, dVb, dVw, st);
+    if (a.dk == 64) return sw ? launch_tc_bwd<64, 1>(a, ws, w, dA, dtau, dUb, dUw, dVb, dVw, st) : launch_tc_bwd<64, 0>(a, ws, w, dA, dtau, dUb, dUw, dVb, dVw, st);
     return cudaErrorInvalidValue;
 }
 

@@ -32,6 +32,7 @@ struct TcArgs {
     int B, H, T, L, r;
     int dvf;        // full d_v of the tensors (= VS x the value channels one CTA owns)
     int l2norm;
+    int sw;         // scalar-write variant (wx = Uw = Vw = NULL, P l.145): w == 1, V' = v, no write-gate load / projection / sigmoid
     float scale, eps;
     const __nv_bfloat16* beta;
     const float *A, *tau, *Ub, *Uw, *Vb, *Vw, *S0;
@@ -181,7 +182,9 @@ __device__ __forceinline__ void wy_solve(const float* Mm, const float* Tm, int n
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
-template <int DK, int DV, int NP, int VS>
+// SW = 1: scalar-write variant (wx = Uw = Vw = NULL, P l.145) -- w == 1, V' = v; compiled separately so that the full-gate
+// kernel carries none of its branches.
+template <int DK, int DV, int NP, int VS, int SW>
 __global__ void __launch_bounds__(128 * NP, 1)
 carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, const __grid_constant__ CUtensorMap mk,
                     const __grid_constant__ CUtensorMap mv, const __grid_constant__ CUtensorMap mf,
@@ -231,7 +234,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     if (warp == 0) tmem_alloc(&mi.tmem_base, TM_COLS);
     for (int i = tid; i < R2 * DV; i += NTH) {
         const int ii = i / DV, x = i % DV;
-        const float v = ii < r ? __ldg(a.Ub + (size_t)ii * a.dvf + vofs + x) : __ldg(a.Uw + (size_t)(ii - r) * a.dvf + vofs + x);
+        const float v = ii < r ? __ldg(a.Ub + (size_t)ii * a.dvf + vofs + x) : (SW ? 0.f : __ldg(a.Uw + (size_t)(ii - r) * a.dvf + vofs + x));
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Ucat + tile_off(R2, ii, x)) = __float2bfloat16_rn(v);
     }
     for (int i = tid; i < DM * 64; i += NTH) {
@@ -239,7 +242,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         float v = 0.f;
         // each gate half padded to 16 columns, so that the two up-projections are separate K = 16 slices
         if (c < 16) { if (c < r && n < DK) v = __ldg(a.Vb + (size_t)n * r + c); }
-        else if (c < 32) { if (c - 16 < r && n < DV) v = __ldg(a.Vw + (size_t)(vofs + n) * r + (c - 16)); }
+        else if (c < 32) { if (c - 16 < r && n < DV && !SW) v = __ldg(a.Vw + (size_t)(vofs + n) * r + (c - 16)); }
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Vcat + tile_off(DM, n, c)) = __float2bfloat16_rn(v);
     }
     for (int j = tid; j < 4 * 128; j += NTH) mi.etot[j >> 7][j & 127] = 1.f;
@@ -304,10 +307,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
     };
     auto issue_wv = [&](int c) {
-        mbar_expect_tx(&mi.bar_wv, 2u * LCc * DV * 2u);
+        mbar_expect_tx(&mi.bar_wv, (SW ? 1u : 2u) * LCc * DV * 2u);
         const int tr = b * a.T + c * LCc;
         for (int cb = 0; cb < DV / 64; ++cb) {
-            tma_load_3d(sm + Lo.WX + cb * 64 * 128, &mwx, &mi.bar_wv, vofs + cb * 64, h, tr);
+            if (!SW) tma_load_3d(sm + Lo.WX + cb * 64 * 128, &mwx, &mi.bar_wv, vofs + cb * 64, h, tr);
             tma_load_3d(sm + Lo.V + cb * 64 * 128, &mv, &mi.bar_wv, vofs + cb * 64, h, tr);
         }
     };
@@ -464,7 +467,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         if (warp == 0) {
             if (elect_one()) {
                 umma_prod<KMAJ, KMAJ, 16>(tmem + TM_X1, 128, DK, sb + Lo.Y1, 128, 0, 0, sb + Lo.Vcat, DM, 0, 0, 16, false);
-                umma_prod<KMAJ, KMAJ, 16>(tmem + TM_X2, 128, DV, sb + Lo.Y1, 128, 0, 16, sb + Lo.Vcat, DM, 0, 16, 16, false);
+                if (!SW) umma_prod<KMAJ, KMAJ, 16>(tmem + TM_X2, 128, DV, sb + Lo.Y1, 128, 0, 16, sb + Lo.Vcat, DM, 0, 16, 16, false);
                 umma_commit(&mi.bar_mma);
             }
             __syncwarp();
@@ -486,13 +489,13 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             const int blk = t >> 4;
             uint32_t pr16[16], pw16[16];
             tmem_ld16(tmem + TM_X1 + lane_base + 8 * cc0, pr16);
-            tmem_ld16(tmem + TM_X2 + lane_base + 8 * cc0, pw16);
+            if (!SW) tmem_ld16(tmem + TM_X2 + lane_base + 8 * cc0, pw16);
             tmem_wait_ld();
 #pragma unroll
             for (int ci = 0; ci < 2; ++ci) {
                 const int cc = cc0 + ci;
                 const uint32_t off = tile_chunk_off(64, t, cc);
-                if (live) {
+                if (live && !SW) {
                     float fw[8], fv[8];
                     unpack8(lds128(sm + Lo.WX + off), fw);
                     unpack8(lds128(sm + Lo.V + off), fv);
@@ -969,7 +972,7 @@ bool tc_fwd_supported(const carve_params_t& p)
 size_t tc_state_tile_bytes(const carve_params_t& p) { return tc::tile_bytes(p.dv, p.dk); }
 size_t tc_record_bytes(const carve_params_t& p) { return tcp::Rec(p.dk, p.dv).total; }
 
-template <int D, int VS>
+template <int D, int VS, int SW>
 static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
 {
     const int LCc = a.L < tcp::LC ? a.L : tcp::LC;
@@ -977,17 +980,18 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
     if (!tc_make_token_map(&mo, a.O, a.B, a.T, a.H, a.dv, LCc)) return cudaErrorInvalidValue;
     if (!tc_make_token_map(&mq, a.q, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mk, a.k, a.B, a.T, a.H, D, LCc) ||
         !tc_make_token_map(&mv, a.v, a.B, a.T, a.H, a.dv, LCc) || !tc_make_token_map(&mf, a.f, a.B, a.T, a.H, D, LCc) ||
-        !tc_make_token_map(&mbx, a.bx, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mwx, a.wx, a.B, a.T, a.H, a.dv, LCc))
+        !tc_make_token_map(&mbx, a.bx, a.B, a.T, a.H, D, LCc) ||
+        !tc_make_token_map(&mwx, a.wx ? a.wx : a.v, a.B, a.T, a.H, a.dv, LCc))   // (scalar-write variant: the map is never used)
         return cudaErrorInvalidValue;
     TcArgs t{};
     t.B = a.B; t.H = a.H; t.T = a.T; t.L = a.L; t.r = a.r; t.l2norm = a.l2norm; t.scale = a.scale; t.eps = a.eps;
-    t.dvf = a.dv;
+    t.dvf = a.dv; t.sw = a.wx == nullptr;
     t.beta = static_cast<const __nv_bfloat16*>(a.beta);
     t.A = a.A; t.tau = a.tau; t.Ub = a.Ub; t.Uw = a.Uw; t.Vb = a.Vb; t.Vw = a.Vw; t.S0 = a.S0;
     t.O = static_cast<__nv_bfloat16*>(a.O); t.S_final = a.S_final; t.rec = rec;
     const size_t smem = tcp::Layout(D, D, 2 * a.r).total;
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
-    auto kern = carve_fwd_tc_kernel<D, D, NP, VS>;
+    auto kern = carve_fwd_tc_kernel<D, D, NP, VS, SW>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
@@ -1005,9 +1009,10 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
 
 cudaError_t tc_fwd_launch(const Args& a, uint8_t* rec, cudaStream_t st)
 {
-    if (a.dk == 128 && a.dv == 256) return launch_tc_fwd<128, 2>(a, rec, st);   // inference only: two CTAs per chain
-    if (a.dk == 128) return launch_tc_fwd<128, 1>(a, rec, st);
-    if (a.dk == 64) return launch_tc_fwd<64, 1>(a, rec, st);
+    const bool sw = a.wx == nullptr;
+    if (a.dk == 128 && a.dv == 256) return sw ? cudaErrorInvalidValue : launch_tc_fwd<128, 2, 0>(a, rec, st);   // inference only: two CTAs per chain
+    if (a.dk == 128) return sw ? launch_tc_fwd<128, 1, 1>(a, rec, st) : launch_tc_fwd<128, 1, 0>(a, rec, st);
+    if (a.dk == 64) return sw ? launch_tc_fwd<64, 1, 1>(a, rec, st) : launch_tc_fwd<64, 1, 0>(a, rec, st);
     return cudaErrorInvalidValue;
 }
 
