@@ -179,6 +179,54 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_step(args):
+    """`--op step`: the recurrent decode call carve_step, one new token per sequence and call.
+    Not the BASELINE.json metric: decode tokens/s (B sequences x 1 token per step) and the fraction of the HBM roofline
+    of a decode step, whose algorithmic traffic is the state's round trip, 2 x 4 dv dk bytes per (batch, head) chain."""
+    import torch
+    from paper_2606_27229_b200 import carve
+    torch.cuda.set_device(0)
+    base = get_cfg(args.config)
+    cfg = base.with_(B=args.decode_batch, T=1, L=16, s0_std=0.1)
+    x = synth.make_inputs(cfg)
+    tok_dt = torch.bfloat16 if cfg.dtype == "bf16" else torch.float32
+    xd = {}
+    for n, a in x.items():
+        if a is None:
+            xd[n] = None
+            continue
+        t = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32))
+        xd[n] = (t.to(tok_dt) if n in synth.TOKEN_TENSORS else t).cuda()
+    p = carve.Params(B=cfg.B, H=cfg.H, T=1, L=16, dk=cfg.dk, dv=cfg.dv, r=cfg.r,
+                     dtype=carve.CARVE_BF16 if cfg.dtype == "bf16" else carve.CARVE_F32)
+    # several state buffers in rotation, together larger than the 126 MB L2
+    nbuf = max(2, int(200e6 // (cfg.B * cfg.H * cfg.dv * cfg.dk * 4)) + 1)
+    S = [xd["S0"].clone() for _ in range(nbuf)]
+    O = torch.empty(cfg.B, 1, cfg.H, cfg.dv, dtype=tok_dt, device="cuda")
+    st = torch.cuda.current_stream()
+    for i in range(max(args.warmup, 3)):
+        carve.carve_step(p, xd, S[i % nbuf], O, st.cuda_stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(st)
+    for i in range(args.steps):
+        carve.carve_step(p, xd, S[i % nbuf], O, st.cuda_stream)
+    e1.record(st)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    peaks = load_peaks()
+    bytes_alg = cfg.B * cfg.H * cfg.dv * cfg.dk * 4 * 2
+    ach = bytes_alg / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "CARVE decode step (carve_step) tokens/sec", "unit": "tokens/s", "n_gpus": 1, "steps": args.steps,
+                      "warmup": args.warmup, "higher_is_better": True, "value": cfg.B / (ms * 1e-3), "ms_per_step": ms,
+                      "dtype": "bf16 tokens, f32 state/arithmetic", "data": "synthetic",
+                      "config": {"workload": f"decode: B={cfg.B} sequences x 1 new token, H={cfg.H}, dk={cfg.dk}, dv={cfg.dv}, r={cfg.r}; "
+                                             f"{nbuf} state buffers in rotation (> L2)"},
+                      "gpu_launches": args.steps,
+                      "roofline": {"bound": "hbm", "kernel": "carve_step_kernel", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                   "frac": ach / peaks["hbm_gbs"], "traffic": None, "algorithmic_bytes_per_launch": bytes_alg}}), flush=True)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -388,6 +436,8 @@ def main():
     ap.add_argument("--config", default="cfg1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fwd-only", action="store_true", help="time carve_fwd alone (inference call, nothing saved)")
+    ap.add_argument("--op", default="train", choices=["train", "step"], help="step: time the decode call carve_step instead")
+    ap.add_argument("--decode-batch", type=int, default=256)
     ap.add_argument("--scalar-write", action="store_true",
                     help="the scalar-write variant (wx = Uw = Vw = NULL, PAPER.md section 4.2): not the BASELINE.json metric's workload")
     args = ap.parse_args()
@@ -406,7 +456,9 @@ def main():
         cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
                "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
         raise SystemExit(subprocess.call(cmd, env=env))
-    if args.impl == "reference":
+    if args.op == "step":
+        run_step(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
