@@ -135,7 +135,7 @@ __device__ __forceinline__ void mma_k(uint32_t d_tmem, int N, uint32_t a_saddr, 
     umma_prod<AMAJ, BMAJ, KMAX>(d_tmem, 128, N, a_saddr, a_rows, a_o0, a_k0, b_saddr, b_rows, b_o0, b_k0, K, accumulate);
 }
 // The MMA / bulk-copy issuing thread: the elected lane of warp 0, inside a warp-uniform branch (tc_common.cuh umma_prod).
-#define LEADER_BEGIN if (warp == 0) { if (elect_one()) {
+#define LEADER_BEGIN if (warp == LEADER_WARP) { if (elect_one()) {
 #define LEADER_END } __syncwarp(); }
 
 // Column sums over the 32 lanes of a warp by a halving butterfly: on return lane l holds in v[0..N/32)
@@ -181,6 +181,7 @@ __global__ void __launch_bounds__(128 * NP, 1)
 carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, const __grid_constant__ CUtensorMap mq)
 {
     constexpr int NTH = 128 * NP;
+    constexpr int LEADER_WARP = NTH / 32 - 1;   // MMA issuer: the last warp (see L1)
     constexpr int HK = D / NP;                     // columns per warpgroup ("half" = part index 0..NP-1)
     constexpr uint32_t TB = tile_bytes(64, D);     // one [64][D] tile
     constexpr uint32_t SBb = tile_bytes(D, D);     // one state tile
@@ -356,7 +357,9 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             }
         }
         // ---- L1: dU = Ktil dS'^T + (scale P)^T dO -> BM_A rows 0..63;  dKtil = U dS' -> BM_KT rows 0..63
-        LEADER_BEGIN
+        //      (issued by the last warp, a Q-side one: only the K-side warps have work behind this product, and the issuing
+        //      lane stays blocked for as long as the 20 instructions take to execute)
+        if (warp == NTH / 32 - 1) { if (elect_one()) {
             mbar_wait(&mi.bar_g1, ph);
             mbar_wait(&mi.bar_pt, ph);
             tc_fence_after();

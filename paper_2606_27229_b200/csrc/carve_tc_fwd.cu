@@ -338,7 +338,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             bulk_s2g(rc + Rc.SB, sb + Lo.Sb, (uint32_t)state_tile);
             bulk_commit();
         }
-        if (fold_now && warp == 0) {
+        if (fold_now && warp == NTH / 32 - 1) {   // (warps 0..3 have P1 behind this product)
             if (elect_one()) {
                 mma_rt<128, MNMAJ, KMAJ, DV>(tmem + TM_X2, R2, sb + Lo.Sb, DV, 0, sb + Lo.Ucat, R2, 0, DV, false);
                 umma_commit(&mi.bar_mma);
@@ -676,7 +676,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         // ---- P8: A|P blocks (one 16-column block per anchoring) and the state products
         PHASE_SYNC();
         PROF(g_prof_fwd, 18);
-        if (warp == 0) {
+        // Issued by the last warp (Q side of the last column part): it has nothing to do in P9a / P9b, and the issuing
+        // lane stays blocked for as long as these 40 instructions take to execute (the MMA queue is a few entries deep).
+        if (warp == NTH / 32 - 1) {
             if (elect_one()) {
                 const int nb = LCc >> 4;
                 mma_rt<128, KMAJ, KMAJ, DK>(tmem + TM_X2, 16, sb + Lo.KQbar, 128, 0, sb + Lo.Y1, 64, 0, DK, false);
