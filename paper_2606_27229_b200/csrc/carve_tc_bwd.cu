@@ -34,6 +34,7 @@ namespace {
 
 using namespace tcp;
 PROF_DECL(g_prof_bwd)
+PROFB_DECL(g_profb_bwd)
 
 struct BwdArgs {
     int B, H, T, L, r;
@@ -393,7 +394,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         }
         PROF(g_prof_bwd, 1);
         // ---- L2: dX = T^T dU: columns x < D/2 -> BM_A rows 0..63 (K-side lanes), x >= D/2 -> rows 64..127 (Q-side lanes)
-        PHASE_SYNC();
+        PROFB_ARRIVE(0); PHASE_SYNC(); PROFB_AFTER(g_profb_bwd, 0);
         PROF(g_prof_bwd, 14);
         LEADER_BEGIN
             mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_A + D / 2, D / 2, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[0], 64, D / 2, 0, LCc, false);
@@ -441,7 +442,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         }
         PROF(g_prof_bwd, 2);
         // ---- L3: [dA;dP] raw, SP = [-dR;dO] S, dS += [-dR;dO]^T [Kbar; scale Qbar]
-        PHASE_SYNC();
+        PROFB_ARRIVE(1); PHASE_SYNC(); PROFB_AFTER(g_profb_bwd, 1);
         PROF(g_prof_bwd, 16);
         LEADER_BEGIN
             mbar_wait(&mi.bar_sb, ph);
@@ -510,7 +511,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         //      with G = product of the whole-block decays between the two blocks, applied by Horner steps.  Every pair
         //      (t,s) enters +Kbar_own_t C_s dA_ts G in row t and -C_s Kbar_own_t dA_ts G in row s with bit-identical
         //      operands, so the pairs that do not straddle a token cancel to fp32 rounding in the reverse cumulative sum.
-        __syncthreads();
+        PROFB_ARRIVE(2); __syncthreads(); PROFB_AFTER(g_profb_bwd, 2);
         PROF(g_prof_bwd, 18);
         if (tid == 0) {   // dS' (DSB) is consumed: stage gamma_t/gamma_a and its inverse there for L5
             mbar_expect_tx(&mi.bar_fi, 2 * TB);
@@ -668,7 +669,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         carry += tot;
                     }
                 }
-            __syncthreads();  // every warp is done reading DAP / C / KQo
+            PROFB_ARRIVE(3); __syncthreads(); PROFB_AFTER(g_profb_bwd, 3);  // every warp is done reading DAP / C / KQo
             PROF(g_prof_bwd, 21);
 #pragma unroll
             for (int side = 0; side < 2; ++side)       // H raw -> S[2..3] ([128][D] tile, over KQo): for dk^, dq^
@@ -700,7 +701,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         }
         PROF(g_prof_bwd, 5);
         // ---- L5: assemble dk^, dq^ (state part) and the state-read / state-write contributions to d log gamma
-        __syncthreads();
+        PROFB_ARRIVE(4); __syncthreads(); PROFB_AFTER(g_profb_bwd, 4);
         mbar_wait(&mi.bar_fi, ph);
         PROF(g_prof_bwd, 22);
         if (warp_active) {
@@ -780,7 +781,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         // ---- L6: d log a_t = dlp_t + carry + sum_{t' > t} XA_t' + sum_{t' >= t} XQ_t' + sum_{t' < t} Z_t' -> BM_KT:
         //      key channels j < D/2 in rows 0..63 (K-side lanes), j >= D/2 in rows 64..127 (Q-side lanes: the 0/1 tile
         //      used as the upper half of the M = 128 operand), so both threads of a token share the epilogue
-        PHASE_SYNC();
+        PROFB_ARRIVE(5); PHASE_SYNC(); PROFB_AFTER(g_profb_bwd, 5);
         PROF(g_prof_bwd, 23);
         LEADER_BEGIN
             const uint32_t tri = sb + Lo.TRI, trh = tri - 8192;
@@ -856,7 +857,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         }
         PROF(g_prof_bwd, 7);
         // ---- L7: ZZ = [db_pre; dw_pre] [Vb | Vw] -> BM_DAP;  dVb | dVw += [db_pre; dw_pre]^T TT2 -> BM_WG
-        PHASE_SYNC();
+        PROFB_ARRIVE(6); PHASE_SYNC(); PROFB_AFTER(g_profb_bwd, 6);
         PROF(g_prof_bwd, 26);
         LEADER_BEGIN
             mma_k<KMAJ, KMAJ, D>(tmem + BM_DAP, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.VcT, 32, 0, 0, D, false);
@@ -905,7 +906,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         }
         PROF(g_prof_bwd, 8);
         // ---- L8: dq^ += dz G -> BM_A rows 64..127;  dG^T = q^T (dz/|q|) -> BM_DAP + 32
-        PHASE_SYNC();
+        PROFB_ARRIVE(7); PHASE_SYNC(); PROFB_AFTER(g_profb_bwd, 7);
         PROF(g_prof_bwd, 28);
         LEADER_BEGIN
             mbar_wait(&mi.bar_g8, ph);
@@ -969,7 +970,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROF(g_prof_bwd, 9);
         // ---- L9: fold glue: dS += [Ub;Uw]^T dG;  d[Ub;Uw]^T += S dG^T -> BM_WU
         if (gate_start) {
-            PHASE_SYNC();
+            PROFB_ARRIVE(8); PHASE_SYNC(); PROFB_AFTER(g_profb_bwd, 8);
             PROF(g_prof_bwd, 30);
             LEADER_BEGIN
                 mma_k<MNMAJ, KMAJ, 32>(tmem + BM_DS, D, sb + Lo.Ucat, 32, 0, 0, sb + Lo.S[1], D, 0, 0, R2, true);
@@ -1193,6 +1194,12 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
 }  // namespace
 
 #ifdef CARVE_PROFILE
+extern "C" void carve_debug_profb_bwd(unsigned long long* out)
+{
+    cudaMemcpyFromSymbol(out, g_profb_bwd, sizeof(g_profb_bwd));
+    static unsigned long long z[64 * 16];
+    cudaMemcpyToSymbol(g_profb_bwd, z, sizeof(z));
+}
 extern "C" void carve_debug_prof_bwd(unsigned long long* out)
 {
     cudaMemcpyFromSymbol(out, g_prof_bwd, sizeof(g_prof_bwd));

@@ -27,6 +27,7 @@ namespace {
 
 using namespace tcp;
 PROF_DECL(g_prof_fwd)
+PROFB_DECL(g_profb_fwd)
 
 struct TcArgs {
     int B, H, T, L, r;
@@ -320,7 +321,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     uint32_t mma_ph = 0, tma_ph = 0, acc_ph = 0;
     // write strength of this thread's token, fetched one chunk ahead (a plain global load: its latency must not sit
     // on the chunk's serial path)
-    float beta_nx = (krole && half == 0 && live) ? __bfloat162float(a.beta[((size_t)b * a.T + t) * a.H + h]) : 0.f;
+    // (kept as raw bf16 bits until it is used, one chunk later: converting it here would make the warp wait for the load)
+    const unsigned short* beta_bits = reinterpret_cast<const unsigned short*>(a.beta);
+    uint32_t beta_nx = (krole && half == 0 && live) ? (uint32_t)__ldg(beta_bits + ((size_t)b * a.T + t) * a.H + h) : 0u;
     PROF_INIT();
     for (int c = 0; c < nchunks; ++c) {
         const bool fold_now = (c % gate_every) == 0;
@@ -328,7 +331,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         uint8_t* rc = rec_chain ? rec_chain + (size_t)c * Rc.total : nullptr;  // this chunk's record
         PROF(g_prof_fwd, 0);
         // ---- P0: fold G^T = S^T Ucat^T -> TM_X2[0, R2)
-        PHASE_SYNC();
+        PROFB_ARRIVE(0); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 0);
         if (tid == 0 && c > 0) {   // the previous chunk's outputs (staged in Y2 by P13)
             for (int cb = 0; cb < DV / 64; ++cb) tma_store_3d(&mo, sb + Lo.Y2 + cb * 8192, vofs + cb * 64, h, b * a.T + (c - 1) * LCc);
             bulk_commit();
@@ -361,8 +364,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             mi.nrm[row][half] = ss;
             if (krole && half == 0) {
                 // clamped away from 0 so that e_t = u_t / beta_t exists (u_t changes by < 1e-30 |e_t|)
-                const float bt = fmaxf(beta_nx, 1e-30f);
-                if (c + 1 < nchunks) beta_nx = __bfloat162float(a.beta[(tok0 + LCc + t) * a.H + h]);
+                const float bt = fmaxf(__uint_as_float(beta_nx << 16), 1e-30f);
+                if (c + 1 < nchunks) beta_nx = (uint32_t)__ldg(beta_bits + (tok0 + LCc + t) * a.H + h);
                 sBeta[t] = bt;
                 if (rc) reinterpret_cast<float*>(rc + Rc.beta)[t] = bt;
             }
@@ -423,7 +426,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         PROF(g_prof_fwd, 2);
         // ---- P2: Z = [k;q] G^T -> TM_X2[32, 32+R2)
-        PHASE_SYNC();
+        PROFB_ARRIVE(1); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 1);
         if (warp == 0) {
             if (elect_one()) {
                 mma_rt<128, KMAJ, MNMAJ, DK>(tmem + TM_X2 + 32, R2, sb + Lo.KQraw, 128, 0, sb + Lo.Vcat, DM, 32, DK, false);
@@ -463,7 +466,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         PROF(g_prof_fwd, 4);
         // ---- P4: b_proj = [tt_b;tt_b] Vb^T -> TM_X1, w_proj = [tt_w;tt_w] Vw^T -> TM_X2 (both row halves get both)
-        PHASE_SYNC();
+        PROFB_ARRIVE(2); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 2);
         if (warp == 0) {
             if (elect_one()) {
                 umma_prod<KMAJ, KMAJ, 16>(tmem + TM_X1, 128, DK, sb + Lo.Y1, 128, 0, 0, sb + Lo.Vcat, DM, 0, 0, 16, false);
@@ -560,7 +563,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         PROF(g_prof_fwd, 6);
         if (tid == 0) bulk_wait_read();   // the output tile has left Y2 (rewritten below)
-        __syncthreads();
+        PROFB_ARRIVE(3); __syncthreads(); PROFB_AFTER(g_profb_fwd, 3);
         PROF(g_prof_fwd, 8);
         // ---- P7b: decayed operands.  Row operands exist in up to four anchorings: version 0 relative to the chunk
         //      start (Kbar, Qbar: also the operand of the state products), version jb relative to the start of
@@ -674,7 +677,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         if (rc && tid == REC_TID) bulk_wait_read();   // the previous chunk's [P;T] copy has left TP (rewritten in P9)
         PROF(g_prof_fwd, 9);
         // ---- P8: A|P blocks (one 16-column block per anchoring) and the state products
-        PHASE_SYNC();
+        PROFB_ARRIVE(4); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 4);
         PROF(g_prof_fwd, 18);
         // Issued by the last warp (Q side of the last column part): it has nothing to do in P9a / P9b, and the issuing
         // lane stays blocked for as long as these 40 instructions take to execute (the MMA queue is a few entries deep).
@@ -820,18 +823,18 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
-        __syncthreads();
+        PROFB_ARRIVE(5); __syncthreads(); PROFB_AFTER(g_profb_fwd, 5);
         PROF(g_prof_fwd, 12);
         // ---- P9c: WY solve U = (I + beta A)^-1 (beta R) in registers (tf32 mma.sync) -> bf16 rows over V'; T -> TP rows 0..63
         diag8_inverse(Mm, Tm, LCc, tid);
-        __syncthreads();
+        PROFB_ARRIVE(6); __syncthreads(); PROFB_AFTER(g_profb_fwd, 6);
         PROF(g_prof_fwd, 26);
         wy_solve<DV>(Mm, Tm, LCc, warp, lane, sb + Lo.Y2, sb + Lo.Us, sb + Lo.TP);
         // the record copies issued so far have left their buffers: the next chunk's loads (P13) may overwrite them
         if (rc && tid == REC_TID) bulk_wait_read();
         PROF(g_prof_fwd, 13);
         // ---- P12: O += P U;  W = U^T Ktil -> TM_X2
-        PHASE_SYNC();
+        PROFB_ARRIVE(7); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 7);
         PROF(g_prof_fwd, 22);
         if (warp == 0) {
             if (elect_one()) {
@@ -956,6 +959,12 @@ bool tc_make_token_map(CUtensorMap* map, const void* base, int B, int T, int H, 
 }
 
 #ifdef CARVE_PROFILE
+extern "C" void carve_debug_profb_fwd(unsigned long long* out)
+{
+    cudaMemcpyFromSymbol(out, g_profb_fwd, sizeof(g_profb_fwd));
+    static unsigned long long z[64 * 16];
+    cudaMemcpyToSymbol(g_profb_fwd, z, sizeof(z));
+}
 extern "C" void carve_debug_prof_fwd(unsigned long long* out)
 {
     cudaMemcpyFromSymbol(out, g_prof_fwd, sizeof(g_prof_fwd));

@@ -23,6 +23,7 @@
 // trip at every point) and are added to the global array once, by PROF_FLUSH at the kernel's end
 #define PROF_INIT()                                            \
     __shared__ unsigned long long prof_s_[80];                 \
+    __shared__ long long prof_arr_[2][16];                     \
     if (threadIdx.x < 80) prof_s_[threadIdx.x] = 0;            \
     __syncthreads();                                           \
     long long prof_t_ = clock64();
@@ -32,6 +33,15 @@
         prof_s_[(threadIdx.x ? 40 : 0) + i] += (unsigned long long)(prof_n_ - prof_t_); \
         prof_t_ = prof_n_;                                                         \
     }
+// barrier-spread profile: per barrier site and warp, how long the warp waited for the last one to arrive
+#define PROFB_DECL(name) static __device__ unsigned long long name[64 * 16];
+#define PROFB_ARRIVE(site) if ((threadIdx.x & 31) == 0) prof_arr_[(site) & 1][threadIdx.x >> 5] = clock64();
+#define PROFB_AFTER(name, site)                                                                     \
+    if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) {                                               \
+        long long mx_ = 0;                                                                          \
+        for (int w_ = 0; w_ < (int)(blockDim.x >> 5); ++w_) mx_ = mx_ > prof_arr_[(site) & 1][w_] ? mx_ : prof_arr_[(site) & 1][w_]; \
+        atomicAdd(&name[(site) * 16 + (threadIdx.x >> 5)], (unsigned long long)(mx_ - prof_arr_[(site) & 1][threadIdx.x >> 5])); \
+    }
 #define PROF_FLUSH(name)                                                           \
     __syncthreads();                                                               \
     if (blockIdx.x == 0 && threadIdx.x < 80) name[threadIdx.x] += prof_s_[threadIdx.x];
@@ -40,6 +50,9 @@
 #define PROF_INIT()
 #define PROF(name, i)
 #define PROF_FLUSH(name)
+#define PROFB_DECL(name)
+#define PROFB_ARRIVE(site)
+#define PROFB_AFTER(name, site)
 #endif
 
 namespace carve {
