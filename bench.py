@@ -356,9 +356,11 @@ def run_ours(args):
     d2h = nb(Oh) + nb(Sfh) + (sum(nb(t) for t in gh.values()) if with_bwd else 0)
     e2e_steps = 0 if args.scalar_write else max(1, min(args.steps, 5))   # the host entry point takes the full write gate only
 
+    hctx = carve.carve_host_ctx_create()     # the call's side streams and events, created once
+
     def e2e_step():
         carve.carve_fwd_bwd_host(p, with_bwd, xh, Oh, Sfh, dOh if with_bwd else None, dSfh if with_bwd else None,
-                                 gh, arena, stream.cuda_stream)
+                                 gh, arena, stream.cuda_stream, ctx=hctx)
     if e2e_steps:
         e2e_step()
     barrier()

@@ -165,6 +165,23 @@ carve_status_t carve_fwd_bwd_host(const carve_params_t *p, int with_bwd, const v
                                   float *dVb, float *dVw, float *dS0, void *device_arena,
                                   size_t arena_bytes, void *cuda_stream);
 
+/*
+ * The same call with caller-owned side streams and events: carve_fwd_bwd_host creates and destroys up to 8 streams and
+ * 17 events per call; a context created once (carve_host_ctx_create) and passed to carve_fwd_bwd_host_ctx removes that
+ * from every step.  One context serves one call at a time.  ctx = NULL behaves as carve_fwd_bwd_host.
+ */
+typedef struct carve_host_ctx carve_host_ctx_t;
+carve_status_t carve_host_ctx_create(carve_host_ctx_t **ctx);
+void carve_host_ctx_destroy(carve_host_ctx_t *ctx);
+carve_status_t carve_fwd_bwd_host_ctx(carve_host_ctx_t *ctx, const carve_params_t *p, int with_bwd, const void *q,
+                                      const void *k, const void *v, const void *f, const void *bx, const void *wx,
+                                      const void *beta, const float *A, const float *tau, const float *Ub,
+                                      const float *Uw, const float *Vb, const float *Vw, const float *S0, void *O,
+                                      float *S_final, const void *dO, const float *dS_final, void *dq, void *dk,
+                                      void *dv, void *df, void *dbx, void *dwx, void *dbeta, float *dA, float *dtau,
+                                      float *dUb, float *dUw, float *dVb, float *dVw, float *dS0, void *device_arena,
+                                      size_t arena_bytes, void *cuda_stream);
+
 /* Number of kernel launches carve_fwd / carve_bwd enqueue for these parameters (for accounting). */
 int carve_num_launches(const carve_params_t *p, int bwd);
 

@@ -20,6 +20,7 @@ CARVE_PATH_AUTO, CARVE_PATH_SIMT, CARVE_PATH_TENSOR = 0, 1, 2
 
 # Every symbol include/carve.h declares (tests check the library exports them all).
 SYMBOLS = ("carve_workspace_bytes", "carve_fwd", "carve_bwd", "carve_step", "carve_host_arena_bytes", "carve_fwd_bwd_host",
+           "carve_host_ctx_create", "carve_host_ctx_destroy", "carve_fwd_bwd_host_ctx",
            "carve_num_launches", "carve_resolved_path", "carve_status_string", "carve_version")
 
 
@@ -89,6 +90,12 @@ def load_library() -> ctypes.CDLL:
         lib.carve_bwd.argtypes = [pp] + [vp] * 30 + [vp, sz, vp]
         lib.carve_fwd_bwd_host.restype = ci
         lib.carve_fwd_bwd_host.argtypes = [pp, ci] + [vp] * 32 + [vp, sz, vp]
+        lib.carve_fwd_bwd_host_ctx.restype = ci
+        lib.carve_fwd_bwd_host_ctx.argtypes = [vp, pp, ci] + [vp] * 32 + [vp, sz, vp]
+        lib.carve_host_ctx_create.restype = ci
+        lib.carve_host_ctx_create.argtypes = [ctypes.POINTER(vp)]
+        lib.carve_host_ctx_destroy.restype = None
+        lib.carve_host_ctx_destroy.argtypes = [vp]
         _lib = lib
     return _lib
 
@@ -164,12 +171,26 @@ def carve_bwd(p: Params, x: dict, dO, dS_final, grads: dict, workspace, stream: 
                                     ctypes.c_void_p(stream)))
 
 
+def carve_host_ctx_create() -> ctypes.c_void_p:
+    """carve_host_ctx_create of carve.h: the side streams and events of the host entry point, owned by the caller."""
+    h = ctypes.c_void_p()
+    _check(load_library().carve_host_ctx_create(ctypes.byref(h)))
+    return h
+
+
+def carve_host_ctx_destroy(ctx) -> None:
+    load_library().carve_host_ctx_destroy(ctx)
+
+
 def carve_fwd_bwd_host(p: Params, with_bwd: bool, x: dict, O, S_final, dO, dS_final, grads: dict, arena,
-                       stream: int = 0) -> None:
-    """carve_fwd_bwd_host of carve.h: all tensors are HOST (pinned) tensors, `arena` is a device byte
-    tensor of carve_host_arena_bytes(p, with_bwd) bytes."""
+                       stream: int = 0, ctx=None) -> None:
+    """carve_fwd_bwd_host (ctx None) / carve_fwd_bwd_host_ctx of carve.h: all tensors are HOST (pinned) tensors, `arena`
+    is a device byte tensor of carve_host_arena_bytes(p, with_bwd) bytes."""
     cp = p.c()
     g = grads or {}
-    _check(load_library().carve_fwd_bwd_host(
-        ctypes.byref(cp), int(with_bwd), *[_ptr(x.get(n)) for n in _FWD_IN], _ptr(O), _ptr(S_final), _ptr(dO),
-        _ptr(dS_final), *[_ptr(g.get(n)) for n in _GRADS], _ptr(arena), _nbytes(arena), ctypes.c_void_p(stream)))
+    args = [ctypes.byref(cp), int(with_bwd), *[_ptr(x.get(n)) for n in _FWD_IN], _ptr(O), _ptr(S_final), _ptr(dO),
+            _ptr(dS_final), *[_ptr(g.get(n)) for n in _GRADS], _ptr(arena), _nbytes(arena), ctypes.c_void_p(stream)]
+    if ctx is None:
+        _check(load_library().carve_fwd_bwd_host(*args))
+    else:
+        _check(load_library().carve_fwd_bwd_host_ctx(ctx, *args))

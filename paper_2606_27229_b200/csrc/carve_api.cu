@@ -2,6 +2,7 @@
 // kernel-family selection and the host-buffer entry point.  No arithmetic of the method here.
 #include <cstdio>
 #include <cstring>
+#include <new>
 
 #include "carve_internal.h"
 
@@ -315,7 +316,12 @@ size_t carve_host_arena_bytes(const carve_params_t* p, int with_bwd)
     return n + per * ns;
 }
 
-carve_status_t carve_fwd_bwd_host(const carve_params_t* p, int with_bwd, const void* q, const void* k,
+struct carve_host_ctx {
+    cudaStream_t side[8];
+    cudaEvent_t fork, join[8], arrived[8];
+};
+
+static carve_status_t host_impl(carve_host_ctx* ctx, const carve_params_t* p, int with_bwd, const void* q, const void* k,
                                   const void* v, const void* f, const void* bx, const void* wx, const void* beta,
                                   const float* A, const float* tau, const float* Ub, const float* Uw,
                                   const float* Vb, const float* Vw, const float* S0, void* O, float* S_final,
@@ -363,13 +369,20 @@ carve_status_t carve_fwd_bwd_host(const carve_params_t* p, int with_bwd, const v
 
     cudaStream_t side[8] = {};
     cudaEvent_t fork = nullptr, join[8] = {}, arrived[8] = {};  // arrived[i]: slice i's host -> device copies done
-    ok = ok && cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) == cudaSuccess;
+    if (ctx) {   // caller-owned streams and events (carve_host_ctx_create): nothing is created or destroyed per call
+        fork = ctx->fork;
+        for (int i = 0; i < 8; ++i) { side[i] = ctx->side[i]; join[i] = ctx->join[i]; arrived[i] = ctx->arrived[i]; }
+    } else {
+        ok = ok && cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) == cudaSuccess;
+    }
     ok = ok && cudaEventRecord(fork, st) == cudaSuccess;
     for (int i = 0; i < ns && ok; ++i) {
         if (ns > 1) {
-            ok = ok && cudaStreamCreateWithFlags(&side[i], cudaStreamNonBlocking) == cudaSuccess;
-            ok = ok && cudaEventCreateWithFlags(&join[i], cudaEventDisableTiming) == cudaSuccess;
-            ok = ok && cudaEventCreateWithFlags(&arrived[i], cudaEventDisableTiming) == cudaSuccess;
+            if (!ctx) {
+                ok = ok && cudaStreamCreateWithFlags(&side[i], cudaStreamNonBlocking) == cudaSuccess;
+                ok = ok && cudaEventCreateWithFlags(&join[i], cudaEventDisableTiming) == cudaSuccess;
+                ok = ok && cudaEventCreateWithFlags(&arrived[i], cudaEventDisableTiming) == cudaSuccess;
+            }
             ok = ok && cudaStreamWaitEvent(side[i], fork, 0) == cudaSuccess;
         } else {
             side[i] = st;
@@ -444,15 +457,70 @@ carve_status_t carve_fwd_bwd_host(const carve_params_t* p, int with_bwd, const v
         down(dVb, w, h.w_vb, st); w += (size_t)p->dk * p->r;
         down(dVw, w, h.w_vw, st);
     }
-    // streams and events are released by the runtime once the work enqueued on them has completed
-    for (int i = 0; i < ns; ++i) {
-        if (ns > 1 && side[i]) cudaStreamDestroy(side[i]);
-        if (join[i]) cudaEventDestroy(join[i]);
-        if (arrived[i]) cudaEventDestroy(arrived[i]);
+    // (without a context) streams and events are released by the runtime once the work enqueued on them has completed
+    if (!ctx) {
+        for (int i = 0; i < ns; ++i) {
+            if (ns > 1 && side[i]) cudaStreamDestroy(side[i]);
+            if (join[i]) cudaEventDestroy(join[i]);
+            if (arrived[i]) cudaEventDestroy(arrived[i]);
+        }
+        if (fork) cudaEventDestroy(fork);
     }
-    if (fork) cudaEventDestroy(fork);
     if (rs != CARVE_OK) return rs;
     return ok ? CARVE_OK : CARVE_ERR_CUDA;
+}
+
+carve_status_t carve_fwd_bwd_host(const carve_params_t* p, int with_bwd, const void* q, const void* k,
+                                  const void* v, const void* f, const void* bx, const void* wx, const void* beta,
+                                  const float* A, const float* tau, const float* Ub, const float* Uw,
+                                  const float* Vb, const float* Vw, const float* S0, void* O, float* S_final,
+                                  const void* dO, const float* dS_final, void* dq, void* dk, void* dv, void* df,
+                                  void* dbx, void* dwx, void* dbeta, float* dA, float* dtau, float* dUb,
+                                  float* dUw, float* dVb, float* dVw, float* dS0, void* device_arena,
+                                  size_t arena_bytes, void* cuda_stream)
+{
+    return host_impl(nullptr, p, with_bwd, q, k, v, f, bx, wx, beta, A, tau, Ub, Uw, Vb, Vw, S0, O, S_final, dO, dS_final, dq, dk, dv, df, dbx, dwx, dbeta, dA, dtau, dUb, dUw, dVb, dVw, dS0, device_arena, arena_bytes, cuda_stream);
+}
+
+carve_status_t carve_host_ctx_create(carve_host_ctx_t** out)
+{
+    if (!out) return CARVE_ERR_NULL;
+    *out = nullptr;
+    carve_host_ctx* c = new (std::nothrow) carve_host_ctx();
+    if (!c) return CARVE_ERR_CUDA;
+    bool ok = cudaEventCreateWithFlags(&c->fork, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < 8; ++i) {
+        ok = ok && cudaStreamCreateWithFlags(&c->side[i], cudaStreamNonBlocking) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&c->join[i], cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&c->arrived[i], cudaEventDisableTiming) == cudaSuccess;
+    }
+    if (!ok) { carve_host_ctx_destroy(c); return CARVE_ERR_CUDA; }
+    *out = c;
+    return CARVE_OK;
+}
+
+void carve_host_ctx_destroy(carve_host_ctx_t* c)
+{
+    if (!c) return;
+    for (int i = 0; i < 8; ++i) {
+        if (c->side[i]) cudaStreamDestroy(c->side[i]);
+        if (c->join[i]) cudaEventDestroy(c->join[i]);
+        if (c->arrived[i]) cudaEventDestroy(c->arrived[i]);
+    }
+    if (c->fork) cudaEventDestroy(c->fork);
+    delete c;
+}
+
+carve_status_t carve_fwd_bwd_host_ctx(carve_host_ctx_t* ctx, const carve_params_t* p, int with_bwd, const void* q, const void* k,
+                                  const void* v, const void* f, const void* bx, const void* wx, const void* beta,
+                                  const float* A, const float* tau, const float* Ub, const float* Uw,
+                                  const float* Vb, const float* Vw, const float* S0, void* O, float* S_final,
+                                  const void* dO, const float* dS_final, void* dq, void* dk, void* dv, void* df,
+                                  void* dbx, void* dwx, void* dbeta, float* dA, float* dtau, float* dUb,
+                                  float* dUw, float* dVb, float* dVw, float* dS0, void* device_arena,
+                                  size_t arena_bytes, void* cuda_stream)
+{
+    return host_impl(ctx, p, with_bwd, q, k, v, f, bx, wx, beta, A, tau, Ub, Uw, Vb, Vw, S0, O, S_final, dO, dS_final, dq, dk, dv, df, dbx, dwx, dbeta, dA, dtau, dUb, dUw, dVb, dVw, dS0, device_arena, arena_bytes, cuda_stream);
 }
 
 }  // extern "C"

@@ -105,3 +105,27 @@ def test_config3_full_tensors(oracle):
 def test_config4_full_tensors(oracle):
     """Config 4 (2048 chains, d = 64, beta = 1 on 10 % of tokens, no decay on 10 % of key dims): every chain of every wave."""
     _full_tensor_parity(oracle, synth.CFG4)
+
+
+@pytest.mark.parametrize("cfg", [synth.CFG1, synth.CFG4, synth.CFG2[128]], ids=lambda c: c.name)
+def test_full_size_run_to_run_bitwise(cfg):
+    """Two back-to-back fwd+bwd calls at full size give bit-identical tensors (no float atomics; and a race between the
+    asynchronous copies -- TMA loads, record bulk copies, the staged output store -- and the threads would show here)."""
+    x, ct = synth.make_inputs(cfg), synth.make_cotangents(cfg)
+    p = params_of(cfg)
+    st = torch.cuda.current_stream().cuda_stream
+    xd = to_device(x, torch.bfloat16)
+    dO = to_device({"dO": ct["dO"]}, torch.bfloat16)["dO"]
+    dSf = torch.from_numpy(ct["dS_final"]).cuda()
+    ws = torch.empty(carve.carve_workspace_bytes(p, True), dtype=torch.uint8, device="cuda")
+    outs = []
+    for _ in range(2):
+        O = torch.empty(cfg.B, cfg.T, cfg.H, cfg.dv, dtype=torch.bfloat16, device="cuda")
+        Sf = torch.empty(cfg.B, cfg.H, cfg.dv, cfg.dk, dtype=torch.float32, device="cuda")
+        g = alloc_grads(p, torch.bfloat16)
+        carve.carve_fwd(p, xd, O, Sf, ws, st)
+        carve.carve_bwd(p, xd, dO, dSf, g, ws, st)
+        torch.cuda.synchronize()
+        outs.append(dict(g, O=O, S_final=Sf))
+    for n in outs[0]:
+        assert torch.equal(outs[0][n], outs[1][n]), n

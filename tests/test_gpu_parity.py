@@ -175,6 +175,17 @@ def test_host_entry_point_matches_device_entry_point(oracle, B):
             assert relerr(got, g[n]) < 1e-5, n
         else:
             assert np.array_equal(got, g[n]), n
+    # the same call with caller-owned streams and events (carve_host_ctx_create), twice on one context: identical results
+    ctx = carve.carve_host_ctx_create()
+    first = {n: gh[n].clone() for n in GRADS}
+    for _ in range(2):
+        Oh.zero_()
+        carve.carve_fwd_bwd_host(p, True, xh, Oh, Sfh, dOh, dSfh, gh, arena, torch.cuda.current_stream().cuda_stream, ctx=ctx)
+        torch.cuda.synchronize()
+        assert np.array_equal(Oh.float().numpy().astype(np.float64), O)
+        for n in GRADS:
+            assert torch.equal(gh[n], first[n]), n
+    carve.carve_host_ctx_destroy(ctx)
 
 
 # ---- both kernel families against the oracle on the same bf16 case --------------------------------
