@@ -32,7 +32,7 @@ constexpr uint32_t TM_X2 = 384;   // G^T | Z, then the log-retention scan, then 
 constexpr uint32_t TM_COLS = 512;
 
 struct Layout {  // byte offsets into the 1024-aligned dynamic shared memory
-    uint32_t Sb, Ucat, Vcat, KQraw, F, BX, WX, V, KQbar, Ktil, Us, Y0, Y1, Y2, TP, Mm, Tm, misc, total;
+    uint32_t Sb, Ucat, Vcat, KQraw, F, BX, WX, V, KQbar, Ktil, Us, Y0, Y1, Y2, V1, V3, TP, Mm, Tm, misc, total;
     __host__ __device__ Layout(int dk, int dv, int r2)
     {
         uint32_t o = 0;
@@ -47,13 +47,19 @@ struct Layout {  // byte offsets into the 1024-aligned dynamic shared memory
         WX = take(tile_bytes(64, dv));      // TMA: write pre-activation    | later Ktil
         V = take(tile_bytes(64, dv));       // TMA: values -> V' = w.v      | later U
         KQbar = F; Ktil = WX; Us = V;
-        Y0 = take((uint32_t)dk * 128);      // G (rows j, cols i) | la_hi | row operands re-anchored at token 32
-        Y1 = take(16384);                   // [0 tt_w; tt_b 0] | la_lo | C (column operand of A and P)
-        Y2 = take(16384);                   // block-triangular ones | beta R
+        // d = 128: one CTA per SM fills the shared memory.  d = 64: compacted to 112 KB so that TWO CTAs (two chains) share an
+        // SM and hide each other's latency (config 4 has 2048 chains): the row operands of anchor blocks 1 and 3 live in TP
+        // (free until P9a), those of block 2 in the upper half of Y1, and beta R / the output tile need only 8 KB.
+        const bool compact = dk == 64;
+        Y1 = take(16384);                   // [tt_b | tt_w] (128 rows) | C (column operand of A and P, 64 rows)
+        Y0 = compact ? Y1 + 8192 : take((uint32_t)dk * 128);   // row operands re-anchored at token 32
+        Y2 = take(compact ? 8192 : 16384);  // beta R | output tile (| d = 128: row operands re-anchored at tokens 16, 48)
         TP = take(16384);                   // rows 0..63 T = (I + beta A)^-1, rows 64..127 P
-        if (tile_bytes(128, dk) >= 32768) { Mm = KQraw; Tm = KQraw + 16384; }
-        else { Mm = take(16384); Tm = take(16384); }  // fp32 scratch of the triangular inverse
-        misc = take(8192);
+        V1 = compact ? TP : Y2;             // row operands re-anchored at token 16 (96 rows) ...
+        V3 = V1 + tile_bytes(96, dk);       // ... and at token 48 (32 rows)
+        Mm = KQraw;                         // fp32 beta A [64][64] over the raw k|q tile (dead after P7)
+        misc = take(6144);                  // MiscT<dk>; at d = 64 it takes 4 KB and the diagonal inverses follow it
+        Tm = compact ? misc + 4096 : KQraw + 16384;   // 8x8 diagonal inverses, [64][8] fp32
         total = o + 1024;                   // slack for the manual 1024-byte alignment
     }
 };
@@ -70,7 +76,10 @@ struct Layout {  // byte offsets into the 1024-aligned dynamic shared memory
 //   KQo  [128][dk]  the same rows anchored at the start of their own 16-token block
 //   CC   [64][dk]   C_s = k^_s gamma_a/gamma_s (a = start of s's 16-token block)
 //   VWX,W [64][dv]  w.v.(1-w) and w;  Bg [64][dk] erase gate b;  FQ,IC [64][dk] gamma_t/gamma_a and its inverse (row-private, piece-major)
-//   tt   [64][32]   tanh bottleneck (bf16, plain rows);  GT [dk][32] G^T (tile);  etot [4][dk], rn [128], beta [64] fp32
+//   tt   [64][64]   tanh bottleneck: the K-side rows of the forward's tile, erase half in chunks 0,1, write half in chunks 2,3
+//   GT   [dk][64]   the forward's Vcat tile: columns 32.. hold G^T;  etot [4][dk], rn [128], beta [64] fp32
+//   (tt, GT, etot, beta leave by bulk copies: per-thread global stores in the sections only a few warps run cost far
+//    more than their bytes)
 struct Rec {
     uint32_t SB, KT, PT, U, K0, Q0, KQo, CC, VWX, W, Bg, FQ, IC, tt, GT, etot, rn, beta, total;
     __host__ __device__ Rec(int dk, int dv)
@@ -90,7 +99,7 @@ struct Rec {
         Bg = take(tile_bytes(64, dk));
         FQ = take(tile_bytes(64, dk));
         IC = take(tile_bytes(64, dk));
-        tt = take(64 * 64);
+        tt = take(64 * 128);               // rows 0..63 of the forward's [tt_b pad 16 | tt_w pad 16] tile (bulk copy)
         GT = take(tile_bytes(dk, 64));
         etot = take(4u * dk * 4u);
         rn = take(128 * 4);
@@ -104,20 +113,19 @@ struct Rec {
 // contiguous bytes both when the forward stores it and when the reverse kernel loads it.
 __host__ __device__ __forceinline__ uint32_t rp_off(int row, int cc) { return (uint32_t)((cc * 64 + row) * 16); }
 
-// misc area (floats unless noted)
-struct Misc {
-    float eA[128], tau[128];    // exp(A_h), tau_h
-    float etot[4][128];         // exp(sum of log a over 16-token anchor block b)
-    float suf[4][128];          // product of etot[b'] over b' > b
-    float gamL[128];            // gamma_{L-1} of the chunk
-    float nrm[128][4];          // partial sums of squares: rows 0..63 k, 64..127 q; [column part]
+// misc area of the forward kernel (floats unless noted), sized by the key dimension
+template <int DK>
+struct MiscT {
+    float eA[DK], tau[DK];      // exp(A_h), tau_h
+    float etot[4][DK];          // exp(sum of log a over 16-token anchor block b)
+    float gamL[DK];             // gamma_{L-1} of the chunk
+    float nrm[128][DK / 32];    // partial sums of squares: rows 0..63 k, 64..127 q; [column part]
     float beta[64];             // write strength of the chunk's tokens
     uint64_t bar_mma, bar_kq, bar_fb, bar_wv;
     uint64_t bar_acc;           // the state products of P8 (waited for after the A|P blocks have been consumed)
     uint32_t tmem_base;
 };
-
-static_assert(sizeof(Misc) <= 8192, "misc area too small");
+static_assert(sizeof(MiscT<128>) <= 6144 && sizeof(MiscT<64>) <= 4096, "misc area too small");
 
 // Bare MUFU transcendentals (flush-to-zero forms: no denormal range fix-up code around them; every use below either
 // has a result whose flush to 0 is the correct limit or an argument >= 1).

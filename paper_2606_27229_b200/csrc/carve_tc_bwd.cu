@@ -809,7 +809,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 for (int i = 0; i < HK / 8; ++i)
                     d4[i] = SW ? make_uint4(0u, 0u, 0u, 0u) : *reinterpret_cast<const uint4*>(gdwx + 8 * (half * (HK / 8) + i));
 #pragma unroll
-                for (int i = 0; i < 4; ++i) t4[i] = ldg128(rc + Rc.tt + t * 64 + 16 * i);
+                for (int i = 0; i < 4; ++i)   // packed chunk i of [tt_b | tt_w] -> chunk of the forward's tile (each half padded to 16 columns)
+                    t4[i] = ldg128(rc + Rc.tt + tile_chunk_off(128, t, i < (r >> 3) ? i : 2 + i - (r >> 3)));
             }
             WAIT_MMA();
             PROF(g_prof_bwd, 24);
@@ -872,7 +873,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(rn_ + Rc.VWX + rp_off(t, cq0 + i)));
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(rn_ + Rc.W + rp_off(t, cq0 + i)));
             }
-            if (!krole && half < 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(rn_ + Rc.tt + t * 64));
+            if (!krole && half < 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(rn_ + Rc.tt + tile_chunk_off(128, t, 0)));
         }
         WAIT_MMA();
         PROF(g_prof_bwd, 27);
@@ -912,7 +913,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mbar_wait(&mi.bar_g8, ph);
             mbar_wait(&mi.bar_g5, ph);
             tc_fence_after();
-            mma_k<KMAJ, KMAJ, 32>(tmem + BM_A, D, sb + Lo.S[0], 128, 0, 0, sb + Lo.S[5], D, 0, 0, R2, true);
+            mma_k<KMAJ, KMAJ, 32>(tmem + BM_A, D, sb + Lo.S[0], 128, 0, 0, sb + Lo.S[5], D, 0, 32, R2, true);   // G^T: columns 32.. of the Vcat tile
             mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_DAP + 32, 32, sb + Lo.S[6], 64, 0, 0, sb + Lo.S[4], 64, 0, 0, LCc, false);
             umma_commit(&mi.bar_mma);
         LEADER_END

@@ -86,7 +86,7 @@ __device__ __forceinline__ void diag8_inverse(const float* Mm, float* Tm, int n,
 #pragma unroll
             for (int s = 0; s < tt; ++s) acc += Mm[mm_idx(o + tt, o + s)] * x[s];
             x[tt] = (tt == c) ? 1.f : (tt < c ? 0.f : -acc);
-            Tm[mm_idx(o + tt, o + c)] = x[tt];
+            Tm[(o + tt) * 8 + c] = x[tt];   // [64][8]: the 8x8 diagonal blocks only
         }
     }
 }
@@ -144,7 +144,7 @@ __device__ __forceinline__ void wy_solve(const float* Mm, const float* Tm, int n
             }
 #pragma unroll
             for (int e = 0; e < 4; ++e) y[e] -= s0[e] + s1[e];
-            const float2 tb = *reinterpret_cast<const float2*>(&Tm[mm_idx(8 * i + g, 8 * i + 2 * l4)]);
+            const float2 tb = *reinterpret_cast<const float2*>(&Tm[(8 * i + g) * 8 + 2 * l4]);
             const uint32_t af[4] = {__float_as_uint(y[0]), __float_as_uint(y[2]), __float_as_uint(y[1]), __float_as_uint(y[3])};
             const uint32_t bf[2] = {__float_as_uint(tb.x), __float_as_uint(tb.y)};
 #pragma unroll
@@ -186,13 +186,15 @@ __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.w
 // SW = 1: scalar-write variant (wx = Uw = Vw = NULL, P l.145) -- w == 1, V' = v; compiled separately so that the full-gate
 // kernel carries none of its branches.
 template <int DK, int DV, int NP, int VS, int SW>
-__global__ void __launch_bounds__(128 * NP, 1)
+__global__ void __launch_bounds__(128 * NP, DK == 64 ? 2 : 1)
 carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, const __grid_constant__ CUtensorMap mk,
                     const __grid_constant__ CUtensorMap mv, const __grid_constant__ CUtensorMap mf,
                     const __grid_constant__ CUtensorMap mbx, const __grid_constant__ CUtensorMap mwx,
                     const __grid_constant__ CUtensorMap mo)
 {
     static_assert(DK == DV, "the shared-memory map assumes dk == dv");
+    // TMEM column map: 4 regions of DK columns (d = 64: 256 columns, so that two CTAs fit the SM's 512)
+    constexpr uint32_t TM_S = 0, TM_ACC = DK, TM_X1 = 2 * DK, TM_X2 = 3 * DK, TM_COLS = 4 * DK;
     constexpr int DM = DK > DV ? DK : DV;
     constexpr int NTH = 128 * NP;
     // issues (and waits for) the record's bulk copies: lane 0 of a Q-side warp of the last column part, which has
@@ -206,6 +208,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     uint8_t* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     const int r = a.r, R2 = 2 * r;
     const Layout Lo(DK, DV, R2);
+    using Misc = MiscT<DK>;
     Misc& mi = *reinterpret_cast<Misc*>(sm + Lo.misc);
     float* sBeta = mi.beta;
     const uint32_t sb = smem_u32(sm);
@@ -246,7 +249,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         else if (c < 32) { if (c - 16 < r && n < DV && !SW) v = __ldg(a.Vw + (size_t)(vofs + n) * r + (c - 16)); }
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Vcat + tile_off(DM, n, c)) = __float2bfloat16_rn(v);
     }
-    for (int j = tid; j < 4 * 128; j += NTH) mi.etot[j >> 7][j & 127] = 1.f;
+    for (int j = tid; j < 4 * DK; j += NTH) mi.etot[j / DK][j % DK] = 1.f;
     for (int j = tid; j < DK; j += NTH) {
         mi.eA[j] = a.A ? __expf(__ldg(a.A + h * DK + j)) : 1.f;
         mi.tau[j] = a.tau ? __ldg(a.tau + h * DK + j) : 0.f;
@@ -367,7 +370,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 const float bt = fmaxf(__uint_as_float(beta_nx << 16), 1e-30f);
                 if (c + 1 < nchunks) beta_nx = (uint32_t)__ldg(beta_bits + (tok0 + LCc + t) * a.H + h);
                 sBeta[t] = bt;
-                if (rc) reinterpret_cast<float*>(rc + Rc.beta)[t] = bt;
             }
         }
         PROF(g_prof_fwd, 21);
@@ -412,21 +414,17 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                     }
                     sts128(sm + Lo.Vcat + tile_chunk_off(DM, row, (32 + c0) / 8), pack8(f));
                     sts128(sm + Lo.Vcat + tile_chunk_off(DM, row, (32 + c0) / 8 + 1), pack8(f + 8));
-                    if (rc) {
-                        *reinterpret_cast<uint4*>(rc + Rc.GT + tile_chunk_off(DK, row, c0 / 8)) = pack8(f);
-                        *reinterpret_cast<uint4*>(rc + Rc.GT + tile_chunk_off(DK, row, c0 / 8 + 1)) = pack8(f + 8);
-                    }
                 }
             }
-        } else if (rc && half == 0 && q * 32 < DK) {
-            // second solve chunk of a gate chunk (L = 128): same G, copied into this chunk's record
-            for (int c0 = 0; c0 < R2; c0 += 8)
-                *reinterpret_cast<uint4*>(rc + Rc.GT + tile_chunk_off(DK, row, c0 / 8)) =
-                    lds128(sm + Lo.Vcat + tile_chunk_off(DM, row, (32 + c0) / 8));
         }
         PROF(g_prof_fwd, 2);
         // ---- P2: Z = [k;q] G^T -> TM_X2[32, 32+R2)
         PROFB_ARRIVE(1); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 1);
+        if (rc && tid == REC_TID) {   // record: the Vcat tile (its columns 32.. hold G^T) and the write strengths
+            bulk_s2g(rc + Rc.GT, sb + Lo.Vcat, tile_bytes(DM, 64));
+            bulk_s2g(rc + Rc.beta, smem_u32(mi.beta), 256);
+            bulk_commit();
+        }
         if (warp == 0) {
             if (elect_one()) {
                 mma_rt<128, KMAJ, MNMAJ, DK>(tmem + TM_X2 + 32, R2, sb + Lo.KQraw, 128, 0, sb + Lo.Vcat, DM, 32, DK, false);
@@ -452,7 +450,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
 #pragma unroll
                         for (int e = 0; e < 8; ++e) f[e] = tanh_fast(__uint_as_float(v[e]) * rnq);
                         const uint4 w = pack8(f);
-                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.tt + t * 64 + sc * 16) = w;
                         const int dst = 8 * sc < r ? sc : 2 + (8 * sc - r) / 8;   // erase half | write half, each padded to 16
                         sts128(sm + Lo.Y1 + tile_chunk_off(128, 64 + t, dst), w);
                         sts128(sm + Lo.Y1 + tile_chunk_off(128, t, dst), w);
@@ -467,6 +464,10 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROF(g_prof_fwd, 4);
         // ---- P4: b_proj = [tt_b;tt_b] Vb^T -> TM_X1, w_proj = [tt_w;tt_w] Vw^T -> TM_X2 (both row halves get both)
         PROFB_ARRIVE(2); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 2);
+        if (rc && tid == REC_TID) {   // record: the K-side rows of the bottleneck tile (Y1 is rewritten in P7, after this thread's wait)
+            bulk_s2g(rc + Rc.tt, sb + Lo.Y1, 8192);
+            bulk_commit();
+        }
         if (warp == 0) {
             if (elect_one()) {
                 umma_prod<KMAJ, KMAJ, 16>(tmem + TM_X1, 128, DK, sb + Lo.Y1, 128, 0, 0, sb + Lo.Vcat, DM, 0, 0, 16, false);
@@ -547,23 +548,21 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
             if (live && (lane & 15) == 15) {   // last token of its anchor block: exp of the block totals
-                float* re = rc ? reinterpret_cast<float*>(rc + Rc.etot) : nullptr;
 #pragma unroll
-                for (int e4 = 0; e4 < 4; ++e4) {
-                    const float4 ev = make_float4(exp_fast(lg[4 * e4]), exp_fast(lg[4 * e4 + 1]), exp_fast(lg[4 * e4 + 2]), exp_fast(lg[4 * e4 + 3]));
-                    *reinterpret_cast<float4*>(&mi.etot[blk][8 * cc0 + 4 * e4]) = ev;
-                    if (re) {
-                        *reinterpret_cast<float4*>(re + blk * DK + 8 * cc0 + 4 * e4) = ev;
-                        if (t == LCc - 1)   // blocks that do not exist at L < 64 count as no decay
-                            for (int b2 = blk + 1; b2 < 4; ++b2)
-                                *reinterpret_cast<float4*>(re + b2 * DK + 8 * cc0 + 4 * e4) = make_float4(1.f, 1.f, 1.f, 1.f);
-                    }
-                }
+                for (int e4 = 0; e4 < 4; ++e4)
+                    *reinterpret_cast<float4*>(&mi.etot[blk][8 * cc0 + 4 * e4]) =
+                        make_float4(exp_fast(lg[4 * e4]), exp_fast(lg[4 * e4 + 1]), exp_fast(lg[4 * e4 + 2]), exp_fast(lg[4 * e4 + 3]));
             }
         }
         PROF(g_prof_fwd, 6);
         if (tid == 0) bulk_wait_read();   // the output tile has left Y2 (rewritten below)
+        if (rc && tid == REC_TID) bulk_wait_read();   // the previous chunk's [P;T] copy has left TP (d = 64: rewritten below; else in P9)
+        fence_async_smem();   // (the block totals leave by a bulk copy)
         PROFB_ARRIVE(3); __syncthreads(); PROFB_AFTER(g_profb_fwd, 3);
+        if (rc && tid == REC_TID) {   // record: exp of the block totals (blocks that do not exist at L < 64 hold 1)
+            bulk_s2g(rc + Rc.etot, smem_u32(&mi.etot[0][0]), 16u * DK);
+            bulk_commit();
+        }
         PROF(g_prof_fwd, 8);
         // ---- P7b: decayed operands.  Row operands exist in up to four anchorings: version 0 relative to the chunk
         //      start (Kbar, Qbar: also the operand of the state products), version jb relative to the start of
@@ -574,9 +573,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             auto ver_row = [&](int jb, bool qrole, int tok, int cc) -> uint8_t* {
                 switch (jb) {
                     case 0: return sm + Lo.KQbar + tile_chunk_off(128, (qrole ? 64 : 0) + tok, cc);
-                    case 1: return sm + Lo.Y2 + tile_chunk_off(96, (qrole ? 48 : 0) + tok - 16, cc);
+                    case 1: return sm + Lo.V1 + tile_chunk_off(96, (qrole ? 48 : 0) + tok - 16, cc);
                     case 2: return sm + Lo.Y0 + tile_chunk_off(64, (qrole ? 32 : 0) + tok - 32, cc);
-                    default: return sm + Lo.Y2 + tile_bytes(96, DK) + tile_chunk_off(32, (qrole ? 16 : 0) + tok - 48, cc);
+                    default: return sm + Lo.V3 + tile_chunk_off(32, (qrole ? 16 : 0) + tok - 48, cc);
                 }
             };
             // Both threads of a token (K-side lane t, Q-side lane 64+t) hold +-(lg_t - lg_a) of the same columns: each
@@ -674,7 +673,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 }
             }
         }
-        if (rc && tid == REC_TID) bulk_wait_read();   // the previous chunk's [P;T] copy has left TP (rewritten in P9)
         PROF(g_prof_fwd, 9);
         // ---- P8: A|P blocks (one 16-column block per anchoring) and the state products
         PROFB_ARRIVE(4); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 4);
@@ -685,9 +683,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             if (elect_one()) {
                 const int nb = LCc >> 4;
                 mma_rt<128, KMAJ, KMAJ, DK>(tmem + TM_X2, 16, sb + Lo.KQbar, 128, 0, sb + Lo.Y1, 64, 0, DK, false);
-                if (nb > 1) mma_rt<128, KMAJ, KMAJ, DK>(tmem + TM_X2 + 16, 16, sb + Lo.Y2, 96, 0, sb + Lo.Y1, 64, 16, DK, false);
+                if (nb > 1) mma_rt<128, KMAJ, KMAJ, DK>(tmem + TM_X2 + 16, 16, sb + Lo.V1, 96, 0, sb + Lo.Y1, 64, 16, DK, false);
                 if (nb > 2) mma_rt<64, KMAJ, KMAJ, DK>(tmem + TM_X2 + 32, 16, sb + Lo.Y0, 64, 0, sb + Lo.Y1, 64, 32, DK, false);
-                if (nb > 3) mma_rt<64, KMAJ, KMAJ, DK>(tmem + TM_X2 + 48, 16, sb + Lo.Y2 + tile_bytes(96, DK), 32, 0, sb + Lo.Y1, 64, 48, DK, false);
+                if (nb > 3) mma_rt<64, KMAJ, KMAJ, DK>(tmem + TM_X2 + 48, 16, sb + Lo.V3, 32, 0, sb + Lo.Y1, 64, 48, DK, false);
                 umma_commit(&mi.bar_mma);   // the A|P blocks: P9a starts on them while the state products still run
                 mma_rt<128, KMAJ, KMAJ, DK>(tmem + TM_ACC, DV, sb + Lo.KQbar, 128, 0, sb + Lo.Sb, DV, 0, DK, false);
                 umma_commit(&mi.bar_acc);
@@ -1005,6 +1003,7 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
     auto kern = carve_fwd_tc_kernel<D, D, NP, VS, SW>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
+    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100);   // (two CTAs per SM at d = 64)
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)(a.B * a.H * VS));
     cfg.blockDim = dim3(128 * NP);
