@@ -62,7 +62,7 @@ constexpr uint32_t BM_WU = 480;   // [x lanes][32]  d[Ub;Uw]^T, accumulated over
 
 constexpr uint32_t SLOT = 16384;
 struct BLayout {  // byte offsets into the 1024-aligned dynamic shared memory
-    uint32_t DSB, SBq, S[7], TRI, VcT, Ucat, FI, misc, total;
+    uint32_t DSB, SBq, S[7], TRI, X, VcT, Ucat, FI, misc, total;
     __host__ __device__ BLayout(int d)
     {
         uint32_t o = 0;
@@ -70,7 +70,8 @@ struct BLayout {  // byte offsets into the 1024-aligned dynamic shared memory
         DSB = take(tile_bytes(d, d));   // bf16 dS' (rows x, cols j)
         SBq = take(tile_bytes(d, d));   // bf16 state entering the chunk (record SB)
         for (int i = 0; i < 7; ++i) S[i] = take(SLOT);
-        TRI = take(24576);              // [64][192] 0/1: cols 0..63 t' > t, cols 64..127 t' >= t, cols 128..191 t' < t
+        TRI = take(8192);               // [64][64] 0/1: t' > t; its MN-major view is t' < t
+        X = take(SLOT);                 // dw_pre (L2 .. L7: staged dwx, then the L7 operand), then dz (L7 .. L8)
         VcT = take(tile_bytes(32, d));  // rows i: [Vb^T ; Vw^T]
         Ucat = take(tile_bytes(32, d)); // rows i: [Ub ; Uw]
         // staging of row-private record tiles (FQ | IC, later b): over DSB once dS' is consumed when it fits (d = 128)
@@ -179,10 +180,17 @@ __device__ __forceinline__ void warp_colsum(float (&v)[N], int lane)
 // NP = column parts per tile row = warpgroups per CTA (threads = 128 NP): 32 columns per thread.
 template <int D, int NP, int SW>   // SW = 1: scalar-write variant (w == 1), compiled separately
 __global__ void __launch_bounds__(128 * NP, 1)
-carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, const __grid_constant__ CUtensorMap mq)
+carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, const __grid_constant__ CUtensorMap mq,
+                    const __grid_constant__ CUtensorMap mdq, const __grid_constant__ CUtensorMap mdk,
+                    const __grid_constant__ CUtensorMap mdv, const __grid_constant__ CUtensorMap mdf,
+                    const __grid_constant__ CUtensorMap mdbx, const __grid_constant__ CUtensorMap mdwx)
 {
     constexpr int NTH = 128 * NP;
     constexpr int LEADER_WARP = NTH / 32 - 1;   // MMA issuer: the last warp (see L1)
+    // The six per-token gradient tiles of a chunk are staged in shared memory (in place over operands that are dead by
+    // then) and leave by TMA stores issued by this one thread (bulk groups are per thread); it also issues the loads that
+    // overwrite a staging tile, after cp.async.bulk.wait_group.read, and publishes the chain's progress flag.
+    constexpr int STORE_TID = NTH - 64;
     constexpr int HK = D / NP;                     // columns per warpgroup ("half" = part index 0..NP-1)
     constexpr uint32_t TB = tile_bytes(64, D);     // one [64][D] tile
     constexpr uint32_t SBb = tile_bytes(D, D);     // one state tile
@@ -217,7 +225,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         mbar_init(&mi.bar_g4a, 1); mbar_init(&mi.bar_g4b, 1); mbar_init(&mi.bar_g5, 1); mbar_init(&mi.bar_g8, 1);
         mbar_init(&mi.bar_fi, 1); mbar_init(&mi.bar_bg, 1); mbar_init(&mi.bar_pt, 1);
         mbar_fence_init();
-        tma_prefetch_desc(&mdO); tma_prefetch_desc(&mq);
+        tma_prefetch_desc(&mdO); tma_prefetch_desc(&mq); tma_prefetch_desc(&mdq); tma_prefetch_desc(&mdk);
+        tma_prefetch_desc(&mdv); tma_prefetch_desc(&mdf); tma_prefetch_desc(&mdbx); tma_prefetch_desc(&mdwx);
     }
     if (warp == 0) tmem_alloc(&mi.tmem_base, TM_COLS);
     for (int i = tid; i < 32 * D; i += NTH) {
@@ -228,10 +237,9 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.VcT + tile_off(32, ii, n)) = __float2bfloat16_rn(vc);
         *reinterpret_cast<__nv_bfloat16*>(sm + Lo.Ucat + tile_off(32, ii, n)) = __float2bfloat16_rn(uc);
     }
-    for (int i = tid; i < 64 * 192; i += NTH) {
-        const int tt_ = i / 192, k = i % 192;
-        const bool one = k < 64 ? (k > tt_) : k < 128 ? (k - 64 >= tt_) : (k - 128 < tt_);
-        *reinterpret_cast<uint16_t*>(sm + Lo.TRI + tile_off(64, tt_, k)) = one ? 0x3F80u : 0u;
+    for (int i = tid; i < 64 * 64; i += NTH) {
+        const int tt_ = i / 64, k = i % 64;
+        *reinterpret_cast<uint16_t*>(sm + Lo.TRI + tile_off(64, tt_, k)) = k > tt_ ? 0x3F80u : 0u;
     }
     if (tid < D) {
         const float* et = reinterpret_cast<const float*>(rec_chain + (size_t)(nchunks - 1) * Rc.total + Rc.etot);
@@ -298,9 +306,22 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         bulk_g2s(sm + Lo.S[4], r2 + Rc.U, TB, &mi.bar_g1);
         for (int cb = 0; cb < D / 64; ++cb)
             tma_load_3d(sm + Lo.S[2] + cb * 16384 + 8192, &mdO, &mi.bar_g1, cb * 64, h, b * a.T + c2 * LCc);
+    };
+    auto issue_g3 = [&](int c2) {
+        const uint8_t* r2 = rec_chain + (size_t)c2 * Rc.total;
         mbar_expect_tx(&mi.bar_g3, 2 * TB);
         bulk_g2s(sm + Lo.S[5], r2 + Rc.K0, TB, &mi.bar_g3);
         bulk_g2s(sm + Lo.S[6], r2 + Rc.Q0, TB, &mi.bar_g3);
+    };
+    // [LCc][D] gradient tile (64-row tile format == the 128-byte-swizzled TMA box) -> global; `cbs` = byte stride
+    // between the two 64-column blocks (8192 for a 64-row tile, 16384 for the lower rows of a 128-row tile)
+    auto store_tile = [&](const CUtensorMap* m, uint32_t src, uint32_t cbs, int trow_) {
+        for (int cb = 0; cb < D / 64; ++cb) tma_store_3d(m, sb + src + cb * cbs, cb * 64, h, trow_);
+    };
+    auto publish = [&](int done) {   // the bulk stores of the first `done` chunks (in processing order) are complete
+        asm volatile("fence.proxy.async.global;" ::: "memory");
+        __threadfence();
+        asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.flags + chain), "r"(done) : "memory");
     };
     auto issue_pt = [&](int c2) {
         mbar_expect_tx(&mi.bar_pt, 16384);
@@ -323,7 +344,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                 mbar_expect_tx(&mi.bar_sb, SBb);
                 bulk_g2s(sm + Lo.SBq, rc + Rc.SB, SBb, &mi.bar_sb);
             }
-            if (it == 0) { issue_l1(c); issue_pt(c); }
+            if (it == 0) { issue_l1(c); issue_g3(c); issue_pt(c); }
         }
         {
             if (tid >= 128 && tid < 128 + D) {
@@ -411,8 +432,6 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             const float bt = live ? mi.beta[t] : 0.f;
             const float rbt = live ? __fdividef(1.f, bt) : 0.f;   // e_t = u_t / beta_t (beta is clamped to >= 1e-30 by the forward)
             float dbs = 0.f;
-            __nv_bfloat16* gdv = a.dv + ((tok0 + t) * a.H + h) * D;
-            __nv_bfloat16* gdwx = a.dwx + ((tok0 + t) * a.H + h) * D;
             uint32_t v[QW];
             if constexpr (QW == 16) tmem_ld16(tmem + BM_A + lane_base + 8 * cq0, v);
             else tmem_ld32(tmem + BM_A + lane_base + 8 * cq0, v);
@@ -434,8 +453,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         o2[e] = dr * xx[e];
                     }
                     sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8(ndr));
-                    stg128(gdv + 8 * cc, pack8(o1));
-                    if (!SW) stg128(gdwx + 8 * cc, pack8(o2));
+                    sts128(sm + Lo.S[0] + tile_chunk_off(64, t, cc), pack8(o1));   // dv, staged over dU
+                    sts128(sm + Lo.X + tile_chunk_off(64, t, cc), pack8(o2));      // dw_pre = dwx (zeros when SW)
                 }
                 mi.dbp[(krole ? 0 : NP) + half][t] = dbs;
             }
@@ -454,6 +473,11 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_DS, D, sb + Lo.S[2], 128, 0, 64, sb + Lo.S[6], 64, 0, 0, LCc, true);
             umma_commit(&mi.bar_mma);
         LEADER_END
+        if (tid == STORE_TID) {
+            store_tile(&mdv, Lo.S[0], 8192, trow);
+            if (!SW) store_tile(&mdwx, Lo.X, 8192, trow);
+            bulk_commit();
+        }
         if (!krole && half == 0 && live)
         {
             float sdb = 0.f;
@@ -669,6 +693,10 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         carry += tot;
                     }
                 }
+            if (tid == STORE_TID) {   // dv has left S[0] (dlp goes there below); every store of the previous chunk is complete
+                bulk_wait_all();
+                if (it > 0) publish(it);
+            }
             PROFB_ARRIVE(3); __syncthreads(); PROFB_AFTER(g_profb_bwd, 3);  // every warp is done reading DAP / C / KQo
             PROF(g_prof_bwd, 21);
 #pragma unroll
@@ -708,7 +736,6 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             if (krole) {
                 const bool bstart = (t & 15) == 0;
                 const uint4 ones4 = make_uint4(0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u);
-                __nv_bfloat16* gdk = a.dk + ((tok0 + t) * a.H + h) * D;
 #pragma unroll
                 for (int s = 0; s < HK; s += 16) {
                     uint32_t vs[16], vk[16];
@@ -740,7 +767,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                                 xa[e] = k0[e] * sp;                 // Kbar_t . dKbar_t (state read), to d log gamma_{t-1}
                                 zz[e] = (c8[e] * suf[e]) * dkt;     // Ktil_t . dKtil_t (state write), to d log gamma_t' for t' > t
                             }
-                            stg128(gdk + j0, pack8(o));
+                            sts128(sm + Lo.S[5] + tile_chunk_off(64, t, cc), pack8(o));    // dk^, staged in place over Kbar_t
                             sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8(xa));   // in place over H_t
                             sts128(sm + Lo.S[4] + tile_chunk_off(64, t, cc), pack8(zz));    // in place over H'_t
                         }
@@ -784,30 +811,29 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         PROFB_ARRIVE(5); PHASE_SYNC(); PROFB_AFTER(g_profb_bwd, 5);
         PROF(g_prof_bwd, 23);
         LEADER_BEGIN
+            // one 0/1 tile: t' > t as stored (K-major), t' < t as its MN-major view; XQ enters with t' >= t: its diagonal
+            // is added in the epilogue below.  `trh`: the tile as the upper half of the M = 128 operand.
             const uint32_t tri = sb + Lo.TRI, trh = tri - 8192;
             mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT, D / 2, tri, 64, 0, 0, sb + Lo.S[2], 128, 0, 0, LCc, false);
-            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT, D / 2, tri, 64, 0, 64, sb + Lo.S[2], 128, 0, 64, LCc, true);
-            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT, D / 2, tri, 64, 0, 128, sb + Lo.S[4], 64, 0, 0, LCc, true);
+            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT, D / 2, tri, 64, 0, 0, sb + Lo.S[2], 128, 0, 64, LCc, true);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_KT, D / 2, tri, 64, 0, 0, sb + Lo.S[4], 64, 0, 0, LCc, true);
             mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 0, sb + Lo.S[2], 128, D / 2, 0, LCc, false);
-            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 64, sb + Lo.S[2], 128, D / 2, 64, LCc, true);
-            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 128, sb + Lo.S[4], 64, D / 2, 0, LCc, true);
+            mma_k<KMAJ, MNMAJ, LC>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 0, sb + Lo.S[2], 128, D / 2, 64, LCc, true);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_KT + D / 2, D / 2, trh, 64, 0, 0, sb + Lo.S[4], 64, D / 2, 0, LCc, true);
             umma_commit(&mi.bar_mma);
-            // K0, Q0 are dead: fetch G^T of the chunk and the raw q rows for L8
+            // gamma_a/gamma_t (second half of FI) and Q0 are dead: fetch G^T of the chunk and the raw q rows for L8
             mbar_expect_tx(&mi.bar_g8, tile_bytes(D, 64));
-            bulk_g2s(sm + Lo.S[5], rc + Rc.GT, tile_bytes(D, 64), &mi.bar_g8);
+            bulk_g2s(sm + Lo.FI + TB, rc + Rc.GT, tile_bytes(D, 64), &mi.bar_g8);
             mbar_expect_tx(&mi.bar_g5, (uint32_t)LCc * D * 2u);
             for (int cb = 0; cb < D / 64; ++cb) tma_load_3d(sm + Lo.S[6] + cb * 8192, &mq, &mi.bar_g5, cb * 64, h, trow);
             mbar_expect_tx(&mi.bar_bg, TB);   // the erase gate b over gamma_t/gamma_a (dead after L5)
             bulk_g2s(sm + Lo.FI, rc + Rc.Bg, TB, &mi.bar_bg);
         LEADER_END
+        if (tid == STORE_TID) { store_tile(&mdk, Lo.S[5], 8192, trow); bulk_commit(); }
         {
-            // dw_pre rows (written to dwx in L2) -> GW rows 64..127, [tt_b|0 ; 0|tt_w] -> S[1]: Q-side threads, loads first
-            uint4 d4[HK / 8], t4[4];
+            // [tt_b|0 ; 0|tt_w] -> S[1]: Q-side threads, loads first
+            uint4 t4[4];
             if (!krole && live) {
-                const __nv_bfloat16* gdwx = a.dwx + ((tok0 + t) * a.H + h) * D;
-#pragma unroll
-                for (int i = 0; i < HK / 8; ++i)
-                    d4[i] = SW ? make_uint4(0u, 0u, 0u, 0u) : *reinterpret_cast<const uint4*>(gdwx + 8 * (half * (HK / 8) + i));
 #pragma unroll
                 for (int i = 0; i < 4; ++i)   // packed chunk i of [tt_b | tt_w] -> chunk of the forward's tile (each half padded to 16 columns)
                     t4[i] = ldg128(rc + Rc.tt + tile_chunk_off(128, t, i < (r >> 3) ? i : 2 + i - (r >> 3)));
@@ -815,8 +841,6 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             WAIT_MMA();
             PROF(g_prof_bwd, 24);
             if (!krole && live) {
-#pragma unroll
-                for (int i = 0; i < HK / 8; ++i) sts128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, half * (HK / 8) + i), d4[i]);
                 // TT2: row t = [tt_b | 0], row 64+t = [0 | tt_w] over 32 columns; part 0 writes the K-side row
                 const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
                 const int rc8 = r >> 3;  // 16-byte chunks per gate half
@@ -830,8 +854,6 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mbar_wait(&mi.bar_bg, ph);
             PROF(g_prof_bwd, 25);
             if (warp_active) {
-                __nv_bfloat16* gdf = a.df + ((tok0 + t) * a.H + h) * D;
-                __nv_bfloat16* gdbx = a.dbx + ((tok0 + t) * a.H + h) * D;
                 uint32_t v[QW];
                 if constexpr (QW == 16) tmem_ld16(tmem + BM_KT + lane_base + 8 * cq0, v);
                 else tmem_ld32(tmem + BM_KT + lane_base + 8 * cq0, v);
@@ -840,32 +862,40 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
 #pragma unroll
                     for (int i = 0; i < QW / 8; ++i) {
                         const int cc = cq0 + i;
-                        float bb[8], dp[8], dla[8], dbp[8];
+                        float bb[8], dp[8], xq[8], dla[8], dbp[8];
                         unpack8(lds128(sm + Lo.FI + rp_off(t, cc)), bb);
                         unpack8(lds128(sm + Lo.S[0] + tile_chunk_off(64, t, cc)), dp);
+                        unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc)), xq);   // the t' = t term of XQ
 #pragma unroll
                         for (int e = 0; e < 8; ++e) {
-                            dla[e] = __uint_as_float(v[8 * i + e]) + dp[e] + mi.extra[8 * cc + e];
+                            dla[e] = (__uint_as_float(v[8 * i + e]) + xq[e]) + dp[e] + mi.extra[8 * cc + e];
                             dbp[e] = -dla[e] * bb[e];
                         }
-                        stg128(gdf + 8 * cc, pack8(dla));    // d log a; the epilogue kernel turns it into df
-                        const uint4 w = pack8(dbp);
-                        stg128(gdbx + 8 * cc, w);
-                        sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), w);   // GW rows 0..63 = db_pre
+                        // d log a (the epilogue kernel turns it into df), staged in place over dlp; db_pre = dbx is both the
+                        // staged gradient tile and rows 0..63 of the L7 operand GW
+                        sts128(sm + Lo.S[0] + tile_chunk_off(64, t, cc), pack8(dla));
+                        sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8(dbp));
                     }
                 }
             }
         }
         PROF(g_prof_bwd, 7);
-        // ---- L7: ZZ = [db_pre; dw_pre] [Vb | Vw] -> BM_DAP;  dVb | dVw += [db_pre; dw_pre]^T TT2 -> BM_WG
+        // ---- L7: ZZ_b = db_pre Vb -> BM_DAP rows 0..63, ZZ_w = dw_pre Vw -> BM_DAP + 16 rows 64..127 (dw_pre: the tile X
+        //      as the upper half of the operand);  dVb | dVw += [db_pre; dw_pre]^T TT2 -> BM_WG
         PROFB_ARRIVE(6); PHASE_SYNC(); PROFB_AFTER(g_profb_bwd, 6);
         PROF(g_prof_bwd, 26);
         LEADER_BEGIN
-            mma_k<KMAJ, KMAJ, D>(tmem + BM_DAP, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.VcT, 32, 0, 0, D, false);
+            mma_k<KMAJ, KMAJ, D>(tmem + BM_DAP, 16, sb + Lo.S[2], 128, 0, 0, sb + Lo.VcT, 32, 0, 0, D, false);
+            mma_k<KMAJ, KMAJ, D>(tmem + BM_DAP + 16, 16, sb + Lo.X - 8192, 64, 0, 0, sb + Lo.VcT, 32, r, 0, D, false);
             mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_WG, 32, sb + Lo.S[2], 128, 0, 0, sb + Lo.S[1], 128, 0, 0, LCc, !first);
-            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_WG, 32, sb + Lo.S[2], 128, 0, 64, sb + Lo.S[1], 128, 0, 64, LCc, true);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_WG, 32, sb + Lo.X, 64, 0, 0, sb + Lo.S[1], 128, 0, 64, LCc, true);
             umma_commit(&mi.bar_mma);
         LEADER_END
+        if (tid == STORE_TID) {
+            store_tile(&mdf, Lo.S[0], 8192, trow);
+            store_tile(&mdbx, Lo.S[2], 16384, trow);
+            bulk_commit();
+        }
         if (c > 0 && live) {   // next chunk's row-private L2 inputs -> L2 cache, so that the loads at its top are short
             const uint8_t* rn_ = rc - Rc.total;
 #pragma unroll
@@ -881,7 +911,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             // dz = ZZ (1 - tt^2): K side owns the erase half (cols 0..r), Q side the write half (cols r..2r)
             const int c0 = krole ? 0 : r;
             uint32_t v[16];
-            tmem_ld16(tmem + BM_DAP + lane_base + c0, v);
+            tmem_ld16(tmem + BM_DAP + lane_base + (krole ? 0 : 16), v);
             tmem_wait_ld();
             if (live) {
                 const float rnq = a.l2norm ? mi.rn[64 + t] : 1.f;
@@ -895,7 +925,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                             dz[e] = __uint_as_float(v[8 * i + e]) * (1.f - tv[e] * tv[e]);
                             dzq[e] = dz[e] * rnq;
                         }
-                        sts128(sm + Lo.S[0] + tile_chunk_off(128, 64 + t, c0 / 8 + i), pack8(dz));    // DZ rows 64..127
+                        sts128(sm + Lo.X + tile_chunk_off(64, t, c0 / 8 + i), pack8(dz));              // DZ (over dw_pre)
                         sts128(sm + Lo.S[4] + tile_chunk_off(64, t, c0 / 8 + i), pack8(dzq));          // DZQ = dz / |q|
                     }
                 }
@@ -913,15 +943,18 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mbar_wait(&mi.bar_g8, ph);
             mbar_wait(&mi.bar_g5, ph);
             tc_fence_after();
-            mma_k<KMAJ, KMAJ, 32>(tmem + BM_A, D, sb + Lo.S[0], 128, 0, 0, sb + Lo.S[5], D, 0, 32, R2, true);   // G^T: columns 32.. of the Vcat tile
+            // DZ: the tile X as the upper half of the operand; G^T: columns 32.. of the forward's Vcat tile
+            mma_k<KMAJ, KMAJ, 32>(tmem + BM_A, D, sb + Lo.X - 8192, 128, 0, 0, sb + Lo.FI + TB, D, 0, 32, R2, true);
             mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_DAP + 32, 32, sb + Lo.S[6], 64, 0, 0, sb + Lo.S[4], 64, 0, 0, LCc, false);
             umma_commit(&mi.bar_mma);
         LEADER_END
         WAIT_MMA();
         PROF(g_prof_bwd, 29);
-        if (tid == 0 && c > 0) issue_l1(c - 1);   // DZ, DZQ, GW, G^T, q are dead
+        if (tid == STORE_TID && c > 0) {   // DZQ, GW, the L1 slots are dead; d log a and dbx have left S[0] / S[2]
+            bulk_wait_read();
+            issue_l1(c - 1);
+        }
         if (!krole && warp_active) {
-            __nv_bfloat16* gdq = a.dq + ((tok0 + t) * a.H + h) * D;
 #pragma unroll
             for (int s = 0; s < HK; s += 32) {
                 uint32_t v[32];
@@ -933,7 +966,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         float f8[8];
 #pragma unroll
                         for (int e = 0; e < 8; ++e) f8[e] = __uint_as_float(v[8 * ch + e]);
-                        stg128(gdq + half * HK + s + 8 * ch, pack8(f8));
+                        sts128(sm + Lo.S[6] + tile_chunk_off(64, t, (half * HK + s) / 8 + ch), pack8(f8));   // dq^, staged over the raw q
                     }
                 }
             }
@@ -991,9 +1024,13 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         // ---- L10: the adjoint of the state entering the chunk
         PROF(g_prof_bwd, 11);
         finalize(true, c == 0);
-        if (tid == 0 && c > 0) {   // every output row of this chunk was stored before the barrier inside finalize: publish it
-            __threadfence();        // (chunk 0 is published below, after the per-chain weight-gradient partials)
-            asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.flags + chain), "r"(nchunks - c) : "memory");
+        if (tid == STORE_TID) {   // (behind the barrier inside finalize)
+            store_tile(&mdq, Lo.S[6], 8192, trow);
+            bulk_commit();
+            if (c > 0) {   // dk^ has left S[5] long ago, dq^ leaves S[6] now: the next chunk's chunk-anchored rows go there
+                bulk_wait_read();
+                issue_g3(c - 1);
+            }
         }
         PROF(g_prof_bwd, 12);
         first = false;
@@ -1016,11 +1053,10 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             if (i < R2) part[i * D + row] = __uint_as_float(wu[i]);
         }
     }
+    if (tid == STORE_TID) bulk_wait_all();
     PHASE_SYNC();
-    if (tid == 0) {   // last publish: chunk 0 AND the partials above are in memory (the reductions run behind the epilogue grid)
-        __threadfence();
-        asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(a.flags + chain), "r"(nchunks) : "memory");
-    }
+    // last publish: chunk 0 AND the partials above are in memory (the reductions run behind the epilogue grid)
+    if (tid == STORE_TID) publish(nchunks);
     if (warp == 0) tmem_dealloc(tmem, TM_COLS);
 }
 
@@ -1145,8 +1181,12 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
                           float* dVb, float* dVw, cudaStream_t st)
 {
     const int LCc = a.L < tcp::LC ? a.L : tcp::LC;
-    CUtensorMap mdO, mq;
-    if (!tc_make_token_map(&mdO, a.dO, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mq, a.q, a.B, a.T, a.H, D, LCc))
+    CUtensorMap mdO, mq, mdq, mdk, mdv, mdf, mdbx, mdwx;
+    if (!tc_make_token_map(&mdO, a.dO, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mq, a.q, a.B, a.T, a.H, D, LCc) ||
+        !tc_make_token_map(&mdq, a.dq, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mdk, a.dk_, a.B, a.T, a.H, D, LCc) ||
+        !tc_make_token_map(&mdv, a.dv_, a.B, a.T, a.H, D, LCc) || !tc_make_token_map(&mdf, a.df, a.B, a.T, a.H, D, LCc) ||
+        !tc_make_token_map(&mdbx, a.dbx, a.B, a.T, a.H, D, LCc) ||
+        !tc_make_token_map(&mdwx, a.dwx ? a.dwx : a.dv_, a.B, a.T, a.H, D, LCc))   // (scalar-write variant: the map is never used)
         return cudaErrorInvalidValue;
     BwdArgs t{};
     t.B = a.B; t.H = a.H; t.T = a.T; t.L = a.L; t.r = a.r; t.l2norm = a.l2norm; t.scale = a.scale; t.eps = a.eps;
@@ -1166,7 +1206,7 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
     if (e != cudaSuccess) return e;
     const int chains = a.B * a.H, nchunks = a.T / LCc;
     if ((e = cudaMemsetAsync(t.flags, 0, (size_t)chains * sizeof(int), st)) != cudaSuccess) return e;
-    kern<<<chains, 128 * NP, smem, st>>>(t, mdO, mq);
+    kern<<<chains, 128 * NP, smem, st>>>(t, mdO, mq, mdq, mdk, mdv, mdf, mdbx, mdwx);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     float* partAT = reinterpret_cast<float*>(ws + w.partAT);
     {
