@@ -385,41 +385,35 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             mbar_wait(&mi.bar_g1, ph);
             mbar_wait(&mi.bar_pt, ph);
             tc_fence_after();
-            mma_k<KMAJ, KMAJ, D>(tmem + BM_A, D, sb + Lo.S[0], 64, 0, 0, sb + Lo.DSB, D, 0, 0, D, false);
-            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_A, D, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[2], 128, 0, 64, LCc, true);
+            // dU^T (lanes x, columns s): all 128 lanes carry results (as dU, lanes = tokens, half of the M = 128 rows were junk)
+            mma_k<KMAJ, KMAJ, D>(tmem + BM_A, 64, sb + Lo.DSB, D, 0, 0, sb + Lo.S[0], 64, 0, 0, D, false);
+            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_A, 64, sb + Lo.S[2], 128, 0, 64, sb + Lo.S[1], 128, 0, 0, LCc, true);
             mma_k<KMAJ, MNMAJ, D>(tmem + BM_KT, D, sb + Lo.S[4], 64, 0, 0, sb + Lo.DSB, D, 0, 0, D, false);
             umma_commit(&mi.bar_mma);
         LEADER_END
-        if (krole) {
-            WAIT_MMA();
-            PROF(g_prof_bwd, 13);
-            if (warp_active) {
+        WAIT_MMA();
+        PROF(g_prof_bwd, 13);
+        if (srow) {   // dU^T -> bf16 [D][64] tile DUT (S[0], over Ktil): 64 / NP columns per thread
+            constexpr int UW = 64 / NP;
+            uint32_t v[UW];
+            if constexpr (UW == 32) tmem_ld32(tmem + BM_A + lane_base + UW * half, v);
+            else tmem_ld16(tmem + BM_A + lane_base + UW * half, v);
+            tmem_wait_ld();
 #pragma unroll
-                for (int s = 0; s < HK; s += 32) {
-                    uint32_t v[32];
-                    tmem_ld32(tmem + BM_A + lane_base + half * HK + s, v);
-                    tmem_wait_ld();
-                    if (live) {
+            for (int ch = 0; ch < UW / 8; ++ch) {
+                float f8[8];
 #pragma unroll
-                        for (int ch = 0; ch < 4; ++ch) {
-                            float f8[8];
-#pragma unroll
-                            for (int e = 0; e < 8; ++e) f8[e] = __uint_as_float(v[8 * ch + e]);
-                            sts128(sm + Lo.S[0] + tile_chunk_off(64, t, (half * HK + s) / 8 + ch), pack8(f8));  // DU over Ktil
-                        }
-                    }
-                }
+                for (int e = 0; e < 8; ++e) f8[e] = __uint_as_float(v[8 * ch + e]);
+                sts128(sm + Lo.S[0] + tile_chunk_off(D, row, (UW / 8) * half + ch), pack8(f8));
             }
-        } else {
-            mma_ph ^= 1u;  // Q-side threads skip this wait
         }
         PROF(g_prof_bwd, 1);
         // ---- L2: dX = T^T dU: columns x < D/2 -> BM_A rows 0..63 (K-side lanes), x >= D/2 -> rows 64..127 (Q-side lanes)
         PROFB_ARRIVE(0); PHASE_SYNC(); PROFB_AFTER(g_profb_bwd, 0);
         PROF(g_prof_bwd, 14);
         LEADER_BEGIN
-            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_A + D / 2, D / 2, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[0], 64, D / 2, 0, LCc, false);
-            mma_k<MNMAJ, MNMAJ, LC>(tmem + BM_A, D / 2, sb + Lo.S[1], 64, 64, 0, sb + Lo.S[0], 64, 0, 0, LCc, false);
+            mma_k<MNMAJ, KMAJ, LC>(tmem + BM_A + D / 2, D / 2, sb + Lo.S[1], 64, 0, 0, sb + Lo.S[0], D, D / 2, 0, LCc, false);
+            mma_k<MNMAJ, KMAJ, LC>(tmem + BM_A, D / 2, sb + Lo.S[1], 64, 64, 0, sb + Lo.S[0], D, 0, 0, LCc, false);
             umma_commit(&mi.bar_mma);
         LEADER_END
         WAIT_MMA();
@@ -497,15 +491,14 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             if constexpr (DW == 32) tmem_ld32(tmem + BM_DAP + lane_base + DW * half, v);
             else tmem_ld16(tmem + BM_DAP + lane_base + DW * half, v);
             tmem_wait_ld();
+            // keep s < t (K side) / s <= t (Q side, scaled): branch-free, one compare against a per-thread limit
+            const float scl = krole ? 1.f : a.scale;
+            const int lim = (live ? (krole ? t : t + 1) : 0) - DW * half;   // keep local column i iff i < lim
 #pragma unroll
             for (int ch = 0; ch < DW / 8; ++ch) {
                 float f8[8];
 #pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int s = DW * half + 8 * ch + e;
-                    const bool keep = live && (krole ? s < t : s <= t);
-                    f8[e] = keep ? (krole ? __uint_as_float(v[8 * ch + e]) : a.scale * __uint_as_float(v[8 * ch + e])) : 0.f;
-                }
+                for (int e = 0; e < 8; ++e) f8[e] = (8 * ch + e < lim) ? scl * __uint_as_float(v[8 * ch + e]) : 0.f;
                 sts128(sm + Lo.S[4] + tile_chunk_off(128, row, (DW / 8) * half + ch), pack8(f8));
             }
         }
@@ -693,9 +686,12 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                         carry += tot;
                     }
                 }
-            if (tid == STORE_TID) {   // dv has left S[0] (dlp goes there below); every store of the previous chunk is complete
-                bulk_wait_all();
-                if (it > 0) publish(it);
+            if (tid == STORE_TID) {
+                bulk_wait_read();   // dv has left S[0] (dlp goes there below)
+                if (it > 0) {       // all but the newest group (dv | dwx of this chunk): the previous chunk's stores are complete
+                    bulk_wait_all_but<1>();
+                    publish(it);
+                }
             }
             PROFB_ARRIVE(3); __syncthreads(); PROFB_AFTER(g_profb_bwd, 3);  // every warp is done reading DAP / C / KQo
             PROF(g_prof_bwd, 21);
@@ -826,13 +822,16 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
             bulk_g2s(sm + Lo.FI + TB, rc + Rc.GT, tile_bytes(D, 64), &mi.bar_g8);
             mbar_expect_tx(&mi.bar_g5, (uint32_t)LCc * D * 2u);
             for (int cb = 0; cb < D / 64; ++cb) tma_load_3d(sm + Lo.S[6] + cb * 8192, &mq, &mi.bar_g5, cb * 64, h, trow);
-            mbar_expect_tx(&mi.bar_bg, TB);   // the erase gate b over gamma_t/gamma_a (dead after L5)
-            bulk_g2s(sm + Lo.FI, rc + Rc.Bg, TB, &mi.bar_bg);
         LEADER_END
         if (tid == STORE_TID) { store_tile(&mdk, Lo.S[5], 8192, trow); bulk_commit(); }
         {
-            // [tt_b|0 ; 0|tt_w] -> S[1]: Q-side threads, loads first
-            uint4 t4[4];
+            // the erase gate b of this thread's columns (row-private, L2-prefetched in L4) and, Q-side threads,
+            // [tt_b|0 ; 0|tt_w] -> S[1]: global loads issued before the wait
+            uint4 b4[QW / 8], t4[4];
+            if (live) {
+#pragma unroll
+                for (int i = 0; i < QW / 8; ++i) b4[i] = ldg128(rc + Rc.Bg + rp_off(t, cq0 + i));
+            }
             if (!krole && live) {
 #pragma unroll
                 for (int i = 0; i < 4; ++i)   // packed chunk i of [tt_b | tt_w] -> chunk of the forward's tile (each half padded to 16 columns)
@@ -851,7 +850,6 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                     else if (half == 1) sts128(sm + Lo.S[1] + tile_chunk_off(128, 64 + t, i), is_w ? t4[i] : z4);
                 }
             }
-            mbar_wait(&mi.bar_bg, ph);
             PROF(g_prof_bwd, 25);
             if (warp_active) {
                 uint32_t v[QW];
@@ -863,7 +861,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
                     for (int i = 0; i < QW / 8; ++i) {
                         const int cc = cq0 + i;
                         float bb[8], dp[8], xq[8], dla[8], dbp[8];
-                        unpack8(lds128(sm + Lo.FI + rp_off(t, cc)), bb);
+                        unpack8(b4[i], bb);
                         unpack8(lds128(sm + Lo.S[0] + tile_chunk_off(64, t, cc)), dp);
                         unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc)), xq);   // the t' = t term of XQ
 #pragma unroll
@@ -907,32 +905,30 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         }
         WAIT_MMA();
         PROF(g_prof_bwd, 27);
-        if (half == 0 && warp_active) {
-            // dz = ZZ (1 - tt^2): K side owns the erase half (cols 0..r), Q side the write half (cols r..2r)
+        if (warp_active) {
+            // dz = ZZ (1 - tt^2): K side owns the erase half (cols 0..r), Q side the write half (cols r..2r); column part
+            // `half` takes the 8 columns [8 half, 8 half + 8) of its side
             const int c0 = krole ? 0 : r;
-            uint32_t v[16];
-            tmem_ld16(tmem + BM_DAP + lane_base + (krole ? 0 : 16), v);
-            tmem_wait_ld();
-            if (live) {
-                const float rnq = a.l2norm ? mi.rn[64 + t] : 1.f;
+            if (half < (r >> 3)) {
+                uint32_t v[8];
+                tmem_ld8(tmem + BM_DAP + lane_base + (krole ? 0 : 16) + 8 * half, v);
+                tmem_wait_ld();
+                if (live) {
+                    const float rnq = a.l2norm ? mi.rn[64 + t] : 1.f;
+                    float tv[8], dz[8], dzq[8];
+                    unpack8(lds128(sm + Lo.S[1] + tile_chunk_off(128, krole ? t : 64 + t, c0 / 8 + half)), tv);
 #pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    if (i < (r >> 3)) {
-                        float tv[8], dz[8], dzq[8];
-                        unpack8(lds128(sm + Lo.S[1] + tile_chunk_off(128, krole ? t : 64 + t, c0 / 8 + i)), tv);
-#pragma unroll
-                        for (int e = 0; e < 8; ++e) {
-                            dz[e] = __uint_as_float(v[8 * i + e]) * (1.f - tv[e] * tv[e]);
-                            dzq[e] = dz[e] * rnq;
-                        }
-                        sts128(sm + Lo.X + tile_chunk_off(64, t, c0 / 8 + i), pack8(dz));              // DZ (over dw_pre)
-                        sts128(sm + Lo.S[4] + tile_chunk_off(64, t, c0 / 8 + i), pack8(dzq));          // DZQ = dz / |q|
+                    for (int e = 0; e < 8; ++e) {
+                        dz[e] = __uint_as_float(v[e]) * (1.f - tv[e] * tv[e]);
+                        dzq[e] = dz[e] * rnq;
                     }
+                    sts128(sm + Lo.X + tile_chunk_off(64, t, c0 / 8 + half), pack8(dz));      // DZ (over dw_pre)
+                    sts128(sm + Lo.S[4] + tile_chunk_off(64, t, c0 / 8 + half), pack8(dzq));   // DZQ = dz / |q|
                 }
-                if (!krole) {  // zero the unused columns [2r, 32) of DZQ (the dG product has N = 32)
-                    const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
-                    for (int i = 2 * (r >> 3); i < 4; ++i) sts128(sm + Lo.S[4] + tile_chunk_off(64, t, i), z4);
-                }
+            }
+            if (!krole && live) {  // zero the unused columns [2r, 32) of DZQ (the dG product has N = 32)
+                const uint4 z4 = make_uint4(0u, 0u, 0u, 0u);
+                for (int i = 2 * (r >> 3) + half; i < 4; i += NP) sts128(sm + Lo.S[4] + tile_chunk_off(64, t, i), z4);
             }
         }
         PROF(g_prof_bwd, 8);

@@ -33,7 +33,9 @@
         prof_s_[(threadIdx.x ? 40 : 0) + i] += (unsigned long long)(prof_n_ - prof_t_); \
         prof_t_ = prof_n_;                                                         \
     }
-// barrier-spread profile: per barrier site and warp, how long the warp waited for the last one to arrive
+// barrier-spread profile (-DCARVE_PROFILE_BARRIERS as well: its own overhead is ~1 K cycles per site, so the per-phase
+// counters are read from a build without it): per barrier site and warp, how long the warp waited for the last one
+#ifdef CARVE_PROFILE_BARRIERS
 #define PROFB_DECL(name) static __device__ unsigned long long name[64 * 16];
 #define PROFB_ARRIVE(site) if ((threadIdx.x & 31) == 0) prof_arr_[(site) & 1][threadIdx.x >> 5] = clock64();
 #define PROFB_AFTER(name, site)                                                                     \
@@ -42,6 +44,11 @@
         for (int w_ = 0; w_ < (int)(blockDim.x >> 5); ++w_) mx_ = mx_ > prof_arr_[(site) & 1][w_] ? mx_ : prof_arr_[(site) & 1][w_]; \
         atomicAdd(&name[(site) * 16 + (threadIdx.x >> 5)], (unsigned long long)(mx_ - prof_arr_[(site) & 1][threadIdx.x >> 5])); \
     }
+#else
+#define PROFB_DECL(name) static __device__ unsigned long long name[64 * 16];
+#define PROFB_ARRIVE(site)
+#define PROFB_AFTER(name, site)
+#endif
 #define PROF_FLUSH(name)                                                           \
     __syncthreads();                                                               \
     if (blockIdx.x == 0 && threadIdx.x < 80) name[threadIdx.x] += prof_s_[threadIdx.x];
@@ -147,6 +154,9 @@ __device__ __forceinline__ void bulk_s2g(void* gdst, uint32_t src_saddr, uint32_
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+// every bulk group of this thread except the N most recent ones is complete (writes performed)
+template <int N>
+__device__ __forceinline__ void bulk_wait_all_but() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
 
 // ---- TMEM ----------------------------------------------------------------------------------------
 // One full warp allocates `ncols` (power of two >= 32) columns; the base address lands in *dst (smem).
