@@ -219,6 +219,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     const Rec Rc(D, D);
     const uint8_t* rec_chain = a.rec + (size_t)chain * nchunks * Rc.total;
 
+    PROF_INIT();
     // ---- one-time setup --------------------------------------------------------------------------
     if (tid == 0) {
         mbar_init(&mi.bar_mma, 1); mbar_init(&mi.bar_g1, 1); mbar_init(&mi.bar_g3, 1); mbar_init(&mi.bar_sb, 1);
@@ -331,7 +332,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     // now on the SMs this grid leaves idle; it follows the per-chain progress flags written below.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     bool first = true, first_glue = true;
-    PROF_INIT();
+    PROF(g_prof_bwd, 38);   // one-time setup
     for (int it = 0, c = nchunks - 1; c >= 0; --c, ++it) {
         const uint32_t ph = (uint32_t)it & 1u;
         const uint8_t* rc = rec_chain + (size_t)c * Rc.total;
@@ -742,30 +743,30 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
 #pragma unroll
                         for (int ch = 0; ch < 2; ++ch) {
                             const int i = s / 8 + ch, cc = half * (HK / 8) + i, j0 = 8 * cc;
-                            float fp[8], ic[8], pk[8], pc[8], k0[8], c8[8], o[8], xa[8], zz[8];
-                            unpack8(bstart ? ones4 : lds128(sm + Lo.FI + rp_off(t - 1, cc)), fp);
-                            unpack8(lds128(sm + Lo.FI + TB + rp_off(t, cc)), ic);
-                            unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, t, cc)), pk);
-                            unpack8(lds128(sm + Lo.S[4] + tile_chunk_off(64, t, cc)), pc);
-                            unpack8(lds128(sm + Lo.S[5] + tile_chunk_off(64, t, cc)), k0);
-                            unpack8(lds128(sm + Lo.S[1] + tile_chunk_off(64, t, cc)), c8);
-                            float pre[8], suf[8];   // gamma_a(blk)/gamma_{-1} and gamma_L/gamma_a(blk)
+                            float2 fp[4], ic[4], pk[4], pc[4], k0[4], c8[4], o[4], xa[4], zz[4];
+                            unpack8p(bstart ? ones4 : lds128(sm + Lo.FI + rp_off(t - 1, cc)), fp);
+                            unpack8p(lds128(sm + Lo.FI + TB + rp_off(t, cc)), ic);
+                            unpack8p(lds128(sm + Lo.S[2] + tile_chunk_off(128, t, cc)), pk);
+                            unpack8p(lds128(sm + Lo.S[4] + tile_chunk_off(64, t, cc)), pc);
+                            unpack8p(lds128(sm + Lo.S[5] + tile_chunk_off(64, t, cc)), k0);
+                            unpack8p(lds128(sm + Lo.S[1] + tile_chunk_off(64, t, cc)), c8);
+                            float2 pre[4], suf[4];   // gamma_a(blk)/gamma_{-1} and gamma_L/gamma_a(blk)
                             *reinterpret_cast<float4*>(pre) = *reinterpret_cast<const float4*>(&mi.pre[blk][j0]);
-                            *reinterpret_cast<float4*>(pre + 4) = *reinterpret_cast<const float4*>(&mi.pre[blk][j0 + 4]);
+                            *reinterpret_cast<float4*>(pre + 2) = *reinterpret_cast<const float4*>(&mi.pre[blk][j0 + 4]);
                             *reinterpret_cast<float4*>(suf) = *reinterpret_cast<const float4*>(&mi.suf[blk][j0]);
-                            *reinterpret_cast<float4*>(suf + 4) = *reinterpret_cast<const float4*>(&mi.suf[blk][j0 + 4]);
+                            *reinterpret_cast<float4*>(suf + 2) = *reinterpret_cast<const float4*>(&mi.suf[blk][j0 + 4]);
 #pragma unroll
-                            for (int e = 0; e < 8; ++e) {
-                                const float sp = __uint_as_float(vs[8 * ch + e]), dkt = __uint_as_float(vk[8 * ch + e]);
-                                const float dkA = fp[e] * (pk[e] + pre[e] * sp);
-                                const float dkC = ic[e] * (pc[e] + suf[e] * dkt);
-                                o[e] = dkA + dkC;
-                                xa[e] = k0[e] * sp;                 // Kbar_t . dKbar_t (state read), to d log gamma_{t-1}
-                                zz[e] = (c8[e] * suf[e]) * dkt;     // Ktil_t . dKtil_t (state write), to d log gamma_t' for t' > t
+                            for (int e = 0; e < 4; ++e) {
+                                const float2 sp = pair_of(vs + 8 * ch + 2 * e), dkt = pair_of(vk + 8 * ch + 2 * e);
+                                const float2 dkA = mul2(fp[e], fma2(pre[e], sp, pk[e]));
+                                const float2 dkC = mul2(ic[e], fma2(suf[e], dkt, pc[e]));
+                                o[e] = add2(dkA, dkC);
+                                xa[e] = mul2(k0[e], sp);                      // Kbar_t . dKbar_t (state read), to d log gamma_{t-1}
+                                zz[e] = mul2(mul2(c8[e], suf[e]), dkt);       // Ktil_t . dKtil_t (state write), to d log gamma_t' for t' > t
                             }
-                            sts128(sm + Lo.S[5] + tile_chunk_off(64, t, cc), pack8(o));    // dk^, staged in place over Kbar_t
-                            sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8(xa));   // in place over H_t
-                            sts128(sm + Lo.S[4] + tile_chunk_off(64, t, cc), pack8(zz));    // in place over H'_t
+                            sts128(sm + Lo.S[5] + tile_chunk_off(64, t, cc), pack8p(o));    // dk^, staged in place over Kbar_t
+                            sts128(sm + Lo.S[2] + tile_chunk_off(128, t, cc), pack8p(xa));   // in place over H_t
+                            sts128(sm + Lo.S[4] + tile_chunk_off(64, t, cc), pack8p(zz));    // in place over H'_t
                         }
                     }
                 }
@@ -779,20 +780,21 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
 #pragma unroll
                         for (int ch = 0; ch < 2; ++ch) {
                             const int i = s / 8 + ch, cc = half * (HK / 8) + i, j0 = 8 * cc;
-                            float fq[8], pq[8], q0[8], xq[8];
-                            unpack8(lds128(sm + Lo.FI + rp_off(t, cc)), fq);
-                            unpack8(lds128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc)), pq);
-                            unpack8(lds128(sm + Lo.S[6] + tile_chunk_off(64, t, cc)), q0);
-                            float pre[8];
+                            float2 fq[4], pq[4], q0[4], xq[4], pre[4];
+                            unpack8p(lds128(sm + Lo.FI + rp_off(t, cc)), fq);
+                            unpack8p(lds128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc)), pq);
+                            unpack8p(lds128(sm + Lo.S[6] + tile_chunk_off(64, t, cc)), q0);
                             *reinterpret_cast<float4*>(pre) = *reinterpret_cast<const float4*>(&mi.pre[blk][j0]);
-                            *reinterpret_cast<float4*>(pre + 4) = *reinterpret_cast<const float4*>(&mi.pre[blk][j0 + 4]);
+                            *reinterpret_cast<float4*>(pre + 2) = *reinterpret_cast<const float4*>(&mi.pre[blk][j0 + 4]);
+                            const float2 sc2 = splat2(a.scale);
 #pragma unroll
-                            for (int e = 0; e < 8; ++e) {
-                                const float sp = __uint_as_float(vs[8 * ch + e]);
-                                vs[8 * ch + e] = __float_as_uint(fq[e] * (pq[e] + pre[e] * a.scale * sp));
-                                xq[e] = q0[e] * sp;                 // scale Qbar_t . (dO S)_t (state read)
+                            for (int e = 0; e < 4; ++e) {
+                                const float2 sp = pair_of(vs + 8 * ch + 2 * e);
+                                const float2 dqv = mul2(fq[e], fma2(mul2(pre[e], sc2), sp, pq[e]));
+                                vs[8 * ch + 2 * e] = __float_as_uint(dqv.x); vs[8 * ch + 2 * e + 1] = __float_as_uint(dqv.y);
+                                xq[e] = mul2(q0[e], sp);            // scale Qbar_t . (dO S)_t (state read)
                             }
-                            sts128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc), pack8(xq));   // in place over H_t
+                            sts128(sm + Lo.S[2] + tile_chunk_off(128, 64 + t, cc), pack8p(xq));   // in place over H_t
                         }
                     }
                     tmem_st16(tmem + BM_A + lane_base + half * HK + s, vs);   // dq^ state part, completed by the L8 MMA
@@ -1032,7 +1034,6 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
         first = false;
     }
 
-    PROF_FLUSH(g_prof_bwd)
     // ---- per-chain partial weight gradients: [dUb|dUw][dVb][dVw] (dA, dtau come from the epilogue kernel)
     if (half == 0 && srow) {
         float* part = a.part + (size_t)chain * a.part_stride;
@@ -1053,6 +1054,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     PHASE_SYNC();
     // last publish: chunk 0 AND the partials above are in memory (the reductions run behind the epilogue grid)
     if (tid == STORE_TID) publish(nchunks);
+    PROF(g_prof_bwd, 39);   // per-chain partials, last publish
+    PROF_FLUSH(g_prof_bwd)
     if (warp == 0) tmem_dealloc(tmem, TM_COLS);
 }
 
@@ -1062,20 +1065,32 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
 //   df = dla . (-exp A) sigmoid(f + tau)            (Eq. 9 l.151), and the per-chunk partial sums of
 //   dtau = sum df,  dA = sum dla . g  with g = -exp(A) softplus(f + tau).
 template <int D>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 carve_bwd_tc_epilogue_kernel(const __nv_bfloat16* __restrict__ gq, const __nv_bfloat16* __restrict__ gk,
                              const __nv_bfloat16* __restrict__ gf, const float* __restrict__ A,
                              const float* __restrict__ tau, __nv_bfloat16* dq, __nv_bfloat16* dk, __nv_bfloat16* df,
                              float* __restrict__ partAT, int T, int H, int LCc, int l2norm, float eps, const int* flags,
                              int chains)
 {
-    constexpr int V = D / 32;   // channels per lane
+    // A lane owns 8 channels (one 16-byte piece) of a row; a warp covers RPW rows per load.  All six loads of a row
+    // group are issued before anything is computed or stored (the in-place stores would otherwise order every later
+    // load behind them): per SM this grid runs on the few SMs the reverse kernel leaves idle, so what counts is the
+    // number of bytes a warp keeps in flight, not the DRAM bandwidth of the whole machine.
+    constexpr int LPR = D / 8, RPW = 32 / LPR, NIT = 64 / (8 * RPW), UN = 1;
     __shared__ float red[8][2][D];
     const int nchunks = T / LCc;
     // blocks in the order the reverse kernel finishes chunks (last chunk of every chain first): this grid may already
     // run, on idle SMs, while the reverse kernel works; a block waits for "its" chunk through the chain's progress flag
     const int c = nchunks - 1 - (int)(blockIdx.x / chains), chain = blockIdx.x % chains, b = chain / H, h = chain % H;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, sub = lane / LPR, l = lane % LPR;
+    float eA[8], ta[8], accA[8], accT[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+        const int j = l * 8 + e;
+        eA[e] = A ? __expf(__ldg(A + h * D + j)) : 1.f;
+        ta[e] = tau ? __ldg(tau + h * D + j) : 0.f;
+        accA[e] = accT[e] = 0.f;
+    }
     if (threadIdx.x == 0) {
         int done;
         do {
@@ -1084,71 +1099,80 @@ carve_bwd_tc_epilogue_kernel(const __nv_bfloat16* __restrict__ gq, const __nv_bf
         } while (done < nchunks - c);
     }
     __syncthreads();
-    float eA[V], ta[V], accA[V], accT[V];
+    auto gsum = [](float x) {   // sum over the LPR lanes of a row
 #pragma unroll
-    for (int e = 0; e < V; ++e) {
-        const int j = lane * V + e;
-        eA[e] = A ? __expf(__ldg(A + h * D + j)) : 1.f;
-        ta[e] = tau ? __ldg(tau + h * D + j) : 0.f;
-        accA[e] = accT[e] = 0.f;
-    }
-    auto load = [&](const __nv_bfloat16* p, float (&o)[V]) {
-        if constexpr (V == 4) {
-            const uint2 w = *reinterpret_cast<const uint2*>(p);
-            o[0] = bf16_lo(w.x); o[1] = bf16_hi(w.x); o[2] = bf16_lo(w.y); o[3] = bf16_hi(w.y);
-        } else {
-            const uint32_t w = *reinterpret_cast<const uint32_t*>(p);
-            o[0] = bf16_lo(w); o[1] = bf16_hi(w);
-        }
-    };
-    auto store = [&](__nv_bfloat16* p, const float (&o)[V]) {
-        if constexpr (V == 4) *reinterpret_cast<uint2*>(p) = make_uint2(pack_bf16(o[0], o[1]), pack_bf16(o[2], o[3]));
-        else *reinterpret_cast<uint32_t*>(p) = pack_bf16(o[0], o[1]);
-    };
-    auto wsum = [](float x) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xFFFFFFFFu, x, o);
+        for (int o = LPR / 2; o > 0; o >>= 1) x += __shfl_xor_sync(0xFFFFFFFFu, x, o);
         return x;
     };
-    for (int tt_ = warp; tt_ < LCc; tt_ += 8) {
-        const size_t ro = (((size_t)b * T + (size_t)c * LCc + tt_) * H + h) * D + lane * V;
-        if (l2norm) {
-            float x[V], dx[V];
+    const size_t row0 = ((size_t)b * T + (size_t)c * LCc) * H + h;
 #pragma unroll
-            for (int which = 0; which < 2; ++which) {
-                const __nv_bfloat16* src = which ? gk : gq;
-                __nv_bfloat16* dst = which ? dk : dq;
-                load(src + ro, x);
-                load(dst + ro, dx);
-                float ss = 0.f;
+    for (int i0 = 0; i0 < NIT; i0 += UN) {
+        uint4 in[UN][6];
+        size_t ro[UN];
+        bool on[UN];
 #pragma unroll
-                for (int e = 0; e < V; ++e) ss += x[e] * x[e];
-                const float rn = rsqrtf(wsum(ss) + eps);
-                float dot = 0.f;
+        for (int u = 0; u < UN; ++u) {
+            const int tt_ = ((i0 + u) * 8 + warp) * RPW + sub;
+            on[u] = tt_ < LCc;
+            ro[u] = (row0 + (size_t)(on[u] ? tt_ : 0) * H) * D + l * 8;
+            const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+            in[u][0] = l2norm ? *reinterpret_cast<const uint4*>(gq + ro[u]) : z;
+            in[u][1] = l2norm ? *reinterpret_cast<const uint4*>(dq + ro[u]) : z;
+            in[u][2] = l2norm ? *reinterpret_cast<const uint4*>(gk + ro[u]) : z;
+            in[u][3] = l2norm ? *reinterpret_cast<const uint4*>(dk + ro[u]) : z;
+            in[u][4] = *reinterpret_cast<const uint4*>(gf + ro[u]);
+            in[u][5] = *reinterpret_cast<const uint4*>(df + ro[u]);
+        }
 #pragma unroll
-                for (int e = 0; e < V; ++e) { x[e] *= rn; dot += x[e] * dx[e]; }
-                dot = wsum(dot);
+        for (int u = 0; u < UN; ++u) {
+            if (l2norm) {
 #pragma unroll
-                for (int e = 0; e < V; ++e) dx[e] = (dx[e] - x[e] * dot) * rn;
-                store(dst + ro, dx);
+                for (int which = 0; which < 2; ++which) {
+                    float x[8], dx[8];
+                    unpack8(in[u][2 * which], x);
+                    unpack8(in[u][2 * which + 1], dx);
+                    float ss = 0.f;
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) ss += x[e] * x[e];
+                    const float rn = rsqrtf(gsum(ss) + eps);
+                    float dot = 0.f;
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) { x[e] *= rn; dot += x[e] * dx[e]; }
+                    dot = gsum(dot);
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) dx[e] = (dx[e] - x[e] * dot) * rn;
+                    if (on[u]) *reinterpret_cast<uint4*>((which ? dk : dq) + ro[u]) = pack8(dx);
+                }
             }
-        }
-        float fv[V], dla[V];
-        load(gf + ro, fv);
-        load(df + ro, dla);
+            float fv[8], dla[8];
+            unpack8(in[u][4], fv);
+            unpack8(in[u][5], dla);
 #pragma unroll
-        for (int e = 0; e < V; ++e) {
-            const float z = fv[e] + ta[e];
-            const float sg = sigmoid_fast(z), sp = softplus_fast(z);
-            const float d = dla[e] * (-eA[e]) * sg;
-            accT[e] += d;
-            accA[e] += dla[e] * (-eA[e] * sp);
-            dla[e] = d;
+            for (int e = 0; e < 8; ++e) {
+                // sigmoid and softplus of the same argument share exp(-|z|): 3 transcendental ops, not 4
+                const float z = fv[e] + ta[e];
+                const float ex = ex2_ftz(-fabsf(z) * kLog2e), s1p = 1.f + ex, rs = rcp_ftz(s1p);
+                const float sg = z >= 0.f ? rs : ex * rs;
+                const float sp = fmaf(kLn2, lg2_ftz(s1p), fmaxf(z, 0.f));
+                const float d = dla[e] * (-eA[e]) * sg;
+                if (on[u]) {
+                    accT[e] += d;
+                    accA[e] += dla[e] * (-eA[e] * sp);
+                }
+                dla[e] = d;
+            }
+            if (on[u]) *reinterpret_cast<uint4*>(df + ro[u]) = pack8(dla);
         }
-        store(df + ro, dla);
     }
 #pragma unroll
-    for (int e = 0; e < V; ++e) { red[warp][0][lane * V + e] = accA[e]; red[warp][1][lane * V + e] = accT[e]; }
+    for (int e = 0; e < 8; ++e) {   // rows of the warp -> one partial per channel
+#pragma unroll
+        for (int o = LPR; o < 32; o <<= 1) {
+            accA[e] += __shfl_xor_sync(0xFFFFFFFFu, accA[e], o);
+            accT[e] += __shfl_xor_sync(0xFFFFFFFFu, accT[e], o);
+        }
+        if (sub == 0) { red[warp][0][l * 8 + e] = accA[e]; red[warp][1][l * 8 + e] = accT[e]; }
+    }
     __syncthreads();
     for (int i = threadIdx.x; i < 2 * D; i += 256) {
         float s = 0.f;

@@ -228,6 +228,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     const bool warp_active = (q & 1) * 32 < LCc;  // this warp holds at least one live token row
     const bool live = t < LCc;
 
+    PROF_INIT();
     // ---- one-time setup --------------------------------------------------------------------------
     if (tid == 0) {
         mbar_init(&mi.bar_mma, 1); mbar_init(&mi.bar_acc, 1); mbar_init(&mi.bar_kq, 1); mbar_init(&mi.bar_fb, 1); mbar_init(&mi.bar_wv, 1);
@@ -327,7 +328,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     // (kept as raw bf16 bits until it is used, one chunk later: converting it here would make the warp wait for the load)
     const unsigned short* beta_bits = reinterpret_cast<const unsigned short*>(a.beta);
     uint32_t beta_nx = (krole && half == 0 && live) ? (uint32_t)__ldg(beta_bits + ((size_t)b * a.T + t) * a.H + h) : 0u;
-    PROF_INIT();
+    PROF(g_prof_fwd, 38);   // one-time setup
     for (int c = 0; c < nchunks; ++c) {
         const bool fold_now = (c % gate_every) == 0;
         const size_t tok0 = (size_t)b * a.T + (size_t)c * LCc;  // first token of the chunk
@@ -909,7 +910,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         tma_ph ^= 1u;
         PROF(g_prof_fwd, 17);
     }
-    PROF_FLUSH(g_prof_fwd)
     if (VS > 1) cluster_wait();   // pairs with the last arrive; also keeps this CTA's shared memory alive for the peer
     PHASE_SYNC();
     if (tid == 0) {   // the last chunk's outputs
@@ -918,6 +918,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         bulk_wait_all();
     }
     if (rec_chain && (tid == 0 || tid == REC_TID)) bulk_wait_all();   // drain the record's bulk stores
+    PROF(g_prof_fwd, 39);   // last output tile, drain
+    PROF_FLUSH(g_prof_fwd)
     if (warp == 0) tmem_dealloc(tmem, TM_COLS);
 }
 
