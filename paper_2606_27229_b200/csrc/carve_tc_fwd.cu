@@ -501,20 +501,22 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 const int cc = cc0 + ci;
                 const uint32_t off = tile_chunk_off(64, t, cc);
                 if (live && !SW) {
-                    float fw[8], fv[8];
-                    unpack8(lds128(sm + Lo.WX + off), fw);
-                    unpack8(lds128(sm + Lo.V + off), fv);
+                    float2 fw[4], fv[4];
+                    unpack8p(lds128(sm + Lo.WX + off), fw);
+                    unpack8p(lds128(sm + Lo.V + off), fv);
+                    const float2 h2 = splat2(0.5f);
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        fw[e] = sigmoid_tanh(fw[e] + __uint_as_float(pw16[8 * ci + e]));
-                        fv[e] *= fw[e];
+                    for (int e = 0; e < 4; ++e) {   // w = sigmoid(wx + w_proj) through one tanh.approx per element (sigmoid_tanh)
+                        const float2 x = mul2(add2(fw[e], pair_of(pw16 + 8 * ci + 2 * e)), h2);
+                        fw[e] = fma2(make_float2(tanh_fast(x.x), tanh_fast(x.y)), h2, h2);
+                        fv[e] = mul2(fv[e], fw[e]);
                     }
-                    sts128(sm + Lo.V + off, pack8(fv));
+                    sts128(sm + Lo.V + off, pack8p(fv));
                     if (rc) {
-                        *reinterpret_cast<uint4*>(rc + Rc.W + rp_off(t, cc)) = pack8(fw);
+                        *reinterpret_cast<uint4*>(rc + Rc.W + rp_off(t, cc)) = pack8p(fw);
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) fv[e] *= 1.f - fw[e];
-                        *reinterpret_cast<uint4*>(rc + Rc.VWX + rp_off(t, cc)) = pack8(fv);
+                        for (int e = 0; e < 4; ++e) fv[e] = mul2(fv[e], fma2(fw[e], splat2(-1.f), splat2(1.f)));
+                        *reinterpret_cast<uint4*>(rc + Rc.VWX + rp_off(t, cc)) = pack8p(fv);
                     }
                 }
                 float fb[8], ff[8], bg[8], ea[8], ta[8];
@@ -593,82 +595,92 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 for (int ci = 0; ci < 2; ++ci) {
                     const int cc = cc0 + ci;
                     if (live) {
-                        float Fp[8], qv[8], kv[8], o[8];
+                        float2 Fp[4], qv[4], kv[4], o[4];
                         {   // column operand C_t, Ktil_t (own anchor), gamma_a/gamma_t >= 1
-                            float kt[8], o1[8], o2[8], ic[8], et[8], sf[8];
-                            unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, t, cc)), kt);
+                            float2 kt[4], o1[4], o2[4], ic[4], et[4], sf[4];
+                            unpack8p(lds128(sm + Lo.KQraw + tile_chunk_off(128, t, cc)), kt);
                             *reinterpret_cast<float4*>(et) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc]);
-                            *reinterpret_cast<float4*>(et + 4) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc + 4]);
+                            *reinterpret_cast<float4*>(et + 2) = *reinterpret_cast<const float4*>(&mi.etot[blk][8 * cc + 4]);
 #pragma unroll
-                            for (int e = 0; e < 8; ++e) sf[e] = 1.f;   // gamma_L / gamma_e(blk): product of etot[b'] over b' > blk
+                            for (int e = 0; e < 4; ++e) sf[e] = splat2(1.f);   // gamma_L / gamma_e(blk): product of etot[b'] over b' > blk
 #pragma unroll
                             for (int b2 = 3; b2 >= 1; --b2) {
                                 if (b2 > blk) {
-                                    const float4 e0 = *reinterpret_cast<const float4*>(&mi.etot[b2][8 * cc]);
-                                    const float4 e1 = *reinterpret_cast<const float4*>(&mi.etot[b2][8 * cc + 4]);
-                                    sf[0] *= e0.x; sf[1] *= e0.y; sf[2] *= e0.z; sf[3] *= e0.w;
-                                    sf[4] *= e1.x; sf[5] *= e1.y; sf[6] *= e1.z; sf[7] *= e1.w;
+                                    float2 eb[4];
+                                    *reinterpret_cast<float4*>(eb) = *reinterpret_cast<const float4*>(&mi.etot[b2][8 * cc]);
+                                    *reinterpret_cast<float4*>(eb + 2) = *reinterpret_cast<const float4*>(&mi.etot[b2][8 * cc + 4]);
+#pragma unroll
+                                    for (int e = 0; e < 4; ++e) sf[e] = mul2(sf[e], eb[e]);
                                 }
                             }
                             if (t == 0) {   // gamma_L of the chunk for these columns (state carry, P13)
-                                *reinterpret_cast<float4*>(&mi.gamL[8 * cc]) = make_float4(sf[0] * et[0], sf[1] * et[1], sf[2] * et[2], sf[3] * et[3]);
-                                *reinterpret_cast<float4*>(&mi.gamL[8 * cc + 4]) = make_float4(sf[4] * et[4], sf[5] * et[5], sf[6] * et[6], sf[7] * et[7]);
-                            }
+                                float2 gl[4];
 #pragma unroll
-                            for (int e = 0; e < 8; ++e) {
-                                const float l2 = lg[8 * ci + e] * kLog2e;         // lg_t - lg_a <= 0
-                                Fp[e] = ex2_ftz(l2);                              // gamma_t / gamma_{a_blk}
-                                const float cx = ex2_ftz(-l2);                    // gamma_{a_blk} / gamma_t >= 1
-                                const float kh = kt[e] * rnk;
+                                for (int e = 0; e < 4; ++e) gl[e] = mul2(sf[e], et[e]);
+                                *reinterpret_cast<float4*>(&mi.gamL[8 * cc]) = *reinterpret_cast<const float4*>(gl);
+                                *reinterpret_cast<float4*>(&mi.gamL[8 * cc + 4]) = *reinterpret_cast<const float4*>(gl + 2);
+                            }
+                            const float2 rnk2 = splat2(rnk);
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                const float2 l2 = mul2(make_float2(lg[8 * ci + 2 * e], lg[8 * ci + 2 * e + 1]), splat2(kLog2e));   // lg_t - lg_a <= 0
+                                Fp[e] = make_float2(ex2_ftz(l2.x), ex2_ftz(l2.y));          // gamma_t / gamma_{a_blk}
+                                const float2 cx = make_float2(ex2_ftz(-l2.x), ex2_ftz(-l2.y));   // gamma_{a_blk} / gamma_t >= 1
+                                const float2 kh = mul2(kt[e], rnk2);
                                 ic[e] = cx;
-                                o1[e] = kh * cx;
-                                o2[e] = kh * ((cx * et[e]) * sf[e]);              // k^ gamma_L / gamma_t, every factor <= 1
+                                o1[e] = mul2(kh, cx);
+                                o2[e] = mul2(kh, mul2(mul2(cx, et[e]), sf[e]));              // k^ gamma_L / gamma_t, every factor <= 1
                             }
                             const uint32_t off = tile_chunk_off(64, t, cc);
-                            sts128(sm + Lo.Y1 + off, pack8(o1));      // C_t
-                            sts128(sm + Lo.Ktil + off, pack8(o2));    // Ktil_t
-                            if (rc) *reinterpret_cast<uint4*>(rc + Rc.IC + rp_off(t, cc)) = pack8(ic);
+                            sts128(sm + Lo.Y1 + off, pack8p(o1));      // C_t
+                            sts128(sm + Lo.Ktil + off, pack8p(o2));    // Ktil_t
+                            if (rc) *reinterpret_cast<uint4*>(rc + Rc.IC + rp_off(t, cc)) = pack8p(ic);
                         }
-                        unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, 64 + t, cc)), qv);
-                        unpack8(lds128(sm + Lo.KQraw + tile_chunk_off(128, krow, cc)), kv);
+                        unpack8p(lds128(sm + Lo.KQraw + tile_chunk_off(128, 64 + t, cc)), qv);
+                        unpack8p(lds128(sm + Lo.KQraw + tile_chunk_off(128, krow, cc)), kv);
+                        {
+                            const float2 rnq2 = splat2(rnq), rnkn2 = splat2(rnkn);
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) { qv[e] *= rnq; kv[e] *= rnkn; }
-                        if (has_next && bn > blk) {  // first row of its block
-                            sts128(ver_row(bn, false, tn, cc), pack8(kv));
-                            if (rc && (bn & 1)) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = pack8(kv);
+                            for (int e = 0; e < 4; ++e) { qv[e] = mul2(qv[e], rnq2); kv[e] = mul2(kv[e], rnkn2); }
                         }
-                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.FQ + rp_off(t, cc)) = pack8(Fp);
+                        if (has_next && bn > blk) {  // first row of its block
+                            sts128(ver_row(bn, false, tn, cc), pack8p(kv));
+                            if (rc && (bn & 1)) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = pack8p(kv);
+                        }
+                        if (rc) *reinterpret_cast<uint4*>(rc + Rc.FQ + rp_off(t, cc)) = pack8p(Fp);
 #pragma unroll
                         for (int jb = 3; jb >= 0; --jb) {
                             if (jb <= blk) {
 #pragma unroll
-                                for (int e = 0; e < 8; ++e) o[e] = qv[e] * Fp[e];
-                                const uint4 wq = pack8(o);
+                                for (int e = 0; e < 4; ++e) o[e] = mul2(qv[e], Fp[e]);
+                                const uint4 wq = pack8p(o);
                                 sts128(ver_row(jb, true, t, cc), wq);
                                 if (rc && jb == blk && (blk & 1)) *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, 64 + t, cc)) = wq;
                                 if (rc && jb == 0 && !s1) {
+                                    const float2 sc2 = splat2(a.scale);
 #pragma unroll
-                                    for (int e = 0; e < 8; ++e) o[e] *= a.scale;
-                                    *reinterpret_cast<uint4*>(rc + Rc.Q0 + tile_chunk_off(64, t, cc)) = pack8(o);
+                                    for (int e = 0; e < 4; ++e) o[e] = mul2(o[e], sc2);
+                                    *reinterpret_cast<uint4*>(rc + Rc.Q0 + tile_chunk_off(64, t, cc)) = pack8p(o);
                                 }
                                 if (has_next) {
 #pragma unroll
-                                    for (int e = 0; e < 8; ++e) o[e] = kv[e] * Fp[e];
-                                    const uint4 wk = pack8(o);
+                                    for (int e = 0; e < 4; ++e) o[e] = mul2(kv[e], Fp[e]);
+                                    const uint4 wk = pack8p(o);
                                     sts128(ver_row(jb, false, tn, cc), wk);
                                     if (rc && jb == blk && bn == blk && (blk & 1))
                                         *reinterpret_cast<uint4*>(rc + Rc.KQo + tile_chunk_off(128, tn, cc)) = wk;
                                 }
                                 if (jb > 0) {
-                                    const float4 e0 = *reinterpret_cast<const float4*>(&mi.etot[jb - 1][8 * cc]);
-                                    const float4 e1 = *reinterpret_cast<const float4*>(&mi.etot[jb - 1][8 * cc + 4]);
-                                    Fp[0] *= e0.x; Fp[1] *= e0.y; Fp[2] *= e0.z; Fp[3] *= e0.w;
-                                    Fp[4] *= e1.x; Fp[5] *= e1.y; Fp[6] *= e1.z; Fp[7] *= e1.w;
+                                    float2 eb[4];
+                                    *reinterpret_cast<float4*>(eb) = *reinterpret_cast<const float4*>(&mi.etot[jb - 1][8 * cc]);
+                                    *reinterpret_cast<float4*>(eb + 2) = *reinterpret_cast<const float4*>(&mi.etot[jb - 1][8 * cc + 4]);
+#pragma unroll
+                                    for (int e = 0; e < 4; ++e) Fp[e] = mul2(Fp[e], eb[e]);
                                 }
                             }
                         }
                         if (!has_next) {  // Kbar_0 = k^_0
-                            sts128(sm + Lo.KQbar + tile_chunk_off(128, 0, cc), pack8(kv));
+                            sts128(sm + Lo.KQbar + tile_chunk_off(128, 0, cc), pack8p(kv));
                         }
                     }
                 }
@@ -806,6 +818,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         tc_fence_after();
         if (krole && warp_active) {
             const float bt = live ? sBeta[t] : 0.f;
+            const float2 bt2 = splat2(bt), neg1 = splat2(-1.f);
             static_assert(HV == 32 && HK == 32, "one 32-column TMEM load per thread and phase");
             uint32_t v[32];
             tmem_ld32(tmem + TM_ACC + lane_base + half * HV, v);
@@ -813,12 +826,12 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             if (live) {
 #pragma unroll
                 for (int ch = 0; ch < 4; ++ch) {
-                    float fv[8];
+                    float2 fv[4];
                     const uint32_t off = tile_chunk_off(64, t, half * 4 + ch);
-                    unpack8(lds128(sm + Lo.V + off), fv);
+                    unpack8p(lds128(sm + Lo.V + off), fv);
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) fv[e] = bt * (fv[e] - __uint_as_float(v[8 * ch + e]));
-                    sts128(sm + Lo.Y2 + off, pack8(fv));
+                    for (int e = 0; e < 4; ++e) fv[e] = mul2(bt2, fma2(pair_of(v + 8 * ch + 2 * e), neg1, fv[e]));
+                    sts128(sm + Lo.Y2 + off, pack8p(fv));
                 }
             }
         }
@@ -863,12 +876,12 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             if (live) {
 #pragma unroll
                 for (int ch = 0; ch < 4; ++ch) {
-                    float f[8];
+                    float2 f[4];
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) f[e] = a.scale * __uint_as_float(v[8 * ch + e]);
+                    for (int e = 0; e < 4; ++e) f[e] = mul2(splat2(a.scale), pair_of(v + 8 * ch + 2 * e));
                     // staged as a bf16 row tile over beta R (dead since the solve); a TMA store sends it to HBM after the
                     // next barrier: 16 KB of STG from one SM would hold the warps for ~500 cycles (27-32 B/clk per SM)
-                    sts128(sm + Lo.Y2 + tile_chunk_off(64, t, half * 4 + ch), pack8(f));
+                    sts128(sm + Lo.Y2 + tile_chunk_off(64, t, half * 4 + ch), pack8p(f));
                 }
             }
         }
@@ -884,10 +897,14 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
               for (int c2 = 0; c2 < 2; ++c2) {
                 const int cc = half * (HK / 8) + 2 * s16 + c2;
                 float f[8];
+                float2 gl[4];
+                *reinterpret_cast<float4*>(gl) = *reinterpret_cast<const float4*>(&mi.gamL[8 * cc]);
+                *reinterpret_cast<float4*>(gl + 2) = *reinterpret_cast<const float4*>(&mi.gamL[8 * cc + 4]);
 #pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    f[e] = __uint_as_float(sv16[8 * c2 + e]) * mi.gamL[8 * cc + e] + __uint_as_float(wv16[8 * c2 + e]);
-                    sv16[8 * c2 + e] = __float_as_uint(f[e]);
+                for (int e = 0; e < 4; ++e) {
+                    const float2 y = fma2(pair_of(sv16 + 8 * c2 + 2 * e), gl[e], pair_of(wv16 + 8 * c2 + 2 * e));
+                    f[2 * e] = y.x; f[2 * e + 1] = y.y;
+                    sv16[8 * c2 + 2 * e] = __float_as_uint(y.x); sv16[8 * c2 + 2 * e + 1] = __float_as_uint(y.y);
                 }
                 const uint4 w = pack8(f);
                 const uint32_t off = tile_chunk_off(DV, row, cc);
