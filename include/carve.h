@@ -56,7 +56,8 @@ typedef enum {
     CARVE_ERR_ALIGN = 4,     /* a base pointer is not 16-byte aligned */
     CARVE_ERR_WORKSPACE = 5, /* workspace missing or smaller than carve_workspace_bytes() */
     CARVE_ERR_ARCH = 6,      /* current device is not compute capability 10.x */
-    CARVE_ERR_CUDA = 7       /* a CUDA runtime call failed (launch, attribute, copy) */
+    CARVE_ERR_CUDA = 7,      /* a CUDA runtime call failed (launch, attribute, copy) */
+    CARVE_ERR_STATIC_LIMIT = 8 /* carve_fwd_bwd_static: the problem needs more than CARVE_STATIC_SCRATCH_BYTES of scratch */
 } carve_status_t;
 
 typedef enum { CARVE_F32 = 0, CARVE_BF16 = 1 } carve_dtype_t;
@@ -181,6 +182,34 @@ carve_status_t carve_fwd_bwd_host_ctx(carve_host_ctx_t *ctx, const carve_params_
                                       void *dv, void *df, void *dbx, void *dwx, void *dbeta, float *dA, float *dtau,
                                       float *dUb, float *dUw, float *dVb, float *dVw, float *dS0, void *device_arena,
                                       size_t arena_bytes, void *cuda_stream);
+
+/*
+ * carve_fwd_bwd_static -- training forward + backward for callers that cannot allocate device memory (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  It is carve_fwd (training) followed by
+ * carve_bwd on `cuda_stream`, with the workspace the two exchange -- the forward's chunk records (Alg. 2 l.315-365,
+ * consumed by the reverse scan of Alg. 4 l.788-817), per-chain weight-gradient partials, progress flags -- held in a
+ * file-scope __device__ array inside the library instead of a caller buffer.  Same kernels, same launch configuration,
+ * same results as the two calls.  Arguments: exactly those of carve_fwd (inputs, O, S_final) and carve_bwd (dO,
+ * dS_final, the gradients), all DEVICE pointers owned by the caller, same layouts, same NULL rules.
+ *   - The array has CARVE_STATIC_SCRATCH_BYTES (16 MiB; carve_static_scratch_bytes() returns it).  Every GPU that
+ *     loads the library holds it until the process exits.
+ *   - A problem with carve_workspace_bytes(p, 1) > CARVE_STATIC_SCRATCH_BYTES returns CARVE_ERR_STATIC_LIMIT and
+ *     launches nothing (tensor path: ~262 KB per (chain, 64-token chunk) at d = 128, i.e. <= 60 chain-chunks).
+ *   - Calls no cudaMalloc, cudaFree or allocating library routine.
+ *   - All calls share the array; it keeps the last call's contents.  The only region that must start at zero (the
+ *     tensor path's progress flags) is cleared by the call itself on `cuda_stream`.
+ *   - Calls that overlap on the GPU (two streams, or two host threads on one device) RACE on the array: keep them on
+ *     one stream per device or order them with events.  Calls on different devices do not interact.
+ * Errors: those of carve_fwd / carve_bwd, plus CARVE_ERR_STATIC_LIMIT.
+ */
+#define CARVE_STATIC_SCRATCH_BYTES (16u << 20)
+size_t carve_static_scratch_bytes(void);
+carve_status_t carve_fwd_bwd_static(const carve_params_t *p, const void *q, const void *k, const void *v, const void *f,
+                                    const void *bx, const void *wx, const void *beta, const float *A, const float *tau,
+                                    const float *Ub, const float *Uw, const float *Vb, const float *Vw, const float *S0,
+                                    void *O, float *S_final, const void *dO, const float *dS_final, void *dq, void *dk,
+                                    void *dv, void *df, void *dbx, void *dwx, void *dbeta, float *dA, float *dtau,
+                                    float *dUb, float *dUw, float *dVb, float *dVw, float *dS0, void *cuda_stream);
 
 /* Number of kernel launches carve_fwd / carve_bwd enqueue for these parameters (for accounting). */
 int carve_num_launches(const carve_params_t *p, int bwd);

@@ -21,6 +21,7 @@ CARVE_PATH_AUTO, CARVE_PATH_SIMT, CARVE_PATH_TENSOR = 0, 1, 2
 # Every symbol include/carve.h declares (tests check the library exports them all).
 SYMBOLS = ("carve_workspace_bytes", "carve_fwd", "carve_bwd", "carve_step", "carve_host_arena_bytes", "carve_fwd_bwd_host",
            "carve_host_ctx_create", "carve_host_ctx_destroy", "carve_fwd_bwd_host_ctx",
+           "carve_fwd_bwd_static", "carve_static_scratch_bytes",
            "carve_num_launches", "carve_resolved_path", "carve_status_string", "carve_version")
 
 
@@ -94,6 +95,10 @@ def load_library() -> ctypes.CDLL:
         lib.carve_fwd_bwd_host_ctx.argtypes = [vp, pp, ci] + [vp] * 32 + [vp, sz, vp]
         lib.carve_host_ctx_create.restype = ci
         lib.carve_host_ctx_create.argtypes = [ctypes.POINTER(vp)]
+        lib.carve_fwd_bwd_static.restype = ci
+        lib.carve_fwd_bwd_static.argtypes = [pp] + [vp] * 32 + [vp]
+        lib.carve_static_scratch_bytes.restype = sz
+        lib.carve_static_scratch_bytes.argtypes = []
         lib.carve_host_ctx_destroy.restype = None
         lib.carve_host_ctx_destroy.argtypes = [vp]
         _lib = lib
@@ -169,6 +174,19 @@ def carve_bwd(p: Params, x: dict, dO, dS_final, grads: dict, workspace, stream: 
     _check(load_library().carve_bwd(ctypes.byref(cp), *[_ptr(x.get(n)) for n in _FWD_IN], _ptr(dO), _ptr(dS_final),
                                     *[_ptr(grads.get(n)) for n in _GRADS], _ptr(workspace), _nbytes(workspace),
                                     ctypes.c_void_p(stream)))
+
+
+def carve_static_scratch_bytes() -> int:
+    return int(load_library().carve_static_scratch_bytes())
+
+
+def carve_fwd_bwd_static(p: Params, x: dict, O, S_final, dO, dS_final, grads: dict, stream: int = 0) -> None:
+    """carve_fwd_bwd_static of carve.h: training forward + backward with the workspace in the library's static device
+    array (no allocation; problems beyond carve_static_scratch_bytes() raise CarveError with CARVE_ERR_STATIC_LIMIT)."""
+    cp = p.c()
+    _check(load_library().carve_fwd_bwd_static(ctypes.byref(cp), *[_ptr(x.get(n)) for n in _FWD_IN], _ptr(O), _ptr(S_final),
+                                               _ptr(dO), _ptr(dS_final), *[_ptr(grads.get(n)) for n in _GRADS],
+                                               ctypes.c_void_p(stream)))
 
 
 def carve_host_ctx_create() -> ctypes.c_void_p:

@@ -116,6 +116,7 @@ const char* carve_status_string(carve_status_t s)
         case CARVE_ERR_WORKSPACE: return "workspace missing or too small";
         case CARVE_ERR_ARCH: return "device is not sm_100";
         case CARVE_ERR_CUDA: return "CUDA runtime error";
+        case CARVE_ERR_STATIC_LIMIT: return "problem needs more scratch than the static no-allocation limit (CARVE_STATIC_SCRATCH_BYTES)";
     }
     return "unknown status";
 }

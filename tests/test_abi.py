@@ -28,7 +28,7 @@ def test_header_symbols_exported(lib):
 
 
 def test_status_strings(lib):
-    for s in range(8):
+    for s in range(9):
         assert len(lib.carve_status_string(s)) > 0
 
 
