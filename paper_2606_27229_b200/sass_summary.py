@@ -1,7 +1,7 @@
 """Per-kernel histogram of the SASS mnemonics that show how a kernel of csrc/libcarve.so talks to the hardware:
 tcgen05.mma (UTCHMMA), TMEM loads/stores (LDTM/STTM), TMA loads/stores/prefetches (UTMALDG/UTMASTG/UTMAPF), bulk copies
 (UBLKCP), legacy tensor-core mma.sync (HMMA), ldmatrix/stmatrix (LDSM/STSM), mbarrier ops (SYNCS), shared loads (LDS)
-and generic loads (LD; should be 0: shared memory is addressed as shared).
+generic loads (LD; should be 0: shared memory is addressed as shared) and packed fp32 pairs (FFMA2/FMUL2/FADD2).
 
     python -m paper_2606_27229_b200.sass_summary > profiles/r2_sass_summary.txt
 """
@@ -14,7 +14,7 @@ import subprocess
 from paper_2606_27229_b200 import build
 
 COLS = ("UTCHMMA", "LDTM", "STTM", "UTMALDG", "UTMASTG", "UTMAPF", "UBLKCP", "HMMA.1688.F32.TF32", "HMMA.16816.F32.BF16",
-        "LDSM", "STSM", "SYNCS", "LDS", "STS", "LD", "ST", "LDG", "STG", "MUFU", "BAR")
+        "LDSM", "STSM", "SYNCS", "LDS", "STS", "LD", "ST", "LDG", "STG", "MUFU", "FFMA2", "FMUL2", "FADD2", "BAR")
 
 
 def main():
