@@ -142,6 +142,21 @@ carve_status_t carve_step(const carve_params_t *p, const void *q, const void *k,
                           const float *Ub, const float *Uw, const float *Vb, const float *Vw, float *S, void *O,
                           void *cuda_stream);
 
+/*
+ * carve_step on a ragged batch (the variable-length batches of a serving step: sequences that receive 0..T new tokens
+ * each).  The token tensors are PACKED: q,k,f,bx [N,H,dk], v,wx,O [N,H,dv], beta [N,H] with N = cu_seqlens[B] rows in
+ * total; sequence b owns rows cu_seqlens[b] .. cu_seqlens[b+1] (DEVICE int32 array of B + 1 non-decreasing entries,
+ * cu_seqlens[0] = 0, read by the kernel: no host synchronisation).  p->T is the declared maximum number of new tokens of
+ * any sequence (1..16); a sequence with more is processed up to p->T tokens only (the caller's contract violation, kept
+ * memory-safe), a sequence with none keeps its state bit for bit and writes no output.  Each sequence's tokens form one
+ * gate chunk of their own length, i.e. the result for sequence b equals carve_step on that sequence alone with
+ * T = its length.  Everything else as carve_step; CARVE_ERR_NULL if cu_seqlens is NULL.
+ */
+carve_status_t carve_step_varlen(const carve_params_t *p, const void *q, const void *k, const void *v, const void *f,
+                                 const void *bx, const void *wx, const void *beta, const float *A, const float *tau,
+                                 const float *Ub, const float *Uw, const float *Vb, const float *Vw, float *S, void *O,
+                                 const int *cu_seqlens, void *cuda_stream);
+
 /* Bytes of device arena carve_fwd_bwd_host needs (device copies of every tensor + workspace). */
 size_t carve_host_arena_bytes(const carve_params_t *p, int with_bwd);
 

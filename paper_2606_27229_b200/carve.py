@@ -21,7 +21,7 @@ CARVE_PATH_AUTO, CARVE_PATH_SIMT, CARVE_PATH_TENSOR = 0, 1, 2
 # Every symbol include/carve.h declares (tests check the library exports them all).
 SYMBOLS = ("carve_workspace_bytes", "carve_fwd", "carve_bwd", "carve_step", "carve_host_arena_bytes", "carve_fwd_bwd_host",
            "carve_host_ctx_create", "carve_host_ctx_destroy", "carve_fwd_bwd_host_ctx",
-           "carve_fwd_bwd_static", "carve_static_scratch_bytes",
+           "carve_fwd_bwd_static", "carve_static_scratch_bytes", "carve_step_varlen",
            "carve_num_launches", "carve_resolved_path", "carve_status_string", "carve_version")
 
 
@@ -87,6 +87,8 @@ def load_library() -> ctypes.CDLL:
         lib.carve_fwd.argtypes = [pp] + [vp] * 16 + [vp, sz, vp]
         lib.carve_step.restype = ci
         lib.carve_step.argtypes = [pp] + [vp] * 15 + [vp]
+        lib.carve_step_varlen.restype = ci
+        lib.carve_step_varlen.argtypes = [pp] + [vp] * 15 + [vp, vp]
         lib.carve_bwd.restype = ci
         lib.carve_bwd.argtypes = [pp] + [vp] * 30 + [vp, sz, vp]
         lib.carve_fwd_bwd_host.restype = ci
@@ -165,6 +167,14 @@ def carve_step(p: Params, x: dict, S, O, stream: int = 0) -> None:
     cp = p.c()
     _check(load_library().carve_step(ctypes.byref(cp), *[_ptr(x.get(n)) for n in _FWD_IN[:-1]], _ptr(S), _ptr(O),
                                      ctypes.c_void_p(stream)))
+
+
+def carve_step_varlen(p: Params, x: dict, S, O, cu_seqlens, stream: int = 0) -> None:
+    """carve_step_varlen of carve.h: packed token tensors [N,H,d] with N = cu_seqlens[B]; `cu_seqlens` is a device int32
+    tensor of B + 1 entries; p.T = the maximum number of new tokens of any sequence (<= 16)."""
+    cp = p.c()
+    _check(load_library().carve_step_varlen(ctypes.byref(cp), *[_ptr(x.get(n)) for n in _FWD_IN[:-1]], _ptr(S), _ptr(O),
+                                            _ptr(cu_seqlens), ctypes.c_void_p(stream)))
 
 
 def carve_bwd(p: Params, x: dict, dO, dS_final, grads: dict, workspace, stream: int = 0) -> None:

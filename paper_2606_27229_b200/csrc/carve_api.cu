@@ -180,10 +180,10 @@ carve_status_t carve_fwd(const carve_params_t* p, const void* q, const void* k, 
                                                                                               : CARVE_ERR_CUDA;
 }
 
-carve_status_t carve_step(const carve_params_t* p, const void* q, const void* k, const void* v, const void* f,
-                          const void* bx, const void* wx, const void* beta, const float* A, const float* tau,
-                          const float* Ub, const float* Uw, const float* Vb, const float* Vw, float* S, void* O,
-                          void* cuda_stream)
+static carve_status_t step_impl(const carve_params_t* p, const void* q, const void* k, const void* v, const void* f,
+                                const void* bx, const void* wx, const void* beta, const float* A, const float* tau,
+                                const float* Ub, const float* Uw, const float* Vb, const float* Vw, float* S, void* O,
+                                const int* cu_seqlens, void* cuda_stream)
 {
     if (!p) return CARVE_ERR_NULL;
     if (p->dtype != CARVE_F32 && p->dtype != CARVE_BF16) return CARVE_ERR_DTYPE;
@@ -195,10 +195,27 @@ carve_status_t carve_step(const carve_params_t* p, const void* q, const void* k,
         if (!aligned16(ptr)) return CARVE_ERR_ALIGN;
     const carve_status_t s = check_arch();
     if (s != CARVE_OK) return s;
-    return step_launch(*p, q, k, v, f, bx, wx, beta, A, tau, Ub, Uw, Vb, Vw, S, O, static_cast<cudaStream_t>(cuda_stream)) ==
-                   cudaSuccess
+    return step_launch(*p, q, k, v, f, bx, wx, beta, A, tau, Ub, Uw, Vb, Vw, S, O, cu_seqlens,
+                       static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess
                ? CARVE_OK
                : CARVE_ERR_CUDA;
+}
+
+carve_status_t carve_step(const carve_params_t* p, const void* q, const void* k, const void* v, const void* f,
+                          const void* bx, const void* wx, const void* beta, const float* A, const float* tau,
+                          const float* Ub, const float* Uw, const float* Vb, const float* Vw, float* S, void* O,
+                          void* cuda_stream)
+{
+    return step_impl(p, q, k, v, f, bx, wx, beta, A, tau, Ub, Uw, Vb, Vw, S, O, nullptr, cuda_stream);
+}
+
+carve_status_t carve_step_varlen(const carve_params_t* p, const void* q, const void* k, const void* v, const void* f,
+                                 const void* bx, const void* wx, const void* beta, const float* A, const float* tau,
+                                 const float* Ub, const float* Uw, const float* Vb, const float* Vw, float* S, void* O,
+                                 const int* cu_seqlens, void* cuda_stream)
+{
+    if (!cu_seqlens) return CARVE_ERR_NULL;
+    return step_impl(p, q, k, v, f, bx, wx, beta, A, tau, Ub, Uw, Vb, Vw, S, O, cu_seqlens, cuda_stream);
 }
 
 // carve_bwd; `epilogue_after`: the tensor path launches its chunk-local epilogue as a plain dependent kernel

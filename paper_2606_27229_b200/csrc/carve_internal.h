@@ -110,7 +110,7 @@ cudaError_t tc_bwd_launch(const Args& a, uint8_t* ws, const TcWsLayout& w, float
 bool step_supported(int dk, int dv);
 cudaError_t step_launch(const carve_params_t& p, const void* q, const void* k, const void* v, const void* f, const void* bx,
                         const void* wx, const void* beta, const float* A, const float* tau, const float* Ub, const float* Uw,
-                        const float* Vb, const float* Vw, float* S, void* O, cudaStream_t st);
+                        const float* Vb, const float* Vw, float* S, void* O, const int* cu_seqlens, cudaStream_t st);
 
 // Deterministic reduction of per-chain partials (carve_simt_bwd.cu), shared by both paths.
 cudaError_t reduce_weights_launch(const float* part, int chains, int stride, int H, int dk, int dv, int r, float* dUb,

@@ -8,6 +8,9 @@
 // With n = 1 this is exact per-token content gating.  It is the same function as carve_fwd with T = L = n (the chunked
 // WY form equals this recurrence), evaluated without the solve because n is small.
 //
+// Ragged batches (carve_step_varlen): the token tensors are packed [total_tokens, H, d] and sequence b owns the rows
+// cu_seqlens[b] .. cu_seqlens[b+1] (0..T tokens each; the variable-length batches of SURVEY 8(f) NEXT-1).
+//
 // One CTA per (batch, head) chain; the state makes one round trip HBM -> shared memory -> HBM per call, which is the
 // algorithmic traffic of a decode step (2 x 4 d_v d_k bytes per chain).  fp32 arithmetic throughout, plain FFMA.
 #include "simt_common.cuh"
@@ -22,6 +25,7 @@ struct StepArgs {
     const float *A, *tau, *Ub, *Uw, *Vb, *Vw;
     float* S;
     void* O;
+    const int* cu;   // ragged batch: tokens of sequence b are rows cu[b] .. cu[b+1] of the packed token tensors (else NULL)
 };
 
 template <typename T, int DK, int DV>
@@ -51,6 +55,11 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
     const T* gbeta = static_cast<const T*>(a.beta);
     T* gO = static_cast<T*>(a.O);
     float* gS = a.S + (size_t)chain * DV * DK;
+    // tokens of this sequence: rows tok0 .. tok0 + n of the [tokens, H, d] tensors (ragged: from cu_seqlens, clamped to the
+    // declared maximum; a sequence without new tokens leaves its state untouched)
+    const int tok0 = a.cu ? __ldg(a.cu + b) : b * a.n;
+    const int n = a.cu ? min(max(__ldg(a.cu + b + 1) - tok0, 0), a.n) : a.n;
+    if (n == 0) return;
 
     for (int i = tid; i < DV * DK / 4; i += NT) {
         const int x = i / (DK / 4), j4 = i % (DK / 4);
@@ -83,8 +92,8 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
     }
     __syncthreads();
 
-    for (int t = 0; t < a.n; ++t) {
-        const size_t tok = ((size_t)b * a.n + t) * a.H + h;
+    for (int t = 0; t < n; ++t) {
+        const size_t tok = ((size_t)tok0 + t) * a.H + h;
         // q^, k^ (D1)
         if (warp < 2) {
             const T* src = warp == 0 ? gq : gk;
@@ -201,9 +210,10 @@ bool step_supported(int dk, int dv)
 
 cudaError_t step_launch(const carve_params_t& p, const void* q, const void* k, const void* v, const void* f, const void* bx,
                         const void* wx, const void* beta, const float* A, const float* tau, const float* Ub, const float* Uw,
-                        const float* Vb, const float* Vw, float* S, void* O, cudaStream_t st)
+                        const float* Vb, const float* Vw, float* S, void* O, const int* cu_seqlens, cudaStream_t st)
 {
     StepArgs a{};
+    a.cu = cu_seqlens;
     a.B = p.B; a.H = p.H; a.n = p.T; a.r = p.r; a.l2norm = p.qk_l2norm; a.scale = p.scale; a.eps = p.eps;
     a.q = q; a.k = k; a.v = v; a.f = f; a.bx = bx; a.wx = wx; a.beta = beta;
     a.A = A; a.tau = tau; a.Ub = Ub; a.Uw = Uw; a.Vb = Vb; a.Vw = Vw; a.S = S; a.O = O;
