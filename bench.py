@@ -227,6 +227,64 @@ def run_step(args):
                                    "frac": ach / peaks["hbm_gbs"], "traffic": None, "algorithmic_bytes_per_launch": bytes_alg}}), flush=True)
 
 
+def run_layer_ends(args):
+    """`--op layer_ends`: the two chunk-local passes around the operator: SiLU on q,k,v and RMSNorm
+    of the assembled output, forward and backward, at the token shape of --config.  Not the BASELINE.json metric: tokens/s
+    through the four launches and, per launch, the fraction of the HBM roofline (algorithmic bytes = every tensor read or
+    written once).  The tensors of one step (1.2 GB at config 1) exceed the 126 MB L2."""
+    import torch
+    from paper_2606_27229_b200 import carve
+    torch.cuda.set_device(0)
+    cfg = get_cfg(args.config)
+    tok_dt = torch.bfloat16 if cfg.dtype == "bf16" else torch.float32
+    e = 2 if cfg.dtype == "bf16" else 4
+    p = carve.Params(B=cfg.B, H=cfg.H, T=cfg.T, L=cfg.L, dk=cfg.dk, dv=cfg.dv, r=cfg.r,
+                     dtype=carve.CARVE_BF16 if cfg.dtype == "bf16" else carve.CARVE_F32)
+    g = torch.Generator(device="cuda").manual_seed(0)
+    mk = lambda d: torch.randn(cfg.B, cfg.T, cfg.H, d, device="cuda", generator=g).to(tok_dt)
+    qx, kx, vx, o, dy = mk(cfg.dk), mk(cfg.dk), mk(cfg.dv), mk(cfg.dv), mk(cfg.dv)
+    q, k, v, y, d_o = (torch.empty_like(t) for t in (qx, kx, vx, o, dy))
+    dq, dk, dv = mk(cfg.dk), mk(cfg.dk), mk(cfg.dv)
+    gain = torch.ones(cfg.H * cfg.dv, device="cuda")
+    dgain = torch.empty_like(gain)
+    ws = torch.empty(carve.carve_out_norm_workspace_bytes(p), dtype=torch.uint8, device="cuda")
+    st = torch.cuda.current_stream()
+    tokh = cfg.B * cfg.T * cfg.H
+    calls = {
+        "silu_qkv_fwd": (lambda: carve.carve_silu_qkv_fwd(p, qx, kx, vx, q, k, v, st.cuda_stream), 2 * tokh * (2 * cfg.dk + cfg.dv) * e, 1),
+        "silu_qkv_bwd": (lambda: carve.carve_silu_qkv_bwd(p, qx, kx, vx, dq, dk, dv, st.cuda_stream), 3 * tokh * (2 * cfg.dk + cfg.dv) * e, 1),
+        "out_norm_fwd": (lambda: carve.carve_out_norm_fwd(p, o, gain, 1e-5, y, st.cuda_stream), 2 * tokh * cfg.dv * e, 1),
+        "out_norm_bwd": (lambda: carve.carve_out_norm_bwd(p, o, gain, 1e-5, dy, d_o, dgain, ws, st.cuda_stream), 3 * tokh * cfg.dv * e, 2),
+    }
+    peaks = load_peaks()
+    per, total_ms, launches = {}, 0.0, 0
+    for name, (fn, nbytes, nl) in calls.items():
+        for _ in range(max(args.warmup, 3)):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(st)
+        for _ in range(args.steps):
+            fn()
+        e1.record(st)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        ach = nbytes / (ms * 1e-3) / 1e9
+        per[name] = {"ms": ms, "algorithmic_bytes": nbytes, "achieved_GBps": ach, "frac": ach / peaks["hbm_gbs"]}
+        total_ms += ms
+        launches += nl * args.steps
+    tot_bytes = sum(c[1] for c in calls.values())
+    ach = tot_bytes / (total_ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "CARVE layer ends (SiLU q,k,v + RMSNorm(o), fwd+bwd) tokens/sec", "unit": "tokens/s", "n_gpus": 1,
+                      "steps": args.steps, "warmup": args.warmup, "higher_is_better": True,
+                      "value": cfg.B * cfg.T / (total_ms * 1e-3), "ms_per_step": total_ms, "dtype": cfg.dtype, "data": "synthetic",
+                      "config": {"workload": f"{cfg.name}: B={cfg.B},H={cfg.H},T={cfg.T},dk={cfg.dk},dv={cfg.dv}; tensors of a step exceed L2"},
+                      "gpu_launches": launches, "calls": per,
+                      "roofline": {"bound": "hbm", "kernel": "the four launches together", "achieved": ach, "peak": peaks["hbm_gbs"],
+                                   "unit": "GB/s", "frac": ach / peaks["hbm_gbs"], "traffic": None,
+                                   "algorithmic_bytes_per_launch": tot_bytes}}), flush=True)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -438,7 +496,8 @@ def main():
     ap.add_argument("--config", default="cfg1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fwd-only", action="store_true", help="time carve_fwd alone (inference call, nothing saved)")
-    ap.add_argument("--op", default="train", choices=["train", "step"], help="step: time the decode call carve_step instead")
+    ap.add_argument("--op", default="train", choices=["train", "step", "layer_ends"],
+                    help="step: time the decode call carve_step instead; layer_ends: the SiLU / RMSNorm passes around the operator")
     ap.add_argument("--decode-batch", type=int, default=256)
     ap.add_argument("--scalar-write", action="store_true",
                     help="the scalar-write variant (wx = Uw = Vw = NULL, PAPER.md section 4.2): not the BASELINE.json metric's workload")
@@ -460,6 +519,8 @@ def main():
         raise SystemExit(subprocess.call(cmd, env=env))
     if args.op == "step":
         run_step(args)
+    elif args.op == "layer_ends":
+        run_layer_ends(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

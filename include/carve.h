@@ -157,6 +157,34 @@ carve_status_t carve_step_varlen(const carve_params_t *p, const void *q, const v
                                  const float *Ub, const float *Uw, const float *Vb, const float *Vw, float *S, void *O,
                                  const int *cu_seqlens, void *cuda_stream);
 
+/*
+ * Layer ends (the two chunk-local "hoisted" launches around the operator, Alg. 3 step 3 l.399 and step 9 l.407): fully
+ * parallel over tokens, no state.  Only B, H, T, dk, dv and dtype of *p are read.  All pointers are DEVICE pointers,
+ * 16-byte aligned, owned by the caller; token tensors are [B,T,H,d] row-major in p->dtype.
+ *
+ * carve_silu_qkv_fwd: q = SiLU(qx), k = SiLU(kx), v = SiLU(vx) (Eq. 6 l.125-126; qx = W_Q h etc. are the outputs of the
+ *   input projections, dense GEMMs outside the path), one launch over the three tensors.  Output may alias its input.
+ *   A tensor is skipped by passing NULL for both of its pointers (only one NULL: CARVE_ERR_NULL).
+ * carve_silu_qkv_bwd: dq, dk, dv hold the gradients w.r.t. q, k, v (carve_bwd's outputs) and are overwritten IN PLACE by the
+ *   gradients w.r.t. qx, kx, vx:  d x = d y (s + x s (1 - s)), s = sigmoid(x).
+ * carve_out_norm_fwd: y = RMSNorm(reshape(o)) (Alg. 1 line 15 l.194): o, y [B,T,H,dv]; every token's H*dv channels are
+ *   scaled by 1/sqrt(mean(o^2) + eps) and by gain [H*dv] (float).  W_O is a dense GEMM outside the path.  Rows of at most
+ *   8 KB (H*dv <= 4096 bf16 / 2048 fp32), else CARVE_ERR_SHAPE.  y may alias o.
+ * carve_out_norm_bwd: d_o [B,T,H,dv] and dgain [H*dv] (float, overwritten) from dy [B,T,H,dv]; the statistics are
+ *   recomputed from o.  `workspace`: carve_out_norm_workspace_bytes(p) bytes of scratch (per-warp partial sums of dgain,
+ *   added in a fixed order: results are run-to-run bitwise identical), CARVE_ERR_WORKSPACE if missing or too small.
+ *   d_o may alias dy.
+ */
+carve_status_t carve_silu_qkv_fwd(const carve_params_t *p, const void *qx, const void *kx, const void *vx, void *q, void *k,
+                                  void *v, void *cuda_stream);
+carve_status_t carve_silu_qkv_bwd(const carve_params_t *p, const void *qx, const void *kx, const void *vx, void *dq, void *dk,
+                                  void *dv, void *cuda_stream);
+carve_status_t carve_out_norm_fwd(const carve_params_t *p, const void *o, const float *gain, float eps, void *y,
+                                  void *cuda_stream);
+size_t carve_out_norm_workspace_bytes(const carve_params_t *p);
+carve_status_t carve_out_norm_bwd(const carve_params_t *p, const void *o, const float *gain, float eps, const void *dy,
+                                  void *d_o, float *dgain, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
 /* Bytes of device arena carve_fwd_bwd_host needs (device copies of every tensor + workspace). */
 size_t carve_host_arena_bytes(const carve_params_t *p, int with_bwd);
 

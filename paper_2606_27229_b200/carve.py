@@ -22,6 +22,8 @@ CARVE_PATH_AUTO, CARVE_PATH_SIMT, CARVE_PATH_TENSOR = 0, 1, 2
 SYMBOLS = ("carve_workspace_bytes", "carve_fwd", "carve_bwd", "carve_step", "carve_host_arena_bytes", "carve_fwd_bwd_host",
            "carve_host_ctx_create", "carve_host_ctx_destroy", "carve_fwd_bwd_host_ctx",
            "carve_fwd_bwd_static", "carve_static_scratch_bytes", "carve_step_varlen",
+           "carve_silu_qkv_fwd", "carve_silu_qkv_bwd", "carve_out_norm_fwd", "carve_out_norm_bwd",
+           "carve_out_norm_workspace_bytes",
            "carve_num_launches", "carve_resolved_path", "carve_status_string", "carve_version")
 
 
@@ -89,6 +91,16 @@ def load_library() -> ctypes.CDLL:
         lib.carve_step.argtypes = [pp] + [vp] * 15 + [vp]
         lib.carve_step_varlen.restype = ci
         lib.carve_step_varlen.argtypes = [pp] + [vp] * 15 + [vp, vp]
+        lib.carve_silu_qkv_fwd.restype = ci
+        lib.carve_silu_qkv_fwd.argtypes = [pp] + [vp] * 6 + [vp]
+        lib.carve_silu_qkv_bwd.restype = ci
+        lib.carve_silu_qkv_bwd.argtypes = [pp] + [vp] * 6 + [vp]
+        lib.carve_out_norm_fwd.restype = ci
+        lib.carve_out_norm_fwd.argtypes = [pp, vp, vp, ctypes.c_float, vp, vp]
+        lib.carve_out_norm_workspace_bytes.restype = sz
+        lib.carve_out_norm_workspace_bytes.argtypes = [pp]
+        lib.carve_out_norm_bwd.restype = ci
+        lib.carve_out_norm_bwd.argtypes = [pp, vp, vp, ctypes.c_float, vp, vp, vp, vp, sz, vp]
         lib.carve_bwd.restype = ci
         lib.carve_bwd.argtypes = [pp] + [vp] * 30 + [vp, sz, vp]
         lib.carve_fwd_bwd_host.restype = ci
@@ -167,6 +179,39 @@ def carve_step(p: Params, x: dict, S, O, stream: int = 0) -> None:
     cp = p.c()
     _check(load_library().carve_step(ctypes.byref(cp), *[_ptr(x.get(n)) for n in _FWD_IN[:-1]], _ptr(S), _ptr(O),
                                      ctypes.c_void_p(stream)))
+
+
+def carve_silu_qkv_fwd(p: Params, qx, kx, vx, q, k, v, stream: int = 0) -> None:
+    """carve_silu_qkv_fwd of carve.h: q, k, v = SiLU(qx), SiLU(kx), SiLU(vx) in one launch (None pairs are skipped)."""
+    cp = p.c()
+    _check(load_library().carve_silu_qkv_fwd(ctypes.byref(cp), _ptr(qx), _ptr(kx), _ptr(vx), _ptr(q), _ptr(k), _ptr(v),
+                                             ctypes.c_void_p(stream)))
+
+
+def carve_silu_qkv_bwd(p: Params, qx, kx, vx, dq, dk, dv, stream: int = 0) -> None:
+    """carve_silu_qkv_bwd of carve.h: dq, dk, dv (gradients w.r.t. q, k, v) become those w.r.t. qx, kx, vx, in place."""
+    cp = p.c()
+    _check(load_library().carve_silu_qkv_bwd(ctypes.byref(cp), _ptr(qx), _ptr(kx), _ptr(vx), _ptr(dq), _ptr(dk), _ptr(dv),
+                                             ctypes.c_void_p(stream)))
+
+
+def carve_out_norm_workspace_bytes(p: Params) -> int:
+    cp = p.c()
+    return int(load_library().carve_out_norm_workspace_bytes(ctypes.byref(cp)))
+
+
+def carve_out_norm_fwd(p: Params, o, gain, eps: float, y, stream: int = 0) -> None:
+    """carve_out_norm_fwd of carve.h: y = RMSNorm over the H*dv channels of every token of o, times gain."""
+    cp = p.c()
+    _check(load_library().carve_out_norm_fwd(ctypes.byref(cp), _ptr(o), _ptr(gain), ctypes.c_float(eps), _ptr(y),
+                                             ctypes.c_void_p(stream)))
+
+
+def carve_out_norm_bwd(p: Params, o, gain, eps: float, dy, d_o, dgain, workspace, stream: int = 0) -> None:
+    """carve_out_norm_bwd of carve.h."""
+    cp = p.c()
+    _check(load_library().carve_out_norm_bwd(ctypes.byref(cp), _ptr(o), _ptr(gain), ctypes.c_float(eps), _ptr(dy), _ptr(d_o),
+                                             _ptr(dgain), _ptr(workspace), _nbytes(workspace), ctypes.c_void_p(stream)))
 
 
 def carve_step_varlen(p: Params, x: dict, S, O, cu_seqlens, stream: int = 0) -> None:

@@ -278,6 +278,81 @@ carve_status_t carve_bwd(const carve_params_t* p, const void* q, const void* k, 
                     dA, dtau, dUb, dUw, dVb, dVw, dS0, workspace, workspace_bytes, cuda_stream, false);
 }
 
+// ---- layer ends -----------------------------------------------------------------
+static carve_status_t ends_params_ok(const carve_params_t* p)
+{
+    if (!p) return CARVE_ERR_NULL;
+    if (p->dtype != CARVE_F32 && p->dtype != CARVE_BF16) return CARVE_ERR_DTYPE;
+    if (p->B <= 0 || p->H <= 0 || p->T <= 0 || p->dk <= 0 || p->dv <= 0) return CARVE_ERR_SHAPE;
+    const int per16 = p->dtype == CARVE_BF16 ? 8 : 4;
+    if (p->dk % per16 || p->dv % per16) return CARVE_ERR_SHAPE;
+    return CARVE_OK;
+}
+
+static carve_status_t silu_impl(const carve_params_t* p, const void* qx, const void* kx, const void* vx, void* q, void* k,
+                                void* v, bool bwd, void* cuda_stream)
+{
+    carve_status_t s = ends_params_ok(p);
+    if (s != CARVE_OK) return s;
+    if ((qx == nullptr) != (q == nullptr) || (kx == nullptr) != (k == nullptr) || (vx == nullptr) != (v == nullptr))
+        return CARVE_ERR_NULL;   // a tensor is skipped by passing NULL for both of its pointers
+    for (const void* ptr : {qx, kx, vx, (const void*)q, (const void*)k, (const void*)v})
+        if (!aligned16(ptr)) return CARVE_ERR_ALIGN;
+    if ((s = check_arch()) != CARVE_OK) return s;
+    return silu_qkv_launch(*p, qx, kx, vx, q, k, v, bwd, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess ? CARVE_OK
+                                                                                                                  : CARVE_ERR_CUDA;
+}
+
+carve_status_t carve_silu_qkv_fwd(const carve_params_t* p, const void* qx, const void* kx, const void* vx, void* q, void* k,
+                                  void* v, void* cuda_stream)
+{
+    return silu_impl(p, qx, kx, vx, q, k, v, false, cuda_stream);
+}
+
+carve_status_t carve_silu_qkv_bwd(const carve_params_t* p, const void* qx, const void* kx, const void* vx, void* dq, void* dk,
+                                  void* dv, void* cuda_stream)
+{
+    return silu_impl(p, qx, kx, vx, dq, dk, dv, true, cuda_stream);
+}
+
+size_t carve_out_norm_workspace_bytes(const carve_params_t* p)
+{
+    if (ends_params_ok(p) != CARVE_OK || !out_norm_supported(*p)) return 0;
+    return out_norm_ws_bytes(*p);
+}
+
+carve_status_t carve_out_norm_fwd(const carve_params_t* p, const void* o, const float* gain, float eps, void* y,
+                                  void* cuda_stream)
+{
+    carve_status_t s = ends_params_ok(p);
+    if (s != CARVE_OK) return s;
+    if (!out_norm_supported(*p)) return CARVE_ERR_SHAPE;
+    if (!o || !gain || !y) return CARVE_ERR_NULL;
+    if (!aligned16(o) || !aligned16(gain) || !aligned16(y)) return CARVE_ERR_ALIGN;
+    if ((s = check_arch()) != CARVE_OK) return s;
+    return out_norm_launch(*p, false, o, gain, eps, nullptr, y, nullptr, nullptr, static_cast<cudaStream_t>(cuda_stream)) ==
+                   cudaSuccess
+               ? CARVE_OK
+               : CARVE_ERR_CUDA;
+}
+
+carve_status_t carve_out_norm_bwd(const carve_params_t* p, const void* o, const float* gain, float eps, const void* dy,
+                                  void* d_o, float* dgain, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    carve_status_t s = ends_params_ok(p);
+    if (s != CARVE_OK) return s;
+    if (!out_norm_supported(*p)) return CARVE_ERR_SHAPE;
+    if (!o || !gain || !dy || !d_o || !dgain) return CARVE_ERR_NULL;
+    for (const void* ptr : {o, (const void*)gain, dy, (const void*)d_o, (const void*)dgain, (const void*)workspace})
+        if (!aligned16(ptr)) return CARVE_ERR_ALIGN;
+    if (!workspace || workspace_bytes < out_norm_ws_bytes(*p)) return CARVE_ERR_WORKSPACE;
+    if ((s = check_arch()) != CARVE_OK) return s;
+    return out_norm_launch(*p, true, o, gain, eps, dy, d_o, static_cast<float*>(workspace), dgain,
+                           static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess
+               ? CARVE_OK
+               : CARVE_ERR_CUDA;
+}
+
 // ---- host-buffer entry point ---------------------------------------------------------------------
 // The batch is cut into up to 8 slices (chains are independent; [B,T,H,d] makes a batch slice one
 // contiguous slab of every token tensor).  Each slice runs copy-in -> carve_fwd -> carve_bwd -> copy-out on a

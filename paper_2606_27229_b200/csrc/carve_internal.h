@@ -108,6 +108,14 @@ cudaError_t tc_bwd_launch(const Args& a, uint8_t* ws, const TcWsLayout& w, float
 
 // Recurrent step (carve_step.cu): n <= 16 new tokens per chain, state in place.
 bool step_supported(int dk, int dv);
+// layer ends (carve_layer_ends.cu)
+cudaError_t silu_qkv_launch(const carve_params_t& p, const void* qx, const void* kx, const void* vx, void* q, void* k, void* v,
+                            bool bwd, cudaStream_t st);
+bool out_norm_supported(const carve_params_t& p);
+size_t out_norm_ws_bytes(const carve_params_t& p);
+cudaError_t out_norm_launch(const carve_params_t& p, bool bwd, const void* o, const float* gain, float eps, const void* dy,
+                            void* out, float* partial, float* dgain, cudaStream_t st);
+
 cudaError_t step_launch(const carve_params_t& p, const void* q, const void* k, const void* v, const void* f, const void* bx,
                         const void* wx, const void* beta, const float* A, const float* tau, const float* Ub, const float* Uw,
                         const float* Vb, const float* Vw, float* S, void* O, const int* cu_seqlens, cudaStream_t st);
