@@ -243,6 +243,8 @@ carve_status_t carve_fwd_bwd_host_ctx(carve_host_ctx_t *ctx, const carve_params_
  *     tensor path's progress flags) is cleared by the call itself on `cuda_stream`.
  *   - Calls that overlap on the GPU (two streams, or two host threads on one device) RACE on the array: keep them on
  *     one stream per device or order them with events.  Calls on different devices do not interact.
+ *   - The first call on a device looks up the array's address (cudaGetSymbolAddress) and, like any first launch, loads the
+ *     kernels; make that call outside stream capture.  Later calls only enqueue work on `cuda_stream`.
  * Errors: those of carve_fwd / carve_bwd, plus CARVE_ERR_STATIC_LIMIT.
  */
 #define CARVE_STATIC_SCRATCH_BYTES (16u << 20)
