@@ -171,7 +171,7 @@ carve_status_t carve_step_varlen(const carve_params_t *p, const void *q, const v
  *   scaled by 1/sqrt(mean(o^2) + eps) and by gain [H*dv] (float).  W_O is a dense GEMM outside the path.  Rows of at most
  *   8 KB (H*dv <= 4096 bf16 / 2048 fp32), else CARVE_ERR_SHAPE.  y may alias o.
  * carve_out_norm_bwd: d_o [B,T,H,dv] and dgain [H*dv] (float, overwritten) from dy [B,T,H,dv]; the statistics are
- *   recomputed from o.  `workspace`: carve_out_norm_workspace_bytes(p) bytes of scratch (per-warp partial sums of dgain,
+ *   recomputed from o.  `workspace`: carve_out_norm_workspace_bytes(p) bytes of scratch (per-block partial sums of dgain,
  *   added in a fixed order: results are run-to-run bitwise identical), CARVE_ERR_WORKSPACE if missing or too small.
  *   d_o may alias dy.
  */

@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(256) carve_out_norm_fwd_kernel(const void* __r
 }
 
 // Backward: d_o = r g dy - x r^3 mean(x g dy);  the warp's share of dgain = sum over its rows of dy x r, accumulated in a
-// shared-memory slice of the warp's own (no atomics) and written once as partial[warp][n] (summed in fixed order by
+// shared-memory slice of the warp's own (no atomics); the block's slices leave as one partial[block][n] (summed in fixed order by
 // carve_out_norm_dgain_kernel).  The row's pieces stay in registers in their 16-byte form between the two passes over the
 // row (statistics, then outputs): with 64 fewer accumulator registers and packed rows two blocks fit an SM.
 template <typename T> struct Raw;
@@ -267,17 +267,19 @@ carve_out_norm_bwd_kernel(const void* __restrict__ o, const float* __restrict__ 
                 Piece<T>::store(d_o, base + lane + 32 * i, out);
             }
     }
-    __syncwarp();
-    float* dst = partial + (size_t)warp * np * N;
-    for (int i = lane; i < np; i += 32) {
-        const float4* p4 = reinterpret_cast<const float4*>(sdg + (size_t)i * N);
-        float4* q4 = reinterpret_cast<float4*>(dst + (size_t)i * N);
-        q4[0] = p4[0];
-        if (N == 8) q4[1] = p4[1];
+    // the block's eight slices, added in warp order, leave as ONE partial per block
+    __syncthreads();
+    const int ncol = np * N;
+    float* dst = partial + (size_t)blockIdx.x * ncol;
+    for (int j = threadIdx.x; j < ncol; j += 256) {
+        float t = 0.f;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) t += sdg_all[(size_t)w * ncol + j];
+        dst[j] = t;
     }
 }
 
-// dgain[j] = sum over the warps' partials in a fixed order (run-to-run identical bits): a block owns 32 columns, its 32
+// dgain[j] = sum over the blocks' partials in a fixed order (run-to-run identical bits): a block owns 32 columns, its 32
 // warps each add a contiguous slice of the partials (128-byte coalesced reads), the slices are combined in slice order.
 __global__ void __launch_bounds__(1024) carve_out_norm_dgain_kernel(const float* __restrict__ partial, float* __restrict__ dgain,
                                                                     int n, int nwarps)
@@ -313,7 +315,7 @@ cudaError_t launch_norm(bool bwd, const void* o, const float* gain, const void* 
     kern<<<kNormBlocks, 256, smem, st>>>(o, gain, dy, out, partial, rows, np, 1.f / (float)n, eps);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    carve_out_norm_dgain_kernel<<<(n + 31) / 32, 1024, 0, st>>>(partial, dgain, n, kNormWarps);
+    carve_out_norm_dgain_kernel<<<(n + 31) / 32, 1024, 0, st>>>(partial, dgain, n, kNormBlocks);
     return cudaGetLastError();
 }
 
@@ -356,7 +358,7 @@ bool out_norm_supported(const carve_params_t& p)
     const size_t n = (size_t)p.H * p.dv, e = p.dtype == CARVE_BF16 ? 2 : 4;
     return n * e % 16 == 0 && n * e / 16 <= 32 * 16;
 }
-size_t out_norm_ws_bytes(const carve_params_t& p) { return (size_t)kNormWarps * p.H * p.dv * sizeof(float); }
+size_t out_norm_ws_bytes(const carve_params_t& p) { return (size_t)kNormBlocks * p.H * p.dv * sizeof(float); }
 
 cudaError_t out_norm_launch(const carve_params_t& p, bool bwd, const void* o, const float* gain, float eps, const void* dy,
                             void* out, float* partial, float* dgain, cudaStream_t st)
