@@ -743,11 +743,14 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
                 if (!qrole) {
                     const float bt = sBeta[tok];
 #pragma unroll
-                    for (int e = 0; e < 16; ++e) Mm[mm_idx(tok, 16 * jb + e)] = bt * __uint_as_float(v[e]);
+                    for (int e = 0; e < 16; e += 4)   // (mm_idx swizzles whole groups of four columns: 16-byte stores)
+                        *reinterpret_cast<float4*>(&Mm[mm_idx(tok, 16 * jb + e)]) =
+                            make_float4(bt * __uint_as_float(v[e]), bt * __uint_as_float(v[e + 1]), bt * __uint_as_float(v[e + 2]),
+                                        bt * __uint_as_float(v[e + 3]));
                 } else {
                     float f[16];
 #pragma unroll
-                    for (int e = 0; e < 16; ++e) f[e] = (16 * jb + e <= tok) ? __uint_as_float(v[e]) : 0.f;
+                    for (int e = 0; e < 16; ++e) f[e] = (e <= tok - 16 * jb) ? __uint_as_float(v[e]) : 0.f;
                     sts128(sm + Lo.TP + tile_chunk_off(128, 64 + tok, 2 * jb), pack8(f));
                     sts128(sm + Lo.TP + tile_chunk_off(128, 64 + tok, 2 * jb + 1), pack8(f + 8));
                     if (rc && !s1) {  // the record keeps scale.P in rows 0..63 (scale = 1: bulk copy of the tile)
