@@ -323,11 +323,11 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     if (tid == 0) { fence_async_smem(); issue_kq(0); issue_fb(0); issue_wv(0); }
 
     uint32_t mma_ph = 0, tma_ph = 0, acc_ph = 0;
-    // write strength of this thread's token, fetched one chunk ahead (a plain global load: its latency must not sit
-    // on the chunk's serial path)
-    // (kept as raw bf16 bits until it is used, one chunk later: converting it here would make the warp wait for the load)
+    // Write strength of this thread's token: fetched at the top of the chunk by an asynchronous 4-byte copy (the aligned
+    // word that holds the bf16 value) straight into the token's slot of mi.beta, and converted in place at the start of
+    // P5, long after it has landed.  No register carries it: as a plain load one chunk ahead its register was spilled, and
+    // the spill store waited for the load right there -- ~1.7 K cycles per chunk on the two warps everybody then waited for.
     const unsigned short* beta_bits = reinterpret_cast<const unsigned short*>(a.beta);
-    uint32_t beta_nx = (krole && half == 0 && live) ? (uint32_t)__ldg(beta_bits + ((size_t)b * a.T + t) * a.H + h) : 0u;
     PROF(g_prof_fwd, 38);   // one-time setup
     for (int c = 0; c < nchunks; ++c) {
         const bool fold_now = (c % gate_every) == 0;
@@ -367,10 +367,11 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
             }
             mi.nrm[row][half] = ss;
             if (krole && half == 0) {
-                // clamped away from 0 so that e_t = u_t / beta_t exists (u_t changes by < 1e-30 |e_t|)
-                const float bt = fmaxf(__uint_as_float(beta_nx << 16), 1e-30f);
-                if (c + 1 < nchunks) beta_nx = (uint32_t)__ldg(beta_bits + (tok0 + LCc + t) * a.H + h);
-                sBeta[t] = bt;
+                const unsigned short* src = beta_bits + (tok0 + t) * a.H + h;
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(&sBeta[t])),
+                             "l"(reinterpret_cast<uintptr_t>(src) & ~(uintptr_t)3)
+                             : "memory");
+                asm volatile("cp.async.commit_group;" ::: "memory");
             }
         }
         PROF(g_prof_fwd, 21);
@@ -423,7 +424,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROFB_ARRIVE(1); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 1);
         if (rc && tid == REC_TID) {   // record: the Vcat tile (its columns 32.. hold G^T) and the write strengths
             bulk_s2g(rc + Rc.GT, sb + Lo.Vcat, tile_bytes(DM, 64));
-            bulk_s2g(rc + Rc.beta, smem_u32(mi.beta), 256);
             bulk_commit();
         }
         if (warp == 0) {
@@ -490,6 +490,13 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         //      (a warp holds 32 consecutive tokens of one role), so log a never leaves the registers.
         float lg[16];
         const int cc0 = half * (HK / 8) + (krole ? 0 : HK / 16);
+        if (krole && half == 0 && live) {   // the write strength has landed (see above): bf16 half of its word -> float, in place
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            const uint32_t w = *reinterpret_cast<const volatile uint32_t*>(&sBeta[t]);
+            const bool hi = (((tok0 + t) * a.H + h) & 1) != 0;
+            // clamped away from 0 so that e_t = u_t / beta_t exists (u_t changes by < 1e-30 |e_t|)
+            sBeta[t] = fmaxf(__uint_as_float(hi ? (w & 0xFFFF0000u) : (w << 16)), 1e-30f);
+        }
         if (warp_active) {
             const int blk = t >> 4;
             uint32_t pr16[16], pw16[16];
@@ -564,6 +571,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         PROFB_ARRIVE(3); __syncthreads(); PROFB_AFTER(g_profb_fwd, 3);
         if (rc && tid == REC_TID) {   // record: exp of the block totals (blocks that do not exist at L < 64 hold 1)
             bulk_s2g(rc + Rc.etot, smem_u32(&mi.etot[0][0]), 16u * DK);
+            bulk_s2g(rc + Rc.beta, smem_u32(mi.beta), 256);
             bulk_commit();
         }
         PROF(g_prof_fwd, 8);
