@@ -102,15 +102,16 @@ __device__ __forceinline__ void diag8_inverse(const float* Mm, float* Tm, int n,
 // one product is ~30 cycles of latency against ~1 K for a tcgen05 round trip, which is why this 64 x 64 solve is not
 // on the tcgen05 pipe.  RHS = beta R comes from the bf16 row tile `rhs` ([64][DVC], ldmatrix.trans); U goes back as a
 // bf16 row tile (stmatrix.trans) over V', T into rows 0..63 of the 128-row tile `tp`.
-template <int DVC>
+template <int DVC, bool WANT_T>
 __device__ __forceinline__ void wy_solve(const float* Mm, const float* Tm, int n, int warp, int lane, uint32_t rhs_saddr,
-                                         uint32_t us_saddr, uint32_t tp_saddr, bool want_t)
+                                         uint32_t us_saddr, uint32_t tp_saddr)
 {
     constexpr int NUW = DVC / 16;   // warps solving for U
     const bool is_u = warp < NUW;
     const int m0 = is_u ? 16 * warp : 16 * (warp - NUW);
-    // (T only feeds the chunk record: an inference call skips it -- its warps share the tensor pipe with the U-warps)
-    if (!is_u && (!want_t || warp >= NUW + 4 || m0 >= n)) return;
+    // (T only feeds the chunk record: the inference kernel skips it -- its warps share the tensor pipe with the U-warps.
+    //  A compile-time switch: as a run-time flag it cost the training forward 3-5 % at config 2.)
+    if (!is_u && (!WANT_T || warp >= NUW + 4 || m0 >= n)) return;
     const int g = lane >> 2, l4 = lane & 3, nblk = n >> 3;
     const int mat = lane >> 3, lr = lane & 7;   // ldmatrix / stmatrix: this lane addresses row lr of matrix `mat`
     float x[8][4];
@@ -186,7 +187,8 @@ __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.w
 
 // SW = 1: scalar-write variant (wx = Uw = Vw = NULL, P l.145) -- w == 1, V' = v; compiled separately so that the full-gate
 // kernel carries none of its branches.
-template <int DK, int DV, int NP, int VS, int SW>
+// TRAIN = 1: the call writes chunk records (a.rec != NULL); only the WY solve depends on it at compile time.
+template <int DK, int DV, int NP, int VS, int SW, int TRAIN>
 __global__ void __launch_bounds__(128 * NP, DK == 64 ? 2 : 1)
 carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, const __grid_constant__ CUtensorMap mk,
                     const __grid_constant__ CUtensorMap mv, const __grid_constant__ CUtensorMap mf,
@@ -201,7 +203,6 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     // issues (and waits for) the record's bulk copies: lane 0 of a Q-side warp of the last column part, which has
     // little or nothing to do in the phases that follow the copies (P9a/P9b/P11), unlike the MMA-issuing thread 0
     constexpr int REC_TID = NTH - 64;
-    constexpr int T_TID = 32 * (DV / 16);   // lane 0 of the first T-warp of the WY solve: sends T to the chunk record
     constexpr int HK = DK / NP, HV = DV / NP;  // columns per warpgroup ("half" = part index 0..NP-1)
     extern __shared__ uint8_t smem_raw[];
     // 1024-byte alignment by an offset from the __shared__ array (not by integer rounding of a generic pointer), so
@@ -261,7 +262,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     const uint32_t tmem = mi.tmem_base;
     const size_t state_tile = tile_bytes(DV, DK);
     const Rec Rc(DK, DV);
-    uint8_t* rec_chain = a.rec ? a.rec + (size_t)chain * nchunks * Rc.total : nullptr;
+    // (the inference kernel sees a constant NULL here: all of the record code below compiles away)
+    uint8_t* rec_chain = (TRAIN && a.rec) ? a.rec + (size_t)chain * nchunks * Rc.total : nullptr;
     const bool s1 = a.scale == 1.f;   // then scale.P and scale.Qbar of the record are the shared-memory tiles themselves
 
     // initial state: fp32 -> TMEM, bf16 -> Sb (and the workspace slot of chunk 0)
@@ -568,7 +570,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         }
         PROF(g_prof_fwd, 6);
         if (tid == 0) bulk_wait_read();   // the output tile has left Y2 (rewritten below)
-        if (rc && (tid == REC_TID || tid == T_TID)) bulk_wait_read();   // the previous chunk's [P;T] copies have left TP (d = 64: rewritten below; else in P9)
+        if (rc && tid == REC_TID) bulk_wait_read();   // the previous chunk's [P;T] copy has left TP (d = 64: rewritten below; else in P9)
         fence_async_smem();   // (the block totals leave by a bulk copy)
         PROFB_ARRIVE(3); __syncthreads(); PROFB_AFTER(g_profb_fwd, 3);
         if (rc && tid == REC_TID) {   // record: exp of the block totals (blocks that do not exist at L < 64 hold 1)
@@ -854,52 +856,27 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         diag8_inverse(Mm, Tm, LCc, tid);
         PROFB_ARRIVE(6); __syncthreads(); PROFB_AFTER(g_profb_fwd, 6);
         PROF(g_prof_fwd, 26);
-        wy_solve<DV>(Mm, Tm, LCc, warp, lane, sb + Lo.Y2, sb + Lo.Us, sb + Lo.TP, rc != nullptr);
+        wy_solve<DV, TRAIN != 0>(Mm, Tm, LCc, warp, lane, sb + Lo.Y2, sb + Lo.Us, sb + Lo.TP);
         // the record copies issued so far have left their buffers: the next chunk's loads (P13) may overwrite them
         if (rc && tid == REC_TID) bulk_wait_read();
         PROF(g_prof_fwd, 13);
         // ---- P12: O += P U;  W = U^T Ktil -> TM_X2
-        // The four T-warps do not hold this barrier up: T only feeds the chunk record, and they finish later than the
-        // U-warps (measured: without them the forward is 5 % faster).  Everybody else meets on named barrier 1 and goes on
-        // to P12, leaving a non-blocking arrival on named barrier 3; the T-warps wait there for each other and for those
-        // arrivals (so every reader of the solve's scratch is done), then one of their threads sends T to the record and
-        // starts the next chunk's k|q load, which overwrites that scratch.
-        PROFB_ARRIVE(7);
-        fence_async_smem();
-        tc_fence_before();
-        if (rc) {
-            if (warp >= DV / 16 && warp < DV / 16 + 4) {
-                asm volatile("bar.sync 3, %0;" ::"n"(NTH) : "memory");
-                if (tid == T_TID) {
-                    bulk_s2g(rc + Rc.PT + 8192, sb + Lo.TP, 8192);
-                    bulk_commit();
-                    if (c + 1 < nchunks) issue_kq(c + 1);
-                }
-            } else {
-                asm volatile("bar.sync 1, %0;" ::"n"(NTH - 128) : "memory");
-                asm volatile("bar.arrive 3, %0;" ::"n"(NTH) : "memory");
-            }
-        } else {
-            __syncthreads();
-        }
-        tc_fence_after();
-        PROFB_AFTER(g_profb_fwd, 7);
+        PROFB_ARRIVE(7); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 7);
         PROF(g_prof_fwd, 22);
         if (warp == 0) {
             if (elect_one()) {
                 mma_rt<128, KMAJ, MNMAJ, LC>(tmem + TM_ACC, DV, sb + Lo.TP, 128, 0, sb + Lo.Us, 64, 0, LCc, true);
                 mma_rt<128, MNMAJ, MNMAJ, LC>(tmem + TM_X2, DK, sb + Lo.Us, 64, 0, sb + Lo.Ktil, 64, 0, LCc, false);
                 umma_commit(&mi.bar_mma);
-                // the inverse scratch (over the raw k|q tile) is consumed; a training call's T-warps may still read it:
-                // there the load is issued by their thread (above)
-                if (!rc && c + 1 < nchunks) issue_kq(c + 1);
+                if (c + 1 < nchunks) issue_kq(c + 1);   // the inverse scratch (over the raw k|q tile at d = 128) is consumed
             }
             __syncwarp();
         }
         if (rc && tid == REC_TID) {
-            // record scale.P (rows 64.. of TP go to rows 0.. of the record tile; T follows from the T-warps, above) and U
+            // record [scale.P ; T] (the two row halves of TP swapped; TP is next written in P9 of the next chunk) and U
             // (its buffer is refilled by the next chunk's loads, issued by this thread at the end of P13)
             if (s1) bulk_s2g(rc + Rc.PT, sb + Lo.TP + 8192, 8192);
+            bulk_s2g(rc + Rc.PT + 8192, sb + Lo.TP, 8192);
             bulk_s2g(rc + Rc.U, sb + Lo.Us, tile_bytes(64, DV));
             bulk_commit();
         }
@@ -972,7 +949,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
         bulk_commit();
         bulk_wait_all();
     }
-    if (rec_chain && (tid == 0 || tid == REC_TID || tid == T_TID)) bulk_wait_all();   // drain the record's bulk stores
+    if (rec_chain && (tid == 0 || tid == REC_TID)) bulk_wait_all();   // drain the record's bulk stores
     PROF(g_prof_fwd, 39);   // last output tile, drain
     PROF_FLUSH(g_prof_fwd)
     if (warp == 0) tmem_dealloc(tmem, TM_COLS);
@@ -1057,7 +1034,7 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
     t.O = static_cast<__nv_bfloat16*>(a.O); t.S_final = a.S_final; t.rec = rec;
     const size_t smem = tcp::Layout(D, D, 2 * a.r).total;
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
-    auto kern = carve_fwd_tc_kernel<D, D, NP, VS, SW>;
+    auto kern = rec ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 0>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100);   // (two CTAs per SM at d = 64)
