@@ -263,7 +263,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     const size_t state_tile = tile_bytes(DV, DK);
     const Rec Rc(DK, DV);
     // (the inference kernel sees a constant NULL here: all of the record code below compiles away)
-    uint8_t* rec_chain = (TRAIN && a.rec) ? a.rec + (size_t)chain * nchunks * Rc.total : nullptr;
+    uint8_t* rec_chain = TRAIN ? a.rec + (size_t)chain * nchunks * Rc.total : nullptr;
     const bool s1 = a.scale == 1.f;   // then scale.P and scale.Qbar of the record are the shared-memory tiles themselves
 
     // initial state: fp32 -> TMEM, bf16 -> Sb (and the workspace slot of chunk 0)
@@ -336,7 +336,8 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     for (int c = 0; c < nchunks; ++c) {
         const bool fold_now = (c % gate_every) == 0;
         const size_t tok0 = (size_t)b * a.T + (size_t)c * LCc;  // first token of the chunk
-        uint8_t* rc = rec_chain ? rec_chain + (size_t)c * Rc.total : nullptr;  // this chunk's record
+        uint8_t* rc = TRAIN ? rec_chain + (size_t)c * Rc.total : nullptr;  // this chunk's record
+        if (TRAIN) __builtin_assume(rc != nullptr);
         PROF(g_prof_fwd, 0);
         // ---- P0: fold G^T = S^T Ucat^T -> TM_X2[0, R2)
         PROFB_ARRIVE(0); PHASE_SYNC(); PROFB_AFTER(g_profb_fwd, 0);
