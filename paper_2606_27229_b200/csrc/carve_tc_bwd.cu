@@ -178,7 +178,9 @@ __device__ __forceinline__ void warp_colsum(float (&v)[N], int lane)
     } while (0)
 
 // NP = column parts per tile row = warpgroups per CTA (threads = 128 NP): 32 columns per thread.
-template <int D, int NP, int SW>   // SW = 1: scalar-write variant (w == 1), compiled separately
+// SW = 1: scalar-write variant (w == 1), compiled separately.  FULL = 1: the solve chunk has all 64 tokens (L >= 64), so
+// the live-row predicates and the anchor-block count are constants.
+template <int D, int NP, int SW, int FULL>
 __global__ void __launch_bounds__(128 * NP, 1)
 carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, const __grid_constant__ CUtensorMap mq,
                     const __grid_constant__ CUtensorMap mdq, const __grid_constant__ CUtensorMap mdk,
@@ -210,7 +212,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     const int t = row & 63;          // token of this row
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
     const int chain = blockIdx.x, b = chain / a.H, h = chain % a.H;
-    const int LCc = a.L < LC ? a.L : LC;
+    const int LCc = FULL ? LC : (a.L < LC ? a.L : LC);
     const int nchunks = a.T / LCc, nb = LCc >> 4, gate_every = a.L / LCc;
     const bool warp_active = (q & 1) * 32 < LCc;   // this warp holds at least one live token row
     const bool live = t < LCc;
@@ -1221,7 +1223,7 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
     t.flags = reinterpret_cast<int*>(ws + w.flags);
     const size_t smem = BLayout(D).total;
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
-    auto kern = carve_bwd_tc_kernel<D, NP, SW>;
+    auto kern = a.L >= tcp::LC ? carve_bwd_tc_kernel<D, NP, SW, 1> : carve_bwd_tc_kernel<D, NP, SW, 0>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int chains = a.B * a.H, nchunks = a.T / LCc;

@@ -187,8 +187,9 @@ __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.w
 
 // SW = 1: scalar-write variant (wx = Uw = Vw = NULL, P l.145) -- w == 1, V' = v; compiled separately so that the full-gate
 // kernel carries none of its branches.
-// TRAIN = 1: the call writes chunk records (a.rec != NULL); only the WY solve depends on it at compile time.
-template <int DK, int DV, int NP, int VS, int SW, int TRAIN>
+// TRAIN = 1: the call writes chunk records (a.rec != NULL).  FULL = 1: the solve chunk has all 64 tokens (L >= 64), so the
+// live-row predicates and the anchor-block count are constants (L < 64 runs the FULL = 0 instance).
+template <int DK, int DV, int NP, int VS, int SW, int TRAIN, int FULL>
 __global__ void __launch_bounds__(128 * NP, DK == 64 ? 2 : 1)
 carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, const __grid_constant__ CUtensorMap mk,
                     const __grid_constant__ CUtensorMap mv, const __grid_constant__ CUtensorMap mf,
@@ -226,7 +227,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     const int crank = VS > 1 ? (int)(blockIdx.x % VS) : 0;   // rank inside the cluster = which slice of value channels
     const int vofs = crank * DV;
     const int chain = blockIdx.x / VS, b = chain / a.H, h = chain % a.H;
-    const int LCc = a.L < LC ? a.L : LC;
+    const int LCc = FULL ? LC : (a.L < LC ? a.L : LC);
     const int nchunks = a.T / LCc, gate_every = a.L / LCc;
     const bool warp_active = (q & 1) * 32 < LCc;  // this warp holds at least one live token row
     const bool live = t < LCc;
@@ -1035,7 +1036,11 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
     t.O = static_cast<__nv_bfloat16*>(a.O); t.S_final = a.S_final; t.rec = rec;
     const size_t smem = tcp::Layout(D, D, 2 * a.r).total;
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
-    auto kern = rec ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 0>;
+    // FULL instance for L >= 64, except the d = 128 training kernel: there the specialised code was measured 7 % slower
+    // (48 instead of 16 bytes of spills at the 128-register cap), while it gains 8-19 % everywhere else
+    const bool full = a.L >= tcp::LC && !(rec && D == 128);
+    auto kern = rec ? (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 0>)
+                    : (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 0>);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100);   // (two CTAs per SM at d = 64)
