@@ -213,7 +213,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
     const int chain = blockIdx.x, b = chain / a.H, h = chain % a.H;
     const int LCc = FULL ? LC : (a.L < LC ? a.L : LC);
-    const int nchunks = a.T / LCc, nb = LCc >> 4, gate_every = a.L / LCc;
+    const int nchunks = a.T / LCc, nb = LCc >> 4, gate_every = FULL ? a.L / LCc : 1;   // (L < 64: one solve chunk per gate chunk)
     const bool warp_active = (q & 1) * 32 < LCc;   // this warp holds at least one live token row
     const bool live = t < LCc;
     const bool srow = row < D;                     // this thread owns a row of the state adjoint
