@@ -187,7 +187,7 @@ __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.w
 
 // SW = 1: scalar-write variant (wx = Uw = Vw = NULL, P l.145) -- w == 1, V' = v; compiled separately so that the full-gate
 // kernel carries none of its branches.
-// TRAIN = 1: the call writes chunk records (a.rec != NULL).  FULL = 1: the solve chunk has all 64 tokens (L >= 64), so the
+// TRAIN != 0: the call writes chunk records (a.rec != NULL); TRAIN = 1 when in addition scale == 1.  FULL = 1: the solve chunk has all 64 tokens (L >= 64), so the
 // live-row predicates and the anchor-block count are constants (L < 64 and the d = 128 training forward run the general
 // FULL = 0 instance).
 template <int DK, int DV, int NP, int VS, int SW, int TRAIN, int FULL>
@@ -266,7 +266,9 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     const Rec Rc(DK, DV);
     // (the inference kernel sees a constant NULL here: all of the record code below compiles away)
     uint8_t* rec_chain = TRAIN ? a.rec + (size_t)chain * nchunks * Rc.total : nullptr;
-    const bool s1 = a.scale == 1.f;   // then scale.P and scale.Qbar of the record are the shared-memory tiles themselves
+    // scale == 1 (TRAIN = 1; TRAIN = 2 is a training call with another scale): then scale.P and scale.Qbar of the record
+    // are the shared-memory tiles themselves, and the per-thread stores of the general case compile away
+    const bool s1 = TRAIN == 1 ? true : a.scale == 1.f;
 
     // initial state: fp32 -> TMEM, bf16 -> Sb (and the workspace slot of chunk 0)
     if (row < DV) {
@@ -1040,8 +1042,10 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
     // FULL instance for L >= 64, except the d = 128 training kernel: there the specialised code was measured 7 % slower
     // (48 instead of 16 bytes of spills at the 128-register cap), while it gains 8-19 % everywhere else
     const bool full = a.L >= tcp::LC && !(rec && D == 128);
-    auto kern = rec ? (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 0>)
-                    : (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 0>);
+    const bool one = a.scale == 1.f;
+    auto kern = !rec ? (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 0>)
+                : one ? (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 0>)
+                      : (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 2, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 2, 0>);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100);   // (two CTAs per SM at d = 64)
