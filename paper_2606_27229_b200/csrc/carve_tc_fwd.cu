@@ -1041,7 +1041,7 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
     // FULL instance for L >= 64, except the d = 128 training kernel: there the specialised code was measured 7 % slower
     // (48 instead of 16 bytes of spills at the 128-register cap), while it gains 8-19 % everywhere else
-    const bool full = a.L >= tcp::LC && !(rec && D == 128);
+    const bool full = a.L >= tcp::LC && !(rec && D == 128 && a.scale != 1.f);
     const bool one = a.scale == 1.f;
     auto kern = !rec ? (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 0>)
                 : one ? (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 0>)
