@@ -1043,9 +1043,14 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
     // (48 instead of 16 bytes of spills at the 128-register cap), while it gains 8-19 % everywhere else
     const bool full = a.L >= tcp::LC && !(rec && D == 128 && a.scale != 1.f);
     const bool one = a.scale == 1.f;
-    auto kern = !rec ? (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 0>)
-                : one ? (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 0>)
-                      : (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 2, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 2, 0>);
+    auto kern = full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 0>;
+    if constexpr (VS == 1) {   // (the value-split cluster is inference only: no training instances of it are compiled)
+        if (rec)
+            kern = one ? (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 0>)
+                       : (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 2, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 2, 0>);
+    } else if (rec) {
+        return cudaErrorInvalidValue;
+    }
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100);   // (two CTAs per SM at d = 64)
