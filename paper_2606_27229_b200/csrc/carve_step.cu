@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
     float* sU = sA + DK;               // [DV] u_t
     float* sW = sU + DV;               // [DV] w_t v_t
     float* sT = sW + DV;               // [R2] tanh bottleneck
-    float* sRed = sT + 64;             // [2] 1/|q|, 1/|k|
+    float* sRed = sT + 64;             // [2] 1/|q|, 1/|k|;  [2..3] the state load's mbarrier;  [4] beta of the token
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int chain = blockIdx.x, b = chain / a.H, h = chain % a.H;
@@ -61,11 +61,21 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
     const int n = a.cu ? min(max(__ldg(a.cu + b + 1) - tok0, 0), a.n) : a.n;
     if (n == 0) return;
 
-    for (int i = tid; i < DV * DK / 4; i += NT) {
-        const int x = i / (DK / 4), j4 = i % (DK / 4);
-        st4s(sS + x * SP + 4 * j4, ldg4(gS + (size_t)i * 4));
+    // The state comes in by bulk copies, one per row (the rows are padded in shared memory), all in flight at once and
+    // asynchronous: the staging of Ucat^T and of the first token's inputs below runs under them.  (As per-thread loads
+    // the 64 KB cost a chain of load round trips per thread; ncu: 5.2 long-scoreboard stalls per issue, 11 % of the DRAM peak.)
+    uint64_t* sbar = reinterpret_cast<uint64_t*>(sRed + 2);
+    const uint32_t sbar_a = (uint32_t)__cvta_generic_to_shared(sbar);
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(sbar_a));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(sbar_a), "r"((uint32_t)(DV * DK * 4)) : "memory");
     }
     __syncthreads();
+    for (int x = tid; x < DV; x += NT)
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"((uint32_t)__cvta_generic_to_shared(sS + x * SP)), "l"(gS + (size_t)x * DK), "r"((uint32_t)(DK * 4)), "r"(sbar_a)
+                     : "memory");
     // fold: G[i][j] = sum_x Ucat[i][x] S[x][j]   (once per call: the gates of all n tokens read the incoming state).
     // Ucat^T is staged in shared memory ([x][i]); a thread owns one key channel j and 8 bottleneck rows, so that one
     // state read feeds 8 FMAs (the first version read the state once per FMA and was 2.2x slower end to end).
@@ -73,6 +83,44 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
     for (int o = tid; o < R2 * DV; o += NT) {
         const int i = o / DV, x = o % DV;
         sUt[x * R2 + i] = i < r ? __ldg(a.Ub + (size_t)i * DV + x) : (a.Uw ? __ldg(a.Uw + (size_t)(i - r) * DV + x) : 0.f);
+    }
+    // token inputs are staged in shared memory one token ahead of their use: all of a token's loads are in flight together
+    // (q, k, f, bx: DK each; v, wx: DV each), instead of one exposed load round trip in each of the six phases of a token
+    float* sIn = sUt + DV * R2;        // [4 DK + 2 DV]: q | k | f | bx | v | wx (raw)
+    constexpr int NIN = (4 * DK + 2 * DV + NT - 1) / NT;   // staged values per thread
+    float in_r[NIN], beta_r = 0.f;
+    auto load_token = [&](int t2) {   // global loads of token t2 into registers (all in flight together)
+        const size_t tok2 = ((size_t)tok0 + t2) * a.H + h;
+#pragma unroll
+        for (int u = 0; u < NIN; ++u) {
+            const int j = tid + u * NT;
+            float vv = 0.f;
+            if (j < DK) vv = ldf<T>(gq, tok2 * DK + j);
+            else if (j < 2 * DK) vv = ldf<T>(gk, tok2 * DK + (j - DK));
+            else if (j < 3 * DK) vv = ldf<T>(gf, tok2 * DK + (j - 2 * DK));
+            else if (j < 4 * DK) vv = ldf<T>(gbx, tok2 * DK + (j - 3 * DK));
+            else if (j < 4 * DK + DV) vv = ldf<T>(gv, tok2 * DV + (j - 4 * DK));
+            else if (j < 4 * DK + 2 * DV) vv = gwx ? ldf<T>(gwx, tok2 * DV + (j - 4 * DK - DV)) : 0.f;
+            in_r[u] = vv;
+        }
+        if (tid == 0) beta_r = ldf<T>(gbeta, tok2);
+    };
+    auto store_token = [&]() {
+#pragma unroll
+        for (int u = 0; u < NIN; ++u) {
+            const int j = tid + u * NT;
+            if (j < 4 * DK + 2 * DV) sIn[j] = in_r[u];
+        }
+        if (tid == 0) sRed[4] = beta_r;
+    };
+    load_token(0);
+    store_token();
+    // wait for the state
+    {
+        uint32_t done = 0;
+        while (!done)
+            asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                         : "=r"(done) : "r"(sbar_a) : "memory");
     }
     __syncthreads();
     for (int o = tid; o < DK * (R2 / 8); o += NT) {
@@ -94,18 +142,19 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
 
     for (int t = 0; t < n; ++t) {
         const size_t tok = ((size_t)tok0 + t) * a.H + h;
+        const float *iq = sIn, *ik = sIn + DK, *if_ = sIn + 2 * DK, *ibx = sIn + 3 * DK, *iv = sIn + 4 * DK, *iwx = sIn + 4 * DK + DV;
         // q^, k^ (D1)
         if (warp < 2) {
-            const T* src = warp == 0 ? gq : gk;
+            const float* src = warp == 0 ? iq : ik;
             float ss = 0.f;
-            for (int j = lane; j < DK; j += 32) { const float x = ldf<T>(src, tok * DK + j); ss = fmaf(x, x, ss); }
+            for (int j = lane; j < DK; j += 32) { const float x = src[j]; ss = fmaf(x, x, ss); }
             ss = warp_sum(ss);
             if (lane == 0) sRed[warp] = a.l2norm ? rsqrtf(ss + a.eps) : 1.f;
         }
         __syncthreads();
         for (int j = tid; j < 2 * DK; j += NT) {
-            if (j < DK) sQ[j] = ldf<T>(gq, tok * DK + j) * sRed[0];
-            else sK[j - DK] = ldf<T>(gk, tok * DK + (j - DK)) * sRed[1];
+            if (j < DK) sQ[j] = iq[j] * sRed[0];
+            else sK[j - DK] = ik[j - DK] * sRed[1];
         }
         __syncthreads();
         // tt = tanh(G q^) (Eq. 7)
@@ -119,26 +168,27 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
         // gates (Eq. 8-9): a_t = exp(g)(1 - b), w_t v_t
         for (int j = tid; j < DK + DV; j += NT) {
             if (j < DK) {
-                float pre = ldf<T>(gbx, tok * DK + j);
+                float pre = ibx[j];
                 for (int i = 0; i < r; ++i) pre = fmaf(__ldg(a.Vb + (size_t)j * r + i), sT[i], pre);
                 const float eA = a.A ? expf(__ldg(a.A + h * DK + j)) : 1.f;
                 const float ta = a.tau ? __ldg(a.tau + h * DK + j) : 0.f;
-                const float g = -eA * softplusf(ldf<T>(gf, tok * DK + j) + ta);
+                const float g = -eA * softplusf(if_[j] + ta);
                 sA[j] = expf(g - softplusf(pre));          // exp(g) (1 - sigmoid(pre)),  log(1 - sigmoid(x)) = -softplus(x)
             } else {
                 const int x = j - DK;
                 float w = 1.f;   // scalar-write variant (wx = NULL, P l.145)
                 if (gwx) {
-                    float pre = ldf<T>(gwx, tok * DV + x);
+                    float pre = iwx[x];
                     for (int i = 0; i < r; ++i) pre = fmaf(__ldg(a.Vw + (size_t)x * r + i), sT[r + i], pre);
                     w = sigmoidf_(pre);
                 }
-                sW[x] = w * ldf<T>(gv, tok * DV + x);
+                sW[x] = w * iv[x];
             }
         }
         __syncthreads();
+        const float beta = sRed[4];
+        if (t + 1 < n) load_token(t + 1);   // the next token's inputs: in flight under the two state phases below
         // u_t = beta (w v - S k^): two threads per state row, half of the key channels each
-        const float beta = ldf<T>(gbeta, tok);
         for (int p = tid; p < 2 * DV; p += NT) {
             const int x = p >> 1, hf = p & 1;
             const float* srow = sS + x * SP + hf * (DK / 2);
@@ -171,6 +221,7 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
             acc += __shfl_xor_sync(0xffffffffu, acc, 1);
             if (hf == 0) stf<T>(gO, tok * DV + x, a.scale * acc);
         }
+        if (t + 1 < n) store_token();
         __syncthreads();
     }
     for (int i = tid; i < DV * DK / 4; i += NT) {
@@ -182,7 +233,7 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
 template <typename T, int DK, int DV>
 cudaError_t launch_step(const StepArgs& a, cudaStream_t st)
 {
-    const size_t smem = ((size_t)(DV + 2 * a.r) * (DK + 4) + 3 * DK + 2 * DV + 64 + 8 + (size_t)DV * 2 * a.r) * sizeof(float);
+    const size_t smem = ((size_t)(DV + 2 * a.r) * (DK + 4) + 3 * DK + 2 * DV + 64 + 8 + (size_t)DV * 2 * a.r + 4 * DK + 2 * DV) * sizeof(float);
     auto kern = carve_step_kernel<T, DK, DV>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
