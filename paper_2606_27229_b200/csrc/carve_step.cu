@@ -80,9 +80,26 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
     // Ucat^T is staged in shared memory ([x][i]); a thread owns one key channel j and 8 bottleneck rows, so that one
     // state read feeds 8 FMAs (the first version read the state once per FMA and was 2.2x slower end to end).
     float* sUt = sRed + 8;             // [DV][R2]
-    for (int o = tid; o < R2 * DV; o += NT) {
-        const int i = o / DV, x = o % DV;
-        sUt[x * R2 + i] = i < r ? __ldg(a.Ub + (size_t)i * DV + x) : (a.Uw ? __ldg(a.Uw + (size_t)(i - r) * DV + x) : 0.f);
+    // (16-byte loads, four in flight per thread: as one scalar load per loop trip this staging was 17 % of the kernel)
+    for (int o0 = tid; o0 < R2 * DV / 4; o0 += 4 * NT) {
+        float4 u4[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int o = o0 + u * NT, i = o / (DV / 4), x4 = o % (DV / 4);
+            u4[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (o < R2 * DV / 4) {
+                if (i < r) u4[u] = ldg4(a.Ub + (size_t)i * DV + 4 * x4);
+                else if (a.Uw) u4[u] = ldg4(a.Uw + (size_t)(i - r) * DV + 4 * x4);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int o = o0 + u * NT, i = o / (DV / 4), x4 = o % (DV / 4);
+            if (o < R2 * DV / 4) {
+                sUt[(4 * x4 + 0) * R2 + i] = u4[u].x; sUt[(4 * x4 + 1) * R2 + i] = u4[u].y;
+                sUt[(4 * x4 + 2) * R2 + i] = u4[u].z; sUt[(4 * x4 + 3) * R2 + i] = u4[u].w;
+            }
+        }
     }
     // token inputs are staged in shared memory one token ahead of their use: all of a token's loads are in flight together
     // (q, k, f, bx: DK each; v, wx: DV each), instead of one exposed load round trip in each of the six phases of a token
@@ -123,20 +140,23 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
                          : "=r"(done) : "r"(sbar_a) : "memory");
     }
     __syncthreads();
-    for (int o = tid; o < DK * (R2 / 8); o += NT) {
-        const int j = o % DK, i0 = 8 * (o / DK);
-        float acc[8];
+    // a thread owns two key channels (j, j + DK/2) and 8 bottleneck rows: 16 FMAs per two state reads and two broadcast
+    // 16-byte reads of Ucat^T (the loop is bound by shared-memory instructions, not by the FMA pipe)
+    for (int o = tid; o < (DK / 2) * (R2 / 8); o += NT) {
+        const int j = o % (DK / 2), i0 = 8 * (o / (DK / 2));
+        float acc[2][8];
 #pragma unroll
-        for (int e = 0; e < 8; ++e) acc[e] = 0.f;
-#pragma unroll 4
+        for (int e = 0; e < 8; ++e) acc[0][e] = acc[1][e] = 0.f;
+#pragma unroll 8
         for (int x = 0; x < DV; ++x) {
-            const float sv = sS[x * SP + j];
+            const float s0 = sS[x * SP + j], s1 = sS[x * SP + j + DK / 2];
             const float4 u0 = ld4s(sUt + x * R2 + i0), u1 = ld4s(sUt + x * R2 + i0 + 4);
-            acc[0] = fmaf(u0.x, sv, acc[0]); acc[1] = fmaf(u0.y, sv, acc[1]); acc[2] = fmaf(u0.z, sv, acc[2]); acc[3] = fmaf(u0.w, sv, acc[3]);
-            acc[4] = fmaf(u1.x, sv, acc[4]); acc[5] = fmaf(u1.y, sv, acc[5]); acc[6] = fmaf(u1.z, sv, acc[6]); acc[7] = fmaf(u1.w, sv, acc[7]);
+            const float uu[8] = {u0.x, u0.y, u0.z, u0.w, u1.x, u1.y, u1.z, u1.w};
+#pragma unroll
+            for (int e = 0; e < 8; ++e) { acc[0][e] = fmaf(uu[e], s0, acc[0][e]); acc[1][e] = fmaf(uu[e], s1, acc[1][e]); }
         }
 #pragma unroll
-        for (int e = 0; e < 8; ++e) sG[(i0 + e) * SP + j] = acc[e];
+        for (int e = 0; e < 8; ++e) { sG[(i0 + e) * SP + j] = acc[0][e]; sG[(i0 + e) * SP + j + DK / 2] = acc[1][e]; }
     }
     __syncthreads();
 
