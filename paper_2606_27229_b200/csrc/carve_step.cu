@@ -79,7 +79,8 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
     // fold: G[i][j] = sum_x Ucat[i][x] S[x][j]   (once per call: the gates of all n tokens read the incoming state).
     // Ucat^T is staged in shared memory ([x][i]); a thread owns one key channel j and 8 bottleneck rows, so that one
     // state read feeds 8 FMAs (the first version read the state once per FMA and was 2.2x slower end to end).
-    float* sUt = sRed + 8;             // [DV][R2]
+    float* sUt = sRed + 8;             // [DV][RP], RP = R2 + 4: the transposing stores below hit 8 banks instead of one
+    const int RP = R2 + 4;
     // (16-byte loads, four in flight per thread: as one scalar load per loop trip this staging was 17 % of the kernel)
     for (int o0 = tid; o0 < R2 * DV / 4; o0 += 4 * NT) {
         float4 u4[4];
@@ -96,14 +97,14 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
         for (int u = 0; u < 4; ++u) {
             const int o = o0 + u * NT, i = o / (DV / 4), x4 = o % (DV / 4);
             if (o < R2 * DV / 4) {
-                sUt[(4 * x4 + 0) * R2 + i] = u4[u].x; sUt[(4 * x4 + 1) * R2 + i] = u4[u].y;
-                sUt[(4 * x4 + 2) * R2 + i] = u4[u].z; sUt[(4 * x4 + 3) * R2 + i] = u4[u].w;
+                sUt[(4 * x4 + 0) * RP + i] = u4[u].x; sUt[(4 * x4 + 1) * RP + i] = u4[u].y;
+                sUt[(4 * x4 + 2) * RP + i] = u4[u].z; sUt[(4 * x4 + 3) * RP + i] = u4[u].w;
             }
         }
     }
     // token inputs are staged in shared memory one token ahead of their use: all of a token's loads are in flight together
     // (q, k, f, bx: DK each; v, wx: DV each), instead of one exposed load round trip in each of the six phases of a token
-    float* sIn = sUt + DV * R2;        // [4 DK + 2 DV]: q | k | f | bx | v | wx (raw)
+    float* sIn = sUt + DV * RP;        // [4 DK + 2 DV]: q | k | f | bx | v | wx (raw)
     constexpr int NIN = (4 * DK + 2 * DV + NT - 1) / NT;   // staged values per thread
     float in_r[NIN], beta_r = 0.f;
     auto load_token = [&](int t2) {   // global loads of token t2 into registers (all in flight together)
@@ -150,7 +151,7 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
 #pragma unroll 8
         for (int x = 0; x < DV; ++x) {
             const float s0 = sS[x * SP + j], s1 = sS[x * SP + j + DK / 2];
-            const float4 u0 = ld4s(sUt + x * R2 + i0), u1 = ld4s(sUt + x * R2 + i0 + 4);
+            const float4 u0 = ld4s(sUt + x * RP + i0), u1 = ld4s(sUt + x * RP + i0 + 4);
             const float uu[8] = {u0.x, u0.y, u0.z, u0.w, u1.x, u1.y, u1.z, u1.w};
 #pragma unroll
             for (int e = 0; e < 8; ++e) { acc[0][e] = fmaf(uu[e], s0, acc[0][e]); acc[1][e] = fmaf(uu[e], s1, acc[1][e]); }
@@ -253,7 +254,7 @@ __global__ void __launch_bounds__(NT, 1) carve_step_kernel(const StepArgs a)
 template <typename T, int DK, int DV>
 cudaError_t launch_step(const StepArgs& a, cudaStream_t st)
 {
-    const size_t smem = ((size_t)(DV + 2 * a.r) * (DK + 4) + 3 * DK + 2 * DV + 64 + 8 + (size_t)DV * 2 * a.r + 4 * DK + 2 * DV) * sizeof(float);
+    const size_t smem = ((size_t)(DV + 2 * a.r) * (DK + 4) + 3 * DK + 2 * DV + 64 + 8 + (size_t)DV * (2 * a.r + 4) + 4 * DK + 2 * DV) * sizeof(float);
     auto kern = carve_step_kernel<T, DK, DV>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
