@@ -212,8 +212,8 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     const int t = row & 63;          // token of this row
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
     const int chain = blockIdx.x, b = chain / a.H, h = chain % a.H;
-    const int LCc = FULL ? LC : (a.L < LC ? a.L : LC);
-    const int nchunks = a.T / LCc, nb = LCc >> 4, gate_every = FULL ? a.L / LCc : 1;   // (L < 64: one solve chunk per gate chunk)
+    const int LCc = FULL == 1 ? LC : FULL > 1 ? FULL : (a.L < LC ? a.L : LC);   // (FULL = 16, 32: that chunk length)
+    const int nchunks = a.T / LCc, nb = LCc >> 4, gate_every = FULL == 1 ? a.L / LCc : 1;   // (L < 64: one solve chunk per gate chunk)
     const bool warp_active = (q & 1) * 32 < LCc;   // this warp holds at least one live token row
     const bool live = t < LCc;
     const bool srow = row < D;                     // this thread owns a row of the state adjoint
@@ -1224,6 +1224,10 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
     const size_t smem = BLayout(D).total;
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
     auto kern = a.L >= tcp::LC ? carve_bwd_tc_kernel<D, NP, SW, 1> : carve_bwd_tc_kernel<D, NP, SW, 0>;
+    if constexpr (D == 128 && SW == 0) {   // config 2's short chunks: the chunk length as a constant as well
+        if (a.L == 16) kern = carve_bwd_tc_kernel<D, NP, SW, 16>;
+        if (a.L == 32) kern = carve_bwd_tc_kernel<D, NP, SW, 32>;
+    }
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int chains = a.B * a.H, nchunks = a.T / LCc;

@@ -228,7 +228,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     const int crank = VS > 1 ? (int)(blockIdx.x % VS) : 0;   // rank inside the cluster = which slice of value channels
     const int vofs = crank * DV;
     const int chain = blockIdx.x / VS, b = chain / a.H, h = chain % a.H;
-    const int LCc = FULL ? LC : (a.L < LC ? a.L : LC);
+    const int LCc = FULL == 1 ? LC : FULL > 1 ? FULL : (a.L < LC ? a.L : LC);   // (FULL = 16, 32: that chunk length)
     const int nchunks = a.T / LCc, gate_every = a.L / LCc;   // (a constant here was measured 4 % slower at d = 64)
     const bool warp_active = (q & 1) * 32 < LCc;  // this warp holds at least one live token row
     const bool live = t < LCc;
@@ -1050,6 +1050,12 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
                        : (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 2, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 2, 0>);
     } else if (rec) {
         return cudaErrorInvalidValue;
+    }
+    if constexpr (D == 128 && VS == 1 && SW == 0) {   // config 2's short chunks: the chunk length as a constant as well
+        if (a.L == 16 && !rec) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 16>;
+        if (a.L == 32 && !rec) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 32>;
+        if (a.L == 16 && rec && one) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 16>;
+        if (a.L == 32 && rec && one) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 32>;
     }
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
