@@ -180,7 +180,8 @@ __device__ __forceinline__ void warp_colsum(float (&v)[N], int lane)
 // NP = column parts per tile row = warpgroups per CTA (threads = 128 NP): 32 columns per thread.
 // SW = 1: scalar-write variant (w == 1), compiled separately.  FULL = 1: the solve chunk has all 64 tokens (L >= 64), so
 // the live-row predicates and the anchor-block count are constants.
-template <int D, int NP, int SW, int FULL>
+// RT != 0: the gate rank r as a constant of the instance (the configs' r = 16 at d = 128, r = 8 at d = 64, full chunks).
+template <int D, int NP, int SW, int FULL, int RT = 0>
 __global__ void __launch_bounds__(128 * NP, 1)
 carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, const __grid_constant__ CUtensorMap mq,
                     const __grid_constant__ CUtensorMap mdq, const __grid_constant__ CUtensorMap mdk,
@@ -204,7 +205,7 @@ carve_bwd_tc_kernel(const BwdArgs a, const __grid_constant__ CUtensorMap mdO, co
     const BLayout Lo(D);
     BMisc& mi = *reinterpret_cast<BMisc*>(sm + Lo.misc);
     const uint32_t sb = smem_u32(sm);
-    const int r = a.r, R2 = 2 * r;
+    const int r = RT ? RT : a.r, R2 = 2 * r;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, q = warp & 3, half = warp >> 2;
     const int row = q * 32 + lane;   // tile row == TMEM lane served by this thread
@@ -1227,6 +1228,9 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
     if constexpr (D == 128 && SW == 0) {   // config 2's short chunks: the chunk length as a constant as well
         if (a.L == 16) kern = carve_bwd_tc_kernel<D, NP, SW, 16>;
         if (a.L == 32) kern = carve_bwd_tc_kernel<D, NP, SW, 32>;
+    }
+    if constexpr (SW == 0) {
+        if (a.L >= tcp::LC && a.r == (D == 128 ? 16 : 8)) kern = carve_bwd_tc_kernel<D, NP, SW, 1, (D == 128 ? 16 : 8)>;
     }
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

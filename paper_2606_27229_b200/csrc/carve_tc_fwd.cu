@@ -190,7 +190,7 @@ __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.w
 // TRAIN != 0: the call writes chunk records (a.rec != NULL); TRAIN = 1 when in addition scale == 1.  FULL = 1: the solve chunk has all 64 tokens (L >= 64), so the
 // live-row predicates and the anchor-block count are constants (L < 64 and the d = 128 training forward run the general
 // FULL = 0 instance).
-template <int DK, int DV, int NP, int VS, int SW, int TRAIN, int FULL>
+template <int DK, int DV, int NP, int VS, int SW, int TRAIN, int FULL, int RT = 0>   // RT != 0: the gate rank r as a constant
 __global__ void __launch_bounds__(128 * NP, DK == 64 ? 2 : 1)
 carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, const __grid_constant__ CUtensorMap mk,
                     const __grid_constant__ CUtensorMap mv, const __grid_constant__ CUtensorMap mf,
@@ -211,7 +211,7 @@ carve_fwd_tc_kernel(const TcArgs a, const __grid_constant__ CUtensorMap mq, cons
     // that the compiler still knows these are shared-memory addresses: LDS/STS with 32-bit address arithmetic
     // instead of generic LD/ST with 64-bit arithmetic.
     uint8_t* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    const int r = a.r, R2 = 2 * r;
+    const int r = RT ? RT : a.r, R2 = 2 * r;
     const Layout Lo(DK, DV, R2);
     using Misc = MiscT<DK>;
     Misc& mi = *reinterpret_cast<Misc*>(sm + Lo.misc);
@@ -1050,6 +1050,11 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
                        : (full ? carve_fwd_tc_kernel<D, D, NP, VS, SW, 2, 1> : carve_fwd_tc_kernel<D, D, NP, VS, SW, 2, 0>);
     } else if (rec) {
         return cudaErrorInvalidValue;
+    }
+    if constexpr (VS == 1 && SW == 0) {   // the configs' rank (r = 16 at d = 128, r = 8 at d = 64), full chunks, scale = 1
+        constexpr int RC = D == 128 ? 16 : 8;
+        if (full && a.r == RC && !rec) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 1, RC>;
+        if (full && a.r == RC && rec && one) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 1, RC>;
     }
     if constexpr (D == 128 && VS == 1 && SW == 0) {   // config 2's short chunks: the chunk length as a constant as well
         if (a.L == 16 && !rec) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 16>;
