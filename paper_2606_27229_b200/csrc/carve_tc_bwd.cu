@@ -1226,12 +1226,10 @@ cudaError_t launch_tc_bwd(const Args& a, uint8_t* ws, const TcWsLayout& w, float
     constexpr int NP = D / 32;   // 32 columns per thread: 256 threads at d = 64, 512 at d = 128
     auto kern = a.L >= tcp::LC ? carve_bwd_tc_kernel<D, NP, SW, 1> : carve_bwd_tc_kernel<D, NP, SW, 0>;
     if constexpr (D == 128 && SW == 0) {   // config 2's short chunks: the chunk length as a constant as well
-        if (a.L == 16) kern = carve_bwd_tc_kernel<D, NP, SW, 16>;
-        if (a.L == 32) kern = carve_bwd_tc_kernel<D, NP, SW, 32>;
+        if (a.L == 16 && a.r == 16) kern = carve_bwd_tc_kernel<D, NP, SW, 16, 16>;
+        if (a.L == 32 && a.r == 16) kern = carve_bwd_tc_kernel<D, NP, SW, 32, 16>;
     }
-    if constexpr (SW == 0) {
-        if (a.L >= tcp::LC && a.r == (D == 128 ? 16 : 8)) kern = carve_bwd_tc_kernel<D, NP, SW, 1, (D == 128 ? 16 : 8)>;
-    }
+    if (a.L >= tcp::LC && a.r == (D == 128 ? 16 : 8)) kern = carve_bwd_tc_kernel<D, NP, SW, 1, (D == 128 ? 16 : 8)>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int chains = a.B * a.H, nchunks = a.T / LCc;

@@ -1051,16 +1051,20 @@ static cudaError_t launch_tc_fwd(const Args& a, uint8_t* rec, cudaStream_t st)
     } else if (rec) {
         return cudaErrorInvalidValue;
     }
-    if constexpr (VS == 1 && SW == 0) {   // the configs' rank (r = 16 at d = 128, r = 8 at d = 64), full chunks, scale = 1
+    {   // the configs' rank (r = 16 at d = 128, r = 8 at d = 64) as a constant: full chunks, scale = 1
         constexpr int RC = D == 128 ? 16 : 8;
         if (full && a.r == RC && !rec) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 1, RC>;
-        if (full && a.r == RC && rec && one) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 1, RC>;
+        if constexpr (VS == 1) {
+            if (full && a.r == RC && rec && one) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 1, RC>;
+        }
     }
     if constexpr (D == 128 && VS == 1 && SW == 0) {   // config 2's short chunks: the chunk length as a constant as well
-        if (a.L == 16 && !rec) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 16>;
-        if (a.L == 32 && !rec) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 32>;
-        if (a.L == 16 && rec && one) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 16>;
-        if (a.L == 32 && rec && one) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 32>;
+        if (a.r == 16) {
+            if (a.L == 16 && !rec) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 16, 16>;
+            if (a.L == 32 && !rec) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 0, 32, 16>;
+            if (a.L == 16 && rec && one) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 16, 16>;
+            if (a.L == 32 && rec && one) kern = carve_fwd_tc_kernel<D, D, NP, VS, SW, 1, 32, 16>;
+        }
     }
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
