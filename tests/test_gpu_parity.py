@@ -234,6 +234,33 @@ def test_tensor_path_scale_and_no_l2norm(oracle):
     _check_fwd_bwd(oracle, cfg, x, path=carve.CARVE_PATH_TENSOR)
 
 
+@pytest.mark.parametrize("dk,r,L,scale", [(128, 8, 64, 1.0), (128, 8, 16, 1.0), (128, 16, 64, 0.5), (128, 16, 32, 0.5),
+                                          (128, 16, 128, 0.5), (64, 16, 64, 1.0), (64, 8, 64, 0.5), (64, 8, 32, 1.0)])
+def test_tensor_path_general_instances(oracle, dk, r, L, scale):
+    """The tensor-path kernels compile as specialised instances (full 64-token chunks, the configs' rank r = 16 at
+    d = 128 / r = 8 at d = 64, scale = 1, chunk lengths 16 and 32 at d = 128) next to general ones of the same source:
+    these cases -- another rank, another scale -- run the general instances, forward + backward."""
+    cfg = synth.Config("t", B=1, H=2, T=256, L=L, dk=dk, dv=dk, r=r, dtype="bf16", wstd=0.1, s0_std=0.05, scale=scale,
+                       seed=dk + r + L)
+    x = synth.scale_qk_rows(synth.make_inputs(cfg, with_decay_params=True), cfg)
+    _check_fwd_bwd(oracle, cfg, x, path=carve.CARVE_PATH_TENSOR)
+
+
+@pytest.mark.parametrize("dk,dv,r,L", [(128, 128, 16, 64), (128, 128, 8, 64), (128, 128, 16, 16), (64, 64, 8, 64), (64, 64, 16, 32),
+                                       (128, 256, 16, 64), (128, 256, 8, 32)])
+def test_tensor_path_inference_instances(oracle, dk, dv, r, L):
+    """Forward without workspace (the inference kernel: no T solve, no record code) in its specialised and general
+    instances, including the two-CTA value split at d_v = 256."""
+    cfg = synth.Config("t", B=1, H=2, T=256, L=L, dk=dk, dv=dv, r=r, dtype="bf16", wstd=0.1, s0_std=0.05, fwd_only=True,
+                       seed=dk + dv + r + L)
+    x = synth.scale_qk_rows(synth.make_inputs(cfg, with_decay_params=True), cfg)
+    p = params_of(cfg, path=carve.CARVE_PATH_TENSOR)
+    assert carve.carve_resolved_path(p, False) == carve.CARVE_PATH_TENSOR
+    O, Sf, _ = run_fwd(p, x, need_bwd=False)
+    O_ref, S_ref = oracle.fwd(oracle_shape(oracle, cfg), x)
+    assert relerr(O, O_ref) <= 2e-2 and relerr(Sf, S_ref) <= 2e-2
+
+
 def test_tensor_path_determinism(oracle):
     cfg = synth.Config("t", B=2, H=3, T=256, L=64, dk=128, dv=128, r=16, dtype="bf16", wstd=0.1, seed=12)
     x, ct = synth.make_inputs(cfg), synth.make_cotangents(cfg)
